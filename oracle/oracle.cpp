@@ -1,0 +1,1232 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY.
+//
+// A plain, slow, obviously-correct CPU statement of the HARM conservative update of ideal
+// GR-MHD that the cuHARM paper (arXiv 2205.02484) describes.  It exists to CHECK the CUDA
+// library; it is not a product path.  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may build, load or call it.  It shares no code, header,
+// table or helper with paper_2205_02484_b200/ (the CUDA path) and neither includes the other.
+//
+// Citations: "P:L<n>" = /root/reference/PAPER.md line n (with the equation it falls in);
+// "A<n>" = a reading of the paper listed in DESIGN.md (where the text is silent or garbled).
+//
+// Arithmetic: IEEE fp64, built with -O2 -ffp-contract=off (no FMA contraction), no blocking,
+// no fusion, no reordering beyond what the equations state.  OpenMP `parallel for` over the
+// outermost zone index is used only so that the timed CPU baseline can use all host cores; every
+// zone's arithmetic is independent of the thread count.
+//
+// Pins (tests/test_oracle_*.py, all `-m "not gpu"`): see the table in DESIGN.md.  Parts whose
+// conventions are fixed by DESIGN.md rather than by the paper or by mathematics are marked
+// "parity unpinned" at the function that implements them.
+
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#include <algorithm>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+extern "C" {
+
+// Same field order as the library's parameter block, declared independently (no shared header).
+struct oracle_params {
+  int32_t struct_bytes;
+  int32_t n1, n2, n3, ng;
+  int32_t coords;  // 0 = MKS (eq. 39), 1 = Minkowski-Cartesian (A39)
+  double a, gam;
+  double r_in, r_out, R0, hslope;
+  double xmin[3], xmax[3];
+  int32_t recon;    // 0 = PLM+MC (eqs. 15-16), 1 = PPM (A20)
+  int32_t riemann;  // 0 = LLF (eq. 17), 1 = HLL (eq. 20)
+  int32_t bc_x1, bc_x2, bc_x3;  // 0 outflow(+inflow check in MKS X1), 1 periodic, 2 polar-reflect, 3 fixed
+  double rho_fl_coef, rho_fl_pow, rho_fl_abs;
+  double u_fl_coef, u_fl_pow, u_fl_abs;
+  double sigma_max, b2_over_u_max, gamma_max;
+  double newton_tol;
+  int32_t newton_maxit, newton_extra;
+  int32_t fixup_max_passes;
+  int32_t reserved;
+};
+
+}  // extern "C"
+
+namespace {
+
+const double PI = 3.14159265358979323846;
+
+// ------------------------------------------------------------------------------------------
+// C-1  Coordinates (eq. 39; A14: the sine argument is pi(1+Y), not pi(1+Y)/2).
+// ------------------------------------------------------------------------------------------
+struct Coord {
+  double r, th, drdX, dthdY, d2thdY2;
+};
+
+Coord coord_map(const oracle_params& p, double X1, double X2) {
+  Coord c;
+  if (p.coords == 1) {  // Minkowski: unused
+    c.r = 1.0; c.th = 0.5 * PI; c.drdX = 1.0; c.dthdY = 1.0; c.d2thdY2 = 0.0;
+    return c;
+  }
+  c.r = p.R0 + std::exp(X1);
+  c.drdX = c.r - p.R0;
+  double arg = PI * (1.0 + X2);
+  c.th = 0.5 * PI * (1.0 + X2) + 0.5 * (1.0 - p.hslope) * std::sin(arg);
+  c.dthdY = 0.5 * PI * (1.0 + (1.0 - p.hslope) * std::cos(arg));
+  c.d2thdY2 = -0.5 * PI * PI * (1.0 - p.hslope) * std::sin(arg);
+  return c;
+}
+
+struct Geom {
+  double gcov[4][4], gcon[4][4], sqrtg, alpha;
+};
+
+// ------------------------------------------------------------------------------------------
+// C-2  Metric (eq. 38), MKS components by the diagonal Jacobian J=(1,r',th',1).
+// Inverse from the KS closed form; sqrt(-g) = Sigma |sin th| |r'| |th'|.
+// polar_face != 0: A32 — the 2-face lies exactly on the axis: sqrt(-g) := 0; sin^2 floored.
+// ------------------------------------------------------------------------------------------
+void ks_cov(double a, double r, double th, double g[4][4]) {
+  double s = std::sin(th), c = std::cos(th);
+  double s2 = s * s;
+  double Sig = r * r + a * a * c * c;  // the paper's rho^2
+  double f = 2.0 * r / Sig;
+  for (int m = 0; m < 4; m++) for (int n = 0; n < 4; n++) g[m][n] = 0.0;
+  g[0][0] = -1.0 + f;
+  g[0][1] = g[1][0] = f;
+  g[0][3] = g[3][0] = -a * s2 * f;
+  g[1][1] = 1.0 + f;
+  g[1][3] = g[3][1] = -a * s2 * (1.0 + f);
+  g[2][2] = Sig;
+  g[3][3] = s2 * (Sig + a * a * s2 * (1.0 + f));
+}
+
+void metric_at(const oracle_params& p, double X1, double X2, int polar_face, Geom& G) {
+  for (int m = 0; m < 4; m++) for (int n = 0; n < 4; n++) { G.gcov[m][n] = 0.0; G.gcon[m][n] = 0.0; }
+  if (p.coords == 1) {
+    G.gcov[0][0] = -1.0; G.gcon[0][0] = -1.0;
+    for (int i = 1; i < 4; i++) { G.gcov[i][i] = 1.0; G.gcon[i][i] = 1.0; }
+    G.sqrtg = 1.0; G.alpha = 1.0;
+    return;
+  }
+  Coord c = coord_map(p, X1, X2);
+  double a = p.a;
+  double gks[4][4];
+  ks_cov(a, c.r, c.th, gks);
+  double J[4] = {1.0, c.drdX, c.dthdY, 1.0};
+  for (int m = 0; m < 4; m++) for (int n = 0; n < 4; n++) G.gcov[m][n] = J[m] * J[n] * gks[m][n];
+  double s = std::sin(c.th), co = std::cos(c.th);
+  double s2 = s * s;
+  if (s2 < 1e-30) s2 = 1e-30;  // A32
+  double Sig = c.r * c.r + a * a * co * co;
+  double f = 2.0 * c.r / Sig;
+  double Del = c.r * c.r - 2.0 * c.r + a * a;
+  double ik[4][4];
+  for (int m = 0; m < 4; m++) for (int n = 0; n < 4; n++) ik[m][n] = 0.0;
+  ik[0][0] = -(1.0 + f);
+  ik[0][1] = ik[1][0] = f;
+  ik[1][1] = Del / Sig;
+  ik[1][3] = ik[3][1] = a / Sig;
+  ik[2][2] = 1.0 / Sig;
+  ik[3][3] = 1.0 / (Sig * s2);
+  for (int m = 0; m < 4; m++) for (int n = 0; n < 4; n++) G.gcon[m][n] = ik[m][n] / (J[m] * J[n]);
+  G.sqrtg = Sig * std::fabs(s) * std::fabs(c.drdX) * std::fabs(c.dthdY);
+  if (polar_face) G.sqrtg = 0.0;  // A32: every 2-flux through the axis is exactly zero
+  G.alpha = 1.0 / std::sqrt(-G.gcon[0][0]);
+}
+
+// ------------------------------------------------------------------------------------------
+// Connection coefficients (A19: closed-form derivatives of eq. 38 pushed through the
+// Jacobian).  conn[l][n][k] = Gamma^l_{n k} = 1/2 g^{l s} (d_n g_{s k} + d_k g_{s n} - d_s g_{n k}).
+// ------------------------------------------------------------------------------------------
+void conn_at(const oracle_params& p, double X1, double X2, double conn[4][4][4]) {
+  for (int l = 0; l < 4; l++) for (int n = 0; n < 4; n++) for (int k = 0; k < 4; k++) conn[l][n][k] = 0.0;
+  if (p.coords == 1) return;
+  Coord c = coord_map(p, X1, X2);
+  double a = p.a, r = c.r, th = c.th;
+  double s = std::sin(th), co = std::cos(th);
+  double s2 = s * s;
+  double Sig = r * r + a * a * co * co;
+  double f = 2.0 * r / Sig;
+  // derivatives of Sigma and f = 2r/Sigma
+  double dSig_r = 2.0 * r, dSig_t = -2.0 * a * a * s * co;
+  double df_r = 2.0 / Sig - 2.0 * r * dSig_r / (Sig * Sig);
+  double df_t = -2.0 * r * dSig_t / (Sig * Sig);
+  double ds2_t = 2.0 * s * co;
+  // KS metric and its r- and theta-derivatives
+  double g[4][4], dgr[4][4], dgt[4][4];
+  ks_cov(a, r, th, g);
+  for (int m = 0; m < 4; m++) for (int n = 0; n < 4; n++) { dgr[m][n] = 0.0; dgt[m][n] = 0.0; }
+  dgr[0][0] = df_r;                      dgt[0][0] = df_t;
+  dgr[0][1] = dgr[1][0] = df_r;          dgt[0][1] = dgt[1][0] = df_t;
+  dgr[0][3] = dgr[3][0] = -a * s2 * df_r;
+  dgt[0][3] = dgt[3][0] = -a * (ds2_t * f + s2 * df_t);
+  dgr[1][1] = df_r;                      dgt[1][1] = df_t;
+  dgr[1][3] = dgr[3][1] = -a * s2 * df_r;
+  dgt[1][3] = dgt[3][1] = -a * (ds2_t * (1.0 + f) + s2 * df_t);
+  dgr[2][2] = dSig_r;                    dgt[2][2] = dSig_t;
+  // g_phiphi = s2 * (Sig + a^2 s2 (1+f))
+  dgr[3][3] = s2 * (dSig_r + a * a * s2 * df_r);
+  dgt[3][3] = ds2_t * (Sig + a * a * s2 * (1.0 + f)) + s2 * (dSig_t + a * a * (ds2_t * (1.0 + f) + s2 * df_t));
+  // MKS: gM_{mn} = J_m J_n g_{mn};  dJ_1/dX = r' (since r' = r - R0),  dJ_2/dY = th''
+  double J[4] = {1.0, c.drdX, c.dthdY, 1.0};
+  double dJ1[4] = {0.0, c.drdX, 0.0, 0.0};     // d J_m / dX
+  double dJ2[4] = {0.0, 0.0, c.d2thdY2, 0.0};  // d J_m / dY
+  double dg[4][4][4];                          // dg[s][k][n] = d_n gM_{s k}
+  for (int m = 0; m < 4; m++) for (int n = 0; n < 4; n++) {
+    dg[m][n][0] = 0.0;
+    dg[m][n][3] = 0.0;
+    dg[m][n][1] = (dJ1[m] * J[n] + J[m] * dJ1[n]) * g[m][n] + J[m] * J[n] * dgr[m][n] * c.drdX;
+    dg[m][n][2] = (dJ2[m] * J[n] + J[m] * dJ2[n]) * g[m][n] + J[m] * J[n] * dgt[m][n] * c.dthdY;
+  }
+  Geom G;
+  metric_at(p, X1, X2, 0, G);
+  for (int l = 0; l < 4; l++)
+    for (int n = 0; n < 4; n++)
+      for (int k = 0; k < 4; k++) {
+        double sum = 0.0;
+        for (int sg = 0; sg < 4; sg++) sum += G.gcon[l][sg] * (dg[sg][k][n] + dg[sg][n][k] - dg[n][k][sg]);
+        conn[l][n][k] = 0.5 * sum;
+      }
+}
+
+// ------------------------------------------------------------------------------------------
+// C-3  Primitive -> fluid state at one metric location (eq. 10).
+// prim = (rho, u, ut1, ut2, ut3, B1, B2, B3).
+// ------------------------------------------------------------------------------------------
+struct State {
+  double ucon[4], ucov[4], bcon[4], bcov[4], bsq, lorentz;
+};
+
+void fluid_state(const double prim[8], const Geom& G, State& S) {
+  double qsq = 0.0;
+  for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) qsq += G.gcov[i][j] * prim[1 + i] * prim[1 + j];
+  double lor = std::sqrt(1.0 + qsq);
+  S.lorentz = lor;
+  double alpha = G.alpha;
+  S.ucon[0] = lor / alpha;
+  for (int i = 1; i < 4; i++) {
+    double beta_i = G.gcon[0][i] * alpha * alpha;
+    S.ucon[i] = prim[1 + i] - lor * beta_i / alpha;  // eq. 10
+  }
+  for (int m = 0; m < 4; m++) {
+    double v = 0.0;
+    for (int n = 0; n < 4; n++) v += G.gcov[m][n] * S.ucon[n];
+    S.ucov[m] = v;
+  }
+  double bt = 0.0;
+  for (int i = 1; i < 4; i++) bt += prim[4 + i] * S.ucov[i];  // b^t = B^i u^mu g_{i mu}
+  S.bcon[0] = bt;
+  for (int i = 1; i < 4; i++) S.bcon[i] = (prim[4 + i] + bt * S.ucon[i]) / S.ucon[0];
+  for (int m = 0; m < 4; m++) {
+    double v = 0.0;
+    for (int n = 0; n < 4; n++) v += G.gcov[m][n] * S.bcon[n];
+    S.bcov[m] = v;
+  }
+  double b2 = 0.0;
+  for (int m = 0; m < 4; m++) b2 += S.bcon[m] * S.bcov[m];
+  S.bsq = b2;
+}
+
+// mixed stress tensor T^m_n (eq. 5 with one index lowered)
+void stress_mixed(const double prim[8], const State& S, double gam, double T[4][4]) {
+  double rho = prim[0], u = prim[1];
+  double p = (gam - 1.0) * u;
+  double w = rho + u + p;
+  for (int m = 0; m < 4; m++)
+    for (int n = 0; n < 4; n++) {
+      double delta = (m == n) ? 1.0 : 0.0;
+      T[m][n] = (w + S.bsq) * S.ucon[m] * S.ucov[n] + (p + 0.5 * S.bsq) * delta - S.bcon[m] * S.bcov[n];
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// C-4  Conserved variables (dir = 0) and fluxes (dir = 1,2,3)  (eqs. 6-8, P:L78-88;
+// A1: induction flux sqrt(-g)(b^i u^d - b^d u^i); A18: energy variable is sqrt(-g) T^t_t).
+// ------------------------------------------------------------------------------------------
+void flux_vector(const double prim[8], const State& S, const Geom& G, double gam, int dir, double out[8]) {
+  double T[4][4];
+  stress_mixed(prim, S, gam, T);
+  out[0] = G.sqrtg * prim[0] * S.ucon[dir];
+  for (int n = 0; n < 4; n++) out[1 + n] = G.sqrtg * T[dir][n];
+  for (int i = 1; i < 4; i++) out[4 + i] = G.sqrtg * (S.bcon[i] * S.ucon[dir] - S.bcon[dir] * S.ucon[i]);
+}
+
+// ------------------------------------------------------------------------------------------
+// C-6  Wave speeds from the quadratic dispersion relation (eqs. 18-19).
+// Roots of A v^2 + B v + C = 0, c1 >= c2.  A29: negative discriminant clamped to 0.
+// ------------------------------------------------------------------------------------------
+void wave_speeds(const double prim[8], const State& S, const Geom& G, double gam, int dir, double* c1, double* c2) {
+  double rho = prim[0], u = prim[1];
+  double p = (gam - 1.0) * u;
+  double w = rho + u + p;
+  double cs2 = gam * p / w;               // eq. 19
+  double va2 = S.bsq / (S.bsq + w);
+  double cms2 = va2 + cs2 * (1.0 - va2);  // eq. 18
+  double ut = S.ucon[0], ud = S.ucon[dir];
+  double A = ut * ut - cms2 * (G.gcon[0][0] + ut * ut);
+  double B = -2.0 * (ut * ud - cms2 * (G.gcon[0][dir] + ut * ud));
+  double C = ud * ud - cms2 * (G.gcon[dir][dir] + ud * ud);
+  double disc = B * B - 4.0 * A * C;
+  if (disc < 0.0) disc = 0.0;
+  double sq = std::sqrt(disc);
+  double ra = (-B + sq) / (2.0 * A);
+  double rb = (-B - sq) / (2.0 * A);
+  *c1 = (ra > rb) ? ra : rb;
+  *c2 = (ra > rb) ? rb : ra;
+}
+
+// ------------------------------------------------------------------------------------------
+// C-5  Reconstruction.  MC-limited slope (eq. 15; A2: signed last branch).
+// ------------------------------------------------------------------------------------------
+double slope_mc(double qm, double q0, double qp) {
+  double dm = q0 - qm, dp = qp - q0;
+  if (dm * dp < 0.0) return 0.0;
+  double dc = 0.5 * (qp - qm);
+  if (std::fabs(dm) < std::fabs(dp) && 2.0 * std::fabs(dm) < std::fabs(dc)) return 2.0 * dm;
+  if (2.0 * std::fabs(dp) < std::fabs(dc)) return 2.0 * dp;
+  return dc;
+}
+
+// Values of one variable at the lower (l) and upper (r) faces of the cell y[2], seen from inside
+// that cell, from the 5 cell values y[0..4] centred on it.
+// recon 0: PLM, eq. 16.  recon 1: PPM, A20 = basic Colella-Woodward (1984):
+// MC-limited slopes, 4th-order interface values, monotonisation; no steepening / flattening.
+void recon_cell(int recon, const double y[5], double* l, double* r) {
+  if (recon == 0) {
+    double dq = slope_mc(y[1], y[2], y[3]);
+    *l = y[2] - 0.5 * dq;
+    *r = y[2] + 0.5 * dq;
+    return;
+  }
+  double dm = slope_mc(y[0], y[1], y[2]);
+  double d0 = slope_mc(y[1], y[2], y[3]);
+  double dp = slope_mc(y[2], y[3], y[4]);
+  double ql = 0.5 * (y[1] + y[2]) - (d0 - dm) / 6.0;
+  double qr = 0.5 * (y[2] + y[3]) - (dp - d0) / 6.0;
+  double yc = y[2];
+  if ((qr - yc) * (yc - ql) <= 0.0) {
+    ql = yc; qr = yc;
+  } else {
+    double d = qr - ql;
+    double m6 = d * (yc - 0.5 * (ql + qr));
+    double lim = d * d / 6.0;
+    if (m6 > lim) ql = 3.0 * yc - 2.0 * qr;
+    else if (m6 < -lim) qr = 3.0 * yc - 2.0 * ql;
+  }
+  *l = ql; *r = qr;
+}
+
+// ------------------------------------------------------------------------------------------
+// C-6  Riemann flux at one face from the two reconstructed states and the FACE metric
+// (P:L139-161).  LLF eq. 17; HLL eq. 20 (A30: denominator guarded).
+// ------------------------------------------------------------------------------------------
+void face_flux(const double pl[8], const double pr[8], const Geom& G, double gam, int dir, int riemann,
+               double Fbar[8], double* cw_out) {
+  State Sl, Sr;
+  fluid_state(pl, G, Sl);
+  fluid_state(pr, G, Sr);
+  double Ul[8], Ur[8], Fl[8], Fr[8];
+  flux_vector(pl, Sl, G, gam, 0, Ul);
+  flux_vector(pr, Sr, G, gam, 0, Ur);
+  flux_vector(pl, Sl, G, gam, dir, Fl);
+  flux_vector(pr, Sr, G, gam, dir, Fr);
+  double c1l, c2l, c1r, c2r;
+  wave_speeds(pl, Sl, G, gam, dir, &c1l, &c2l);
+  wave_speeds(pr, Sr, G, gam, dir, &c1r, &c2r);
+  double cmax = std::max(0.0, std::max(c1r, c1l));
+  double cmin = std::max(0.0, std::max(-c2r, -c2l));
+  double cw = std::max(cmax, cmin);
+  *cw_out = cw;
+  for (int v = 0; v < 8; v++) {
+    if (riemann == 0) {
+      Fbar[v] = 0.5 * (Fl[v] + Fr[v] - cw * (Ur[v] - Ul[v]));  // eq. 17
+    } else {
+      double den = std::max(cmax + cmin, 1e-300);
+      Fbar[v] = (cmax * Fl[v] + cmin * Fr[v] - cmax * cmin * (Ur[v] - Ul[v])) / den;  // eq. 20
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// C-8  Source S_nu = sqrt(-g) T^k_l Gamma^l_{nu k} at the centre (eq. 7, eq. 14).
+// ------------------------------------------------------------------------------------------
+void source_term(const double prim[8], const Geom& G, const double conn[4][4][4], double gam, double S[4]) {
+  State st;
+  fluid_state(prim, G, st);
+  double T[4][4];
+  stress_mixed(prim, st, gam, T);
+  for (int nu = 0; nu < 4; nu++) {
+    double sum = 0.0;
+    for (int k = 0; k < 4; k++) for (int l = 0; l < 4; l++) sum += T[k][l] * conn[l][nu][k];
+    S[nu] = G.sqrtg * sum;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// C-10  Noble 2D inversion (eqs. 27-31; A6 sign of eq. 30; A7 D = alpha rho u^t;
+// A8 Newton policy).  Returns 0 = ok or a failure code; on failure the fluid primitives are the
+// guess.  B^i = U_B / sqrt(-g) always.
+//   1: D <= 0 or non-finite input   2: no convergence in maxit   3: W <= 0 or non-finite
+//   4: v^2 outside [0,1)            5: rho <= 0                  6: u < 0
+// ------------------------------------------------------------------------------------------
+int invert_2d(const double U[8], const Geom& G, double gam, double prim[8], double tol, int maxit, int extra,
+              int* iters_out) {
+  double guess[8];
+  for (int v = 0; v < 8; v++) guess[v] = prim[v];
+  *iters_out = 0;
+  double alpha = G.alpha, sg = G.sqrtg;
+  for (int i = 1; i < 4; i++) prim[4 + i] = U[4 + i] / sg;
+  double D = alpha * U[0] / sg;
+  double Qcov[4], Bc[4];
+  for (int m = 0; m < 4; m++) Qcov[m] = alpha * U[1 + m] / sg;
+  Bc[0] = 0.0;
+  for (int i = 1; i < 4; i++) Bc[i] = alpha * U[4 + i] / sg;
+  bool finite_in = std::isfinite(D);
+  for (int m = 0; m < 4; m++) finite_in = finite_in && std::isfinite(Qcov[m]) && std::isfinite(Bc[m]);
+  if (!finite_in || !(D > 0.0)) return 1;
+  double Qcon[4];
+  for (int m = 0; m < 4; m++) {
+    double v = 0.0;
+    for (int n = 0; n < 4; n++) v += G.gcon[m][n] * Qcov[n];
+    Qcon[m] = v;
+  }
+  double Bsq = 0.0;
+  for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) Bsq += G.gcov[i][j] * Bc[i] * Bc[j];
+  double QdotB = 0.0;
+  for (int i = 1; i < 4; i++) QdotB += Qcov[i] * Bc[i];
+  double ncon[4];
+  ncon[0] = 1.0 / alpha;
+  for (int i = 1; i < 4; i++) ncon[i] = -alpha * G.gcon[0][i];
+  double Qdotn = 0.0;
+  for (int m = 0; m < 4; m++) Qdotn += Qcov[m] * ncon[m];
+  double Qsq = 0.0;
+  for (int m = 0; m < 4; m++) Qsq += Qcon[m] * Qcov[m];
+  double Qtsq = Qsq + Qdotn * Qdotn;
+  double QdB2 = QdotB * QdotB;
+  double gfac = (gam - 1.0) / gam;
+  // initial guess (A8, A35)
+  double qsq = 0.0;
+  for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) qsq += G.gcov[i][j] * guess[1 + i] * guess[1 + j];
+  double W = (1.0 + qsq) * (guess[0] + gam * guess[1]);
+  double v2 = 0.0;
+  for (int tries = 0; tries < 400; tries++) {
+    v2 = (Qtsq + QdB2 * (Bsq + 2.0 * W) / (W * W)) / ((Bsq + W) * (Bsq + W));
+    if (v2 < 1.0) break;
+    W *= 10.0;
+  }
+  if (!(v2 < 1.0) || !(W > 0.0)) return 3;
+  if (v2 < 0.0) v2 = 0.0;
+  bool converged = false;
+  int extra_left = -1;
+  int it = 0;
+  for (it = 1; it <= maxit; it++) {
+    double W2 = W * W, W3 = W2 * W;
+    double omv = 1.0 - v2;
+    double sq = std::sqrt(omv);
+    double pg = gfac * (W * omv - D * sq);  // eq. 31
+    double f1 = Qtsq - v2 * (Bsq + W) * (Bsq + W) + QdB2 * (Bsq + 2.0 * W) / W2;  // eq. 29
+    double f2 = -Qdotn - 0.5 * Bsq * (1.0 + v2) + QdB2 / (2.0 * W2) - W + pg;      // eq. 30 (A6)
+    double j11 = -2.0 * (Bsq + W) * (v2 + QdB2 / W3);
+    double j12 = -(Bsq + W) * (Bsq + W);
+    double j21 = -1.0 - QdB2 / W3 + gfac * omv;
+    double j22 = -0.5 * Bsq + gfac * (-W + D / (2.0 * sq));
+    double det = j11 * j22 - j12 * j21;
+    double dW = (-f1 * j22 + f2 * j12) / det;
+    double dv = (-f2 * j11 + f1 * j21) / det;
+    double Wn = std::fabs(W + dW);
+    double vn = v2 + dv;
+    if (vn < 0.0) vn = 0.0;
+    if (vn > 1.0 - 1e-15) vn = 1.0 - 1e-15;
+    double err = (Wn == 0.0) ? std::fabs(dW) : std::fabs(dW / Wn);
+    W = Wn; v2 = vn;
+    if (!std::isfinite(W) || !std::isfinite(v2)) { *iters_out = it; return 3; }
+    if (extra_left < 0) {
+      if (err <= tol) { extra_left = extra; }
+    } else {
+      extra_left--;
+    }
+    if (extra_left == 0) { converged = true; break; }
+  }
+  *iters_out = (it > maxit) ? maxit : it;
+  if (!converged) return 2;
+  if (!(W > 0.0)) return 3;
+  if (!(v2 >= 0.0 && v2 < 1.0)) return 4;
+  double lor = 1.0 / std::sqrt(1.0 - v2);
+  double rho = D / lor;
+  double w = W * (1.0 - v2);
+  double u = (w - rho) / gam;
+  if (!(rho > 0.0)) return 5;
+  if (!(u >= 0.0)) return 6;
+  prim[0] = rho;
+  prim[1] = u;
+  for (int i = 1; i < 4; i++) {
+    double Qt = Qcon[i] + ncon[i] * Qdotn;
+    prim[1 + i] = lor * (Qt + QdotB * Bc[i] / W) / (W + Bsq);
+  }
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------
+// C-12  Floors (eqs. 35-37; A9-A12).  "parity unpinned" for the ceiling mechanism
+// (A11) — the paper gives no formula; post-conditions and idempotence are pinned.
+// Returns a bit mask: 1 rho floor, 2 u floor, 4 ceiling applied, 8 Lorentz cap, 16 ceiling
+// re-inversion failed (additive fallback used).
+// ------------------------------------------------------------------------------------------
+int apply_floors(const oracle_params& p, double r, const Geom& G, double prim[8]) {
+  int mask = 0;
+  double rfl = std::max(p.rho_fl_abs, p.rho_fl_coef * std::pow(r, p.rho_fl_pow));
+  double ufl = std::max(p.u_fl_abs, p.u_fl_coef * std::pow(r, p.u_fl_pow));
+  if (prim[0] < rfl) { prim[0] = rfl; mask |= 1; }
+  if (prim[1] < ufl) { prim[1] = ufl; mask |= 2; }
+  if (p.sigma_max > 0.0 || p.b2_over_u_max > 0.0) {
+    State S;
+    fluid_state(prim, G, S);
+    double drho = 0.0, du = 0.0;
+    if (p.sigma_max > 0.0) drho = std::max(0.0, S.bsq / p.sigma_max - prim[0]);
+    if (p.b2_over_u_max > 0.0) du = std::max(0.0, S.bsq / p.b2_over_u_max - prim[1]);
+    if (drho > 0.0 || du > 0.0) {
+      mask |= 4;
+      double U[8], Uadd[8];
+      flux_vector(prim, S, G, p.gam, 0, U);
+      double padd[8] = {drho, du, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};  // at rest in the normal-observer frame
+      State Sa;
+      fluid_state(padd, G, Sa);
+      flux_vector(padd, Sa, G, p.gam, 0, Uadd);
+      for (int v = 0; v < 8; v++) U[v] += Uadd[v];
+      double trial[8];
+      for (int v = 0; v < 8; v++) trial[v] = prim[v];
+      int iters;
+      int flag = invert_2d(U, G, p.gam, trial, p.newton_tol, p.newton_maxit, p.newton_extra, &iters);
+      if (flag == 0) {
+        for (int v = 0; v < 5; v++) prim[v] = trial[v];
+      } else {
+        prim[0] += drho; prim[1] += du; mask |= 16;
+      }
+      // the injection slows the fluid, which raises b^2 a little: enforce eqs. 36-37 exactly with a final
+      // clamp at fixed velocity (b^2 does not depend on rho, u at fixed utilde^i, B^i)
+      State S2;
+      fluid_state(prim, G, S2);
+      if (p.sigma_max > 0.0) prim[0] = std::max(prim[0], S2.bsq / p.sigma_max);
+      if (p.b2_over_u_max > 0.0) prim[1] = std::max(prim[1], S2.bsq / p.b2_over_u_max);
+    }
+  }
+  if (p.gamma_max > 0.0) {
+    double qsq = 0.0;
+    for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) qsq += G.gcov[i][j] * prim[1 + i] * prim[1 + j];
+    double lor = std::sqrt(1.0 + qsq);
+    if (lor > p.gamma_max) {
+      double fac = std::sqrt((p.gamma_max * p.gamma_max - 1.0) / (lor * lor - 1.0));  // A12
+      for (int i = 1; i < 4; i++) prim[1 + i] *= fac;
+      mask |= 8;
+    }
+  }
+  return mask;
+}
+
+// ------------------------------------------------------------------------------------------
+// Grid context
+// ------------------------------------------------------------------------------------------
+struct Ctx {
+  oracle_params p;
+  int n1g, n2g, n3g, ng;
+  size_t nz;  // zones per variable, extended grid
+  double dx[3], x0[3];
+  std::vector<Geom> gc, gf1, gf2;   // centre, 1-face (i-1/2,j), 2-face (i,j-1/2); index i*n2g+j
+  std::vector<double> conn;         // [i*n2g+j][4][4][4]
+  std::vector<double> rc;           // r at centre
+  double* prim;                     // bound, caller-owned
+  std::vector<double> F[3], E[3], Phalf, Pnew, cw[3];
+  std::vector<int32_t> flag;
+  int64_t stats[8];
+  double cwmax[3];
+
+  size_t idx(int i, int j, int k) const { return ((size_t)i * n2g + j) * n3g + k; }
+  size_t vidx(int v, int i, int j, int k) const { return (size_t)v * nz + idx(i, j, k); }
+};
+
+void get_prim(const Ctx& c, const double* P, int i, int j, int k, double out[8]) {
+  for (int v = 0; v < 8; v++) out[v] = P[c.vidx(v, i, j, k)];
+}
+
+const Geom& geom_face(const Ctx& c, int dir, int i, int j) {
+  if (dir == 1) return c.gf1[(size_t)i * c.n2g + j];
+  if (dir == 2) return c.gf2[(size_t)i * c.n2g + j];
+  return c.gc[(size_t)i * c.n2g + j];  // the metric is phi-independent: 3-faces == centres
+}
+
+void build_geometry(Ctx& c) {
+  const oracle_params& p = c.p;
+  size_t n = (size_t)c.n1g * c.n2g;
+  c.gc.resize(n); c.gf1.resize(n); c.gf2.resize(n);
+  c.conn.assign(n * 64, 0.0);
+  c.rc.assign(n, 1.0);
+  for (int i = 0; i < c.n1g; i++)
+    for (int j = 0; j < c.n2g; j++) {
+      int I = i - c.ng, J = j - c.ng;
+      double X1c = c.x0[0] + (I + 0.5) * c.dx[0], X2c = c.x0[1] + (J + 0.5) * c.dx[1];
+      double X1f = c.x0[0] + I * c.dx[0], X2f = c.x0[1] + J * c.dx[1];
+      size_t q = (size_t)i * c.n2g + j;
+      metric_at(p, X1c, X2c, 0, c.gc[q]);
+      metric_at(p, X1f, X2c, 0, c.gf1[q]);
+      int polar = (p.coords == 0 && p.bc_x2 == 2 && (J == 0 || J == p.n2)) ? 1 : 0;
+      metric_at(p, X1c, X2f, polar, c.gf2[q]);
+      double cn[4][4][4];
+      conn_at(p, X1c, X2c, cn);
+      std::memcpy(&c.conn[q * 64], cn, sizeof(cn));
+      c.rc[q] = coord_map(p, X1c, X2c).r;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// C-13  Boundary conditions (A15 outflow + inflow check; "parity unpinned" for the
+// inflow check and the sqrt(-g) B rescale, which the paper does not spell out).
+// Order: X1, then X2, then X3, each over the full extended range of the other two.
+// ------------------------------------------------------------------------------------------
+void inflow_check(const Ctx& c, double prim[8], const Geom& G, int inner) {
+  State S;
+  fluid_state(prim, G, S);
+  bool bad = inner ? (S.ucon[1] > 0.0) : (S.ucon[1] < 0.0);
+  if (!bad) return;
+  double lor = S.lorentz;
+  double alpha = G.alpha;
+  double vt[4];
+  for (int i = 1; i < 4; i++) vt[i] = prim[1 + i] / lor;
+  vt[1] = (G.gcon[0][1] * alpha * alpha) / alpha;  // beta^1 / alpha  => u^1 = 0
+  double vsq = 0.0;
+  for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) vsq += G.gcov[i][j] * vt[i] * vt[j];
+  double gmax = (c.p.gamma_max > 0.0) ? c.p.gamma_max : 50.0;
+  double vmax = 1.0 - 1.0 / (gmax * gmax);
+  if (vsq > vmax) vsq = vmax;
+  double ln = 1.0 / std::sqrt(1.0 - vsq);
+  for (int i = 1; i < 4; i++) prim[1 + i] = ln * vt[i];
+}
+
+void apply_bc(const Ctx& c, double* P) {
+  const int ng = c.ng, n1 = c.p.n1, n2 = c.p.n2, n3 = c.p.n3;
+  // X1
+  if (c.p.bc_x1 != 3) {
+    for (int g = 0; g < ng; g++)
+      for (int side = 0; side < 2; side++) {
+        int ig = side ? (ng + n1 + g) : (ng - 1 - g);
+        int is;
+        if (c.p.bc_x1 == 1) is = side ? (ng + g) : (ng + n1 - 1 - g);
+        else is = side ? (ng + n1 - 1) : ng;  // outflow: adjacent interior zone
+        for (int j = 0; j < c.n2g; j++)
+          for (int k = 0; k < c.n3g; k++) {
+            double q[8];
+            get_prim(c, P, is, j, k, q);
+            if (c.p.bc_x1 == 0) {
+              const Geom& Gs = c.gc[(size_t)is * c.n2g + j];
+              const Geom& Gg = c.gc[(size_t)ig * c.n2g + j];
+              double ratio = Gs.sqrtg / Gg.sqrtg;
+              for (int b = 5; b < 8; b++) q[b] *= ratio;
+              if (c.p.coords == 0) inflow_check(c, q, Gg, side == 0);
+            }
+            for (int v = 0; v < 8; v++) P[c.vidx(v, ig, j, k)] = q[v];
+          }
+      }
+  }
+  // X2
+  if (c.p.bc_x2 != 3) {
+    for (int g = 0; g < ng; g++)
+      for (int side = 0; side < 2; side++) {
+        int jg = side ? (ng + n2 + g) : (ng - 1 - g);
+        int js;
+        if (c.p.bc_x2 == 1) js = side ? (ng + g) : (ng + n2 - 1 - g);
+        else if (c.p.bc_x2 == 2) js = side ? (ng + n2 - 1 - g) : (ng + g);  // mirror
+        else js = side ? (ng + n2 - 1) : ng;
+        for (int i = 0; i < c.n1g; i++)
+          for (int k = 0; k < c.n3g; k++) {
+            double q[8];
+            get_prim(c, P, i, js, k, q);
+            if (c.p.bc_x2 == 2) { q[3] = -q[3]; q[6] = -q[6]; }  // u^2 -> -u^2, B^2 -> -B^2
+            if (c.p.bc_x2 == 0) {
+              double ratio = c.gc[(size_t)i * c.n2g + js].sqrtg / c.gc[(size_t)i * c.n2g + jg].sqrtg;
+              for (int b = 5; b < 8; b++) q[b] *= ratio;
+            }
+            for (int v = 0; v < 8; v++) P[c.vidx(v, i, jg, k)] = q[v];
+          }
+      }
+  }
+  // X3
+  if (c.p.bc_x3 != 3) {
+    for (int g = 0; g < ng; g++)
+      for (int side = 0; side < 2; side++) {
+        int kg = side ? (ng + n3 + g) : (ng - 1 - g);
+        int ks;
+        if (c.p.bc_x3 == 1) {
+          // periodic; for n3 < ng wrap repeatedly
+          int K = side ? (n3 + g) : (-1 - g);
+          int Kw = ((K % n3) + n3) % n3;
+          ks = ng + Kw;
+        } else {
+          ks = side ? (ng + n3 - 1) : ng;
+        }
+        for (int i = 0; i < c.n1g; i++)
+          for (int j = 0; j < c.n2g; j++)
+            for (int v = 0; v < 8; v++) P[c.vidx(v, i, j, kg)] = P[c.vidx(v, i, j, ks)];
+      }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Face fluxes in one direction over the range the flux-CT average needs (C-6):
+// d-face index 0..N_d, transverse zones -1..N.  F[v] stored at the index of the zone whose
+// LOWER d-face it is.  cw stored likewise (0 elsewhere).
+// ------------------------------------------------------------------------------------------
+void flux_dir(Ctx& c, const double* P, int dir, std::vector<double>& F, std::vector<double>& CW, double* cwmax) {
+  const int ng = c.ng;
+  int n[3] = {c.p.n1, c.p.n2, c.p.n3};
+  int lo[3], hi[3];
+  for (int d = 0; d < 3; d++) {
+    if (d == dir - 1) { lo[d] = ng; hi[d] = ng + n[d]; }
+    else { lo[d] = ng - 1; hi[d] = ng + n[d]; }
+  }
+  int e[3] = {0, 0, 0};
+  e[dir - 1] = 1;
+  F.assign(8 * c.nz, 0.0);
+  CW.assign(c.nz, 0.0);
+  double cmax_all = 0.0;
+#pragma omp parallel for reduction(max : cmax_all) schedule(static)
+  for (int i = lo[0]; i <= hi[0]; i++)
+    for (int j = lo[1]; j <= hi[1]; j++)
+      for (int k = lo[2]; k <= hi[2]; k++) {
+        // cell "m" = (i,j,k)-e is on the left of the face, cell "p" = (i,j,k) on the right
+        double pl[8], pr[8];
+        for (int v = 0; v < 8; v++) {
+          double ym[5], yp[5];
+          for (int s = 0; s < 5; s++) {
+            int o = s - 2;
+            ym[s] = P[c.vidx(v, i - e[0] + o * e[0], j - e[1] + o * e[1], k - e[2] + o * e[2])];
+            yp[s] = P[c.vidx(v, i + o * e[0], j + o * e[1], k + o * e[2])];
+          }
+          double l, r;
+          recon_cell(c.p.recon, ym, &l, &r);
+          pl[v] = r;  // q^l at the face = upper-face value of the left cell
+          recon_cell(c.p.recon, yp, &l, &r);
+          pr[v] = l;  // q^r at the face = lower-face value of the right cell
+        }
+        const Geom& G = geom_face(c, dir, i, j);
+        double Fb[8], cw;
+        face_flux(pl, pr, G, c.p.gam, dir, c.p.riemann, Fb, &cw);
+        for (int v = 0; v < 8; v++) F[c.vidx(v, i, j, k)] = Fb[v];
+        CW[c.idx(i, j, k)] = cw;
+        if (cw > cmax_all) cmax_all = cw;
+      }
+  *cwmax = cmax_all;
+}
+
+// ------------------------------------------------------------------------------------------
+// C-7  Flux-CT (eqs. 21-22; A3: the two edges bounding the face).
+// E^1_{i,j,k} lives on the edge (I, J-1/2, K-1/2), E^2 on (I-1/2, J, K-1/2), E^3 on (I-1/2, J-1/2, K).
+// ------------------------------------------------------------------------------------------
+void flux_ct(Ctx& c) {
+  const int ng = c.ng, n1 = c.p.n1, n2 = c.p.n2, n3 = c.p.n3;
+  std::vector<double>&F1 = c.F[0], &F2 = c.F[1], &F3 = c.F[2];
+  for (int d = 0; d < 3; d++) c.E[d].assign(c.nz, 0.0);
+  const int B1 = 5, B2 = 6, B3 = 7;
+#pragma omp parallel for schedule(static)
+  for (int i = ng; i <= ng + n1; i++)
+    for (int j = ng; j <= ng + n2; j++)
+      for (int k = ng; k <= ng + n3; k++) {
+        c.E[0][c.idx(i, j, k)] = 0.25 * (F2[c.vidx(B3, i, j, k)] + F2[c.vidx(B3, i, j, k - 1)] -
+                                         F3[c.vidx(B2, i, j, k)] - F3[c.vidx(B2, i, j - 1, k)]);
+        c.E[1][c.idx(i, j, k)] = 0.25 * (F3[c.vidx(B1, i, j, k)] + F3[c.vidx(B1, i - 1, j, k)] -
+                                         F1[c.vidx(B3, i, j, k)] - F1[c.vidx(B3, i, j, k - 1)]);
+        c.E[2][c.idx(i, j, k)] = 0.25 * (F1[c.vidx(B2, i, j, k)] + F1[c.vidx(B2, i, j - 1, k)] -
+                                         F2[c.vidx(B1, i, j, k)] - F2[c.vidx(B1, i - 1, j, k)]);
+      }
+  const std::vector<double>&E1 = c.E[0], &E2 = c.E[1], &E3 = c.E[2];
+#pragma omp parallel for schedule(static)
+  for (int i = ng; i <= ng + n1; i++)
+    for (int j = ng; j <= ng + n2; j++)
+      for (int k = ng; k <= ng + n3; k++) {
+        bool in1 = i < ng + n1, in2 = j < ng + n2, in3 = k < ng + n3;
+        if (in2 && in3) {  // 1-face (I-1/2, J, K)
+          F1[c.vidx(B1, i, j, k)] = 0.0;
+          F1[c.vidx(B2, i, j, k)] = 0.5 * (E3[c.idx(i, j, k)] + E3[c.idx(i, j + 1, k)]);
+          F1[c.vidx(B3, i, j, k)] = -0.5 * (E2[c.idx(i, j, k)] + E2[c.idx(i, j, k + 1)]);
+        }
+        if (in1 && in3) {  // 2-face (I, J-1/2, K)
+          F2[c.vidx(B2, i, j, k)] = 0.0;
+          F2[c.vidx(B3, i, j, k)] = 0.5 * (E1[c.idx(i, j, k)] + E1[c.idx(i, j, k + 1)]);
+          F2[c.vidx(B1, i, j, k)] = -0.5 * (E3[c.idx(i, j, k)] + E3[c.idx(i + 1, j, k)]);
+        }
+        if (in1 && in2) {  // 3-face (I, J, K-1/2)
+          F3[c.vidx(B3, i, j, k)] = 0.0;
+          F3[c.vidx(B1, i, j, k)] = 0.5 * (E2[c.idx(i, j, k)] + E2[c.idx(i + 1, j, k)]);
+          F3[c.vidx(B2, i, j, k)] = -0.5 * (E1[c.idx(i, j, k)] + E1[c.idx(i, j + 1, k)]);
+        }
+      }
+}
+
+// ------------------------------------------------------------------------------------------
+// C-11  Fix-up of failed zones (eq. 34; A13 deterministic Jacobi passes).
+// "parity unpinned": stencil choice / pass order are DESIGN.md conventions.
+// ------------------------------------------------------------------------------------------
+void fixup(Ctx& c, double* P) {
+  const int ng = c.ng, n1 = c.p.n1, n2 = c.p.n2, n3 = c.p.n3;
+  int64_t nbad = 0;
+  for (size_t q = 0; q < c.nz; q++) if (c.flag[q]) nbad++;
+  c.stats[0] += nbad;
+  if (!nbad) return;
+  std::vector<int32_t> fl(c.flag);
+  std::vector<double> snap(5 * c.nz);
+  const int fo[4][2] = {{1, 0}, {-1, 0}, {0, 1}, {0, -1}};
+  const int dg[4][2] = {{1, 1}, {1, -1}, {-1, 1}, {-1, -1}};
+  for (int pass = 0; pass <= c.p.fixup_max_passes; pass++) {
+    bool last = (pass == c.p.fixup_max_passes);
+    std::vector<int32_t> flnew(fl);
+    std::memcpy(snap.data(), P, 5 * c.nz * sizeof(double));
+    int64_t left = 0;
+    for (int i = ng; i < ng + n1; i++)
+      for (int j = ng; j < ng + n2; j++)
+        for (int k = ng; k < ng + n3; k++) {
+          size_t q = c.idx(i, j, k);
+          if (!fl[q]) continue;
+          bool facegood = true, diaggood = true;
+          for (int m = 0; m < 4; m++) {
+            if (fl[c.idx(i + fo[m][0], j + fo[m][1], k)]) facegood = false;
+            if (fl[c.idx(i + dg[m][0], j + dg[m][1], k)]) diaggood = false;
+          }
+          const int(*st)[2] = nullptr;
+          if (facegood) st = fo; else if (diaggood) st = dg;
+          if (st) {
+            for (int v = 0; v < 5; v++) {
+              double sum = 0.0;
+              for (int m = 0; m < 4; m++) sum += snap[c.vidx(v, i + st[m][0], j + st[m][1], k)];
+              P[c.vidx(v, i, j, k)] = 0.25 * sum;
+            }
+          } else if (last) {
+            int cnt = 0;
+            double sum[5] = {0, 0, 0, 0, 0};
+            for (int di = -1; di <= 1; di++)
+              for (int dj = -1; dj <= 1; dj++) {
+                if (!di && !dj) continue;
+                if (fl[c.idx(i + di, j + dj, k)]) continue;
+                cnt++;
+                for (int v = 0; v < 5; v++) sum[v] += snap[c.vidx(v, i + di, j + dj, k)];
+              }
+            if (cnt > 0) for (int v = 0; v < 5; v++) P[c.vidx(v, i, j, k)] = sum[v] / cnt;
+            c.stats[7]++;
+          } else {
+            left++;
+            continue;
+          }
+          flnew[q] = 0;
+          c.stats[1]++;
+          // floors on the repaired zone (A34)
+          double q8[8];
+          get_prim(c, P, i, j, k, q8);
+          size_t g2 = (size_t)i * c.n2g + j;
+          apply_floors(c.p, c.rc[g2], c.gc[g2], q8);
+          for (int v = 0; v < 5; v++) P[c.vidx(v, i, j, k)] = q8[v];
+        }
+    fl.swap(flnew);
+    if (!left) break;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// C-9  One RK2 substep (eq. 25; A5 source added; A34 order; A35 guess).
+// ------------------------------------------------------------------------------------------
+void substep(Ctx& c, const double* Pflux, const double* Pbase, double dtau, double* Pout, bool record_cw) {
+  double cwm[3];
+  for (int d = 1; d <= 3; d++) flux_dir(c, Pflux, d, c.F[d - 1], c.cw[d - 1], &cwm[d - 1]);
+  if (record_cw) for (int d = 0; d < 3; d++) c.cwmax[d] = cwm[d];
+  flux_ct(c);
+  const int ng = c.ng, n1 = c.p.n1, n2 = c.p.n2, n3 = c.p.n3;
+  std::memcpy(Pout, Pbase, 8 * c.nz * sizeof(double));
+  std::fill(c.flag.begin(), c.flag.end(), 0);
+  int64_t nfl_rho = 0, nfl_u = 0, nceil = 0, ncap = 0, nits = 0;
+#pragma omp parallel for reduction(+ : nfl_rho, nfl_u, nceil, ncap, nits) schedule(static)
+  for (int i = ng; i < ng + n1; i++)
+    for (int j = ng; j < ng + n2; j++)
+      for (int k = ng; k < ng + n3; k++) {
+        size_t g2 = (size_t)i * c.n2g + j;
+        const Geom& G = c.gc[g2];
+        double pb[8], pf[8];
+        get_prim(c, Pbase, i, j, k, pb);
+        get_prim(c, Pflux, i, j, k, pf);
+        State Sb;
+        fluid_state(pb, G, Sb);
+        double U[8];
+        flux_vector(pb, Sb, G, c.p.gam, 0, U);
+        double S[4];
+        const double(*cn)[4][4] = reinterpret_cast<const double(*)[4][4]>(&c.conn[g2 * 64]);
+        source_term(pf, G, cn, c.p.gam, S);
+        for (int v = 0; v < 8; v++) {
+          double div = (c.F[0][c.vidx(v, i + 1, j, k)] - c.F[0][c.vidx(v, i, j, k)]) / c.dx[0] +
+                       (c.F[1][c.vidx(v, i, j + 1, k)] - c.F[1][c.vidx(v, i, j, k)]) / c.dx[1] +
+                       (c.F[2][c.vidx(v, i, j, k + 1)] - c.F[2][c.vidx(v, i, j, k)]) / c.dx[2];
+          double src = (v >= 1 && v <= 4) ? S[v - 1] : 0.0;
+          U[v] = U[v] + dtau * (-div + src);
+        }
+        double pn[8];
+        for (int v = 0; v < 8; v++) pn[v] = pb[v];  // A35
+        int iters;
+        int flag = invert_2d(U, G, c.p.gam, pn, c.p.newton_tol, c.p.newton_maxit, c.p.newton_extra, &iters);
+        nits += iters;
+        if (flag == 0) {
+          int m = apply_floors(c.p, c.rc[g2], G, pn);
+          nfl_rho += (m & 1) ? 1 : 0; nfl_u += (m & 2) ? 1 : 0; nceil += (m & 4) ? 1 : 0; ncap += (m & 8) ? 1 : 0;
+        }
+        c.flag[c.idx(i, j, k)] = flag;
+        for (int v = 0; v < 8; v++) Pout[c.vidx(v, i, j, k)] = pn[v];
+      }
+  c.stats[2] += nfl_rho; c.stats[3] += nfl_u; c.stats[4] += nceil; c.stats[5] += ncap; c.stats[6] += nits;
+  // A34: ghosts are refreshed before the repair (so that ghost donors belong to the same state) and after it
+  apply_bc(c, Pout);
+  fixup(c, Pout);
+  apply_bc(c, Pout);
+}
+
+}  // namespace
+
+// ==========================================================================================
+// C interface (host pointers everywhere).
+// ==========================================================================================
+extern "C" {
+
+typedef struct OracleCtx* oracle_handle;
+struct OracleCtx { Ctx c; };
+
+void oracle_set_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
+int oracle_get_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+// ---- point-level entry points (for the pins) ----
+void oracle_coord_map(const oracle_params* p, double X1, double X2, double out[5]) {
+  Coord c = coord_map(*p, X1, X2);
+  out[0] = c.r; out[1] = c.th; out[2] = c.drdX; out[3] = c.dthdY; out[4] = c.d2thdY2;
+}
+
+void oracle_metric_at(const oracle_params* p, double X1, double X2, int polar_face, double gcov[16], double gcon[16],
+                      double* sqrtg, double* alpha) {
+  Geom G;
+  metric_at(*p, X1, X2, polar_face, G);
+  std::memcpy(gcov, G.gcov, sizeof(G.gcov));
+  std::memcpy(gcon, G.gcon, sizeof(G.gcon));
+  *sqrtg = G.sqrtg; *alpha = G.alpha;
+}
+
+void oracle_conn_at(const oracle_params* p, double X1, double X2, double conn[64]) {
+  double cn[4][4][4];
+  conn_at(*p, X1, X2, cn);
+  std::memcpy(conn, cn, sizeof(cn));
+}
+
+static void geom_from_arrays(const double gcov[16], const double gcon[16], double sqrtg, Geom& G) {
+  std::memcpy(G.gcov, gcov, sizeof(G.gcov));
+  std::memcpy(G.gcon, gcon, sizeof(G.gcon));
+  G.sqrtg = sqrtg;
+  G.alpha = 1.0 / std::sqrt(-G.gcon[0][0]);
+}
+
+void oracle_fluid_state(const double prim[8], const double gcov[16], const double gcon[16], double ucon[4],
+                        double ucov[4], double bcon[4], double bcov[4], double* bsq) {
+  Geom G; geom_from_arrays(gcov, gcon, 1.0, G);
+  State S; fluid_state(prim, G, S);
+  for (int m = 0; m < 4; m++) { ucon[m] = S.ucon[m]; ucov[m] = S.ucov[m]; bcon[m] = S.bcon[m]; bcov[m] = S.bcov[m]; }
+  *bsq = S.bsq;
+}
+
+void oracle_flux_vector(const double prim[8], const double gcov[16], const double gcon[16], double sqrtg, double gam,
+                        int dir, double out[8]) {
+  Geom G; geom_from_arrays(gcov, gcon, sqrtg, G);
+  State S; fluid_state(prim, G, S);
+  flux_vector(prim, S, G, gam, dir, out);
+}
+
+void oracle_wave_speeds(const double prim[8], const double gcov[16], const double gcon[16], double gam, int dir,
+                        double* c1, double* c2) {
+  Geom G; geom_from_arrays(gcov, gcon, 1.0, G);
+  State S; fluid_state(prim, G, S);
+  wave_speeds(prim, S, G, gam, dir, c1, c2);
+}
+
+double oracle_slope_mc(double qm, double q0, double qp) { return slope_mc(qm, q0, qp); }
+
+void oracle_recon_cell(int recon, const double y[5], double* l, double* r) { recon_cell(recon, y, l, r); }
+
+void oracle_face_flux(const double pl[8], const double pr[8], const double gcov[16], const double gcon[16],
+                      double sqrtg, double gam, int dir, int riemann, double Fbar[8], double* cw) {
+  Geom G; geom_from_arrays(gcov, gcon, sqrtg, G);
+  face_flux(pl, pr, G, gam, dir, riemann, Fbar, cw);
+}
+
+void oracle_source_term(const double prim[8], const double gcov[16], const double gcon[16], double sqrtg,
+                        const double conn[64], double gam, double S[4]) {
+  Geom G; geom_from_arrays(gcov, gcon, sqrtg, G);
+  source_term(prim, G, reinterpret_cast<const double(*)[4][4]>(conn), gam, S);
+}
+
+int oracle_invert_2d(const double U[8], const double gcov[16], const double gcon[16], double sqrtg, double gam,
+                     double prim_inout[8], double tol, int maxit, int extra, int* iters) {
+  Geom G; geom_from_arrays(gcov, gcon, sqrtg, G);
+  return invert_2d(U, G, gam, prim_inout, tol, maxit, extra, iters);
+}
+
+int oracle_apply_floors(const oracle_params* p, double r, const double gcov[16], const double gcon[16], double sqrtg,
+                        double prim_inout[8]) {
+  Geom G; geom_from_arrays(gcov, gcon, sqrtg, G);
+  return apply_floors(*p, r, G, prim_inout);
+}
+
+// ---- grid-level entry points (mirror the library's calls, host pointers) ----
+int oracle_grid_init(oracle_handle* out, const oracle_params* p) {
+  if (!out || !p) return -1;
+  if (p->struct_bytes != (int32_t)sizeof(oracle_params)) return -1;
+  if (p->n1 < 1 || p->n2 < 1 || p->n3 < 1 || p->ng < 3) return -1;
+  OracleCtx* h = new OracleCtx();
+  Ctx& c = h->c;
+  c.p = *p;
+  c.ng = p->ng;
+  c.n1g = p->n1 + 2 * p->ng; c.n2g = p->n2 + 2 * p->ng; c.n3g = p->n3 + 2 * p->ng;
+  c.nz = (size_t)c.n1g * c.n2g * c.n3g;
+  if (p->coords == 0) {
+    c.x0[0] = std::log(p->r_in - p->R0);
+    c.dx[0] = (std::log(p->r_out - p->R0) - std::log(p->r_in - p->R0)) / p->n1;
+    c.x0[1] = -1.0; c.dx[1] = 2.0 / p->n2;
+    c.x0[2] = 0.0;  c.dx[2] = 2.0 * PI / p->n3;
+  } else {
+    int n[3] = {p->n1, p->n2, p->n3};
+    for (int d = 0; d < 3; d++) { c.x0[d] = p->xmin[d]; c.dx[d] = (p->xmax[d] - p->xmin[d]) / n[d]; }
+  }
+  build_geometry(c);
+  c.prim = nullptr;
+  c.flag.assign(c.nz, 0);
+  c.Phalf.assign(8 * c.nz, 0.0);
+  c.Pnew.assign(8 * c.nz, 0.0);
+  for (int s = 0; s < 8; s++) c.stats[s] = 0;
+  for (int d = 0; d < 3; d++) c.cwmax[d] = 0.0;
+  *out = h;
+  return 0;
+}
+
+int oracle_destroy(oracle_handle h) { delete h; return 0; }
+
+// loc 0 centre, 1 = 1-face, 2 = 2-face: 22 comps (gcov 00 01 02 03 11 12 13 22 23 33, gcon same, sqrtg, alpha)
+// loc 3: 40 comps Gamma^l_{nk}, l-major, (n,k) in the same 10-pair order.  out[comp][n1g][n2g].
+int oracle_get_geom(oracle_handle h, int loc, double* out) {
+  Ctx& c = h->c;
+  static const int pm[10] = {0, 0, 0, 0, 1, 1, 1, 2, 2, 3}, pn[10] = {0, 1, 2, 3, 1, 2, 3, 2, 3, 3};
+  size_t n = (size_t)c.n1g * c.n2g;
+  if (loc >= 0 && loc <= 2) {
+    const std::vector<Geom>& g = (loc == 0) ? c.gc : (loc == 1) ? c.gf1 : c.gf2;
+    for (size_t q = 0; q < n; q++) {
+      for (int s = 0; s < 10; s++) { out[s * n + q] = g[q].gcov[pm[s]][pn[s]]; out[(10 + s) * n + q] = g[q].gcon[pm[s]][pn[s]]; }
+      out[20 * n + q] = g[q].sqrtg;
+      out[21 * n + q] = g[q].alpha;
+    }
+    return 0;
+  }
+  if (loc == 3) {
+    for (size_t q = 0; q < n; q++)
+      for (int l = 0; l < 4; l++)
+        for (int s = 0; s < 10; s++) out[(size_t)(l * 10 + s) * n + q] = c.conn[q * 64 + l * 16 + pm[s] * 4 + pn[s]];
+    return 0;
+  }
+  return -1;
+}
+
+int oracle_bind(oracle_handle h, double* prim) {
+  h->c.prim = prim;
+  apply_bc(h->c, prim);
+  return 0;
+}
+
+int oracle_apply_bc(oracle_handle h, double* prim) { apply_bc(h->c, prim); return 0; }
+
+// one full RK2 step in place (eq. 25)
+int oracle_step(oracle_handle h, double dt) {
+  Ctx& c = h->c;
+  if (!c.prim) return -2;
+  substep(c, c.prim, c.prim, 0.5 * dt, c.Phalf.data(), true);
+  substep(c, c.Phalf.data(), c.prim, dt, c.Pnew.data(), false);
+  std::memcpy(c.prim, c.Pnew.data(), 8 * c.nz * sizeof(double));
+  return 0;
+}
+
+// stage-level: fluxes of one direction from an arbitrary primitive array (before flux-CT)
+int oracle_flux_dir(oracle_handle h, const double* prim, int dir, double* F_out, double* cw_out, double* cwmax) {
+  Ctx& c = h->c;
+  std::vector<double> F, CW;
+  double m;
+  flux_dir(c, prim, dir, F, CW, &m);
+  if (F_out) std::memcpy(F_out, F.data(), 8 * c.nz * sizeof(double));
+  if (cw_out) std::memcpy(cw_out, CW.data(), c.nz * sizeof(double));
+  if (cwmax) *cwmax = m;
+  return 0;
+}
+
+// stage-level: flux-CT on caller-provided flux arrays [8][nz] each (in place) -> EMFs [3][nz]
+int oracle_flux_ct(oracle_handle h, double* F1, double* F2, double* F3, double* E_out) {
+  Ctx& c = h->c;
+  double* Fs[3] = {F1, F2, F3};
+  for (int d = 0; d < 3; d++) c.F[d].assign(Fs[d], Fs[d] + 8 * c.nz);
+  flux_ct(c);
+  for (int d = 0; d < 3; d++) {
+    std::memcpy(Fs[d], c.F[d].data(), 8 * c.nz * sizeof(double));
+    if (E_out) std::memcpy(E_out + d * c.nz, c.E[d].data(), c.nz * sizeof(double));
+  }
+  return 0;
+}
+
+// stage-level: conserved update with caller-provided (already CT-replaced) fluxes; for the flux-CT pin
+// "arbitrary fluxes leave eq. 23 unchanged" only the B components are updated here:
+// prim B^i <- (sqrt(-g) B^i - dtau * div F(B^i)) / sqrt(-g)
+int oracle_update_B_only(oracle_handle h, double* prim, const double* F1, const double* F2, const double* F3,
+                         double dtau) {
+  Ctx& c = h->c;
+  const int ng = c.ng;
+  const double* Fs[3] = {F1, F2, F3};
+  std::vector<double> out(3 * c.nz);
+  for (int i = ng; i < ng + c.p.n1; i++)
+    for (int j = ng; j < ng + c.p.n2; j++)
+      for (int k = ng; k < ng + c.p.n3; k++) {
+        double sg = c.gc[(size_t)i * c.n2g + j].sqrtg;
+        for (int v = 5; v < 8; v++) {
+          double div = (Fs[0][c.vidx(v, i + 1, j, k)] - Fs[0][c.vidx(v, i, j, k)]) / c.dx[0] +
+                       (Fs[1][c.vidx(v, i, j + 1, k)] - Fs[1][c.vidx(v, i, j, k)]) / c.dx[1] +
+                       (Fs[2][c.vidx(v, i, j, k + 1)] - Fs[2][c.vidx(v, i, j, k)]) / c.dx[2];
+          double U = sg * prim[c.vidx(v, i, j, k)] + dtau * (-div);
+          out[(size_t)(v - 5) * c.nz + c.idx(i, j, k)] = U / sg;
+        }
+      }
+  for (int i = ng; i < ng + c.p.n1; i++)
+    for (int j = ng; j < ng + c.p.n2; j++)
+      for (int k = ng; k < ng + c.p.n3; k++)
+        for (int v = 5; v < 8; v++) prim[c.vidx(v, i, j, k)] = out[(size_t)(v - 5) * c.nz + c.idx(i, j, k)];
+  return 0;
+}
+
+int oracle_prim_to_cons(oracle_handle h, const double* prim, double* U) {
+  Ctx& c = h->c;
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < c.n1g; i++)
+    for (int j = 0; j < c.n2g; j++)
+      for (int k = 0; k < c.n3g; k++) {
+        const Geom& G = c.gc[(size_t)i * c.n2g + j];
+        double q[8], out[8];
+        get_prim(c, prim, i, j, k, q);
+        State S;
+        fluid_state(q, G, S);
+        flux_vector(q, S, G, c.p.gam, 0, out);
+        for (int v = 0; v < 8; v++) U[c.vidx(v, i, j, k)] = out[v];
+      }
+  return 0;
+}
+
+// pure inversion on full-grid arrays: no floors, no fix-ups
+int oracle_cons_to_prim(oracle_handle h, const double* U, double* prim_inout, int32_t* flag) {
+  Ctx& c = h->c;
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < c.n1g; i++)
+    for (int j = 0; j < c.n2g; j++)
+      for (int k = 0; k < c.n3g; k++) {
+        const Geom& G = c.gc[(size_t)i * c.n2g + j];
+        double u8[8], q[8];
+        for (int v = 0; v < 8; v++) { u8[v] = U[c.vidx(v, i, j, k)]; q[v] = prim_inout[c.vidx(v, i, j, k)]; }
+        int iters;
+        int f = invert_2d(u8, G, c.p.gam, q, c.p.newton_tol, c.p.newton_maxit, c.p.newton_extra, &iters);
+        for (int v = 0; v < 8; v++) prim_inout[c.vidx(v, i, j, k)] = q[v];
+        if (flag) flag[c.idx(i, j, k)] = f;
+      }
+  return 0;
+}
+
+// C-14 (eq. 26; A17): dt^l = xi dx^l / max over faces of c_w^l ; 1/dt = sum_l 1/dt^l
+int oracle_cfl_dt(oracle_handle h, double xi, double* dt_out) {
+  Ctx& c = h->c;
+  if (!c.prim) return -2;
+  double inv = 0.0;
+  for (int d = 1; d <= 3; d++) {
+    double m;
+    flux_dir(c, c.prim, d, c.F[d - 1], c.cw[d - 1], &m);
+    double dtl = xi * c.dx[d - 1] / m;
+    inv += 1.0 / dtl;
+  }
+  *dt_out = 1.0 / inv;
+  return 0;
+}
+
+// dt from the predictor's face speeds of the last oracle_step (the paper's "next time step")
+int oracle_last_cfl_dt(oracle_handle h, double xi, double* dt_out) {
+  Ctx& c = h->c;
+  double inv = 0.0;
+  for (int d = 0; d < 3; d++) inv += c.cwmax[d] / (xi * c.dx[d]);
+  *dt_out = 1.0 / inv;
+  return 0;
+}
+
+// C-15 (eq. 23; A4): corner-centred divergence of sqrt(-g) B over corners whose 8 (4 in
+// 2D) cells are interior (periodic X3 copies count as interior).
+int oracle_divb(oracle_handle h, double* max_abs, double* max_norm) {
+  Ctx& c = h->c;
+  if (!c.prim) return -2;
+  const int ng = c.ng, n1 = c.p.n1, n2 = c.p.n2, n3 = c.p.n3;
+  double mabs = 0.0, mnorm = 0.0;
+  bool two_d = (n3 == 1);
+  int khi = two_d ? ng : ((c.p.bc_x3 == 1) ? ng + n3 - 1 : ng + n3 - 2);
+  for (int i = ng; i <= ng + n1 - 2; i++)
+    for (int j = ng; j <= ng + n2 - 2; j++)
+      for (int k = ng; k <= khi; k++) {
+        double D = 0.0, A = 0.0;
+        int nl3 = two_d ? 1 : 2;
+        for (int l1 = 0; l1 < 2; l1++)
+          for (int l2 = 0; l2 < 2; l2++)
+            for (int l3 = 0; l3 < nl3; l3++) {
+              int ii = i + l1, jj = j + l2, kk = k + l3;
+              double sg = c.gc[(size_t)ii * c.n2g + jj].sqrtg;
+              double w = two_d ? 0.5 : 0.25;
+              double t1 = (l1 ? 1.0 : -1.0) * sg * c.prim[c.vidx(5, ii, jj, kk)] * w / c.dx[0];
+              double t2 = (l2 ? 1.0 : -1.0) * sg * c.prim[c.vidx(6, ii, jj, kk)] * w / c.dx[1];
+              D += t1 + t2; A += std::fabs(t1) + std::fabs(t2);
+              if (!two_d) {
+                double t3 = (l3 ? 1.0 : -1.0) * sg * c.prim[c.vidx(7, ii, jj, kk)] * w / c.dx[2];
+                D += t3; A += std::fabs(t3);
+              }
+            }
+        if (std::fabs(D) > mabs) mabs = std::fabs(D);
+        if (A > 0.0 && std::fabs(D) / A > mnorm) mnorm = std::fabs(D) / A;
+      }
+  *max_abs = mabs; *max_norm = mnorm;
+  return 0;
+}
+
+// 0 failed inversions, 1 zones repaired, 2 rho-floor hits, 3 u-floor hits, 4 ceilings, 5 Lorentz caps,
+// 6 Newton iterations, 7 zones repaired by the last-resort rule
+int oracle_get_stats(oracle_handle h, int64_t out[8]) {
+  for (int s = 0; s < 8; s++) out[s] = h->c.stats[s];
+  return 0;
+}
+
+int oracle_get_flags(oracle_handle h, int32_t* out) {
+  std::memcpy(out, h->c.flag.data(), h->c.nz * sizeof(int32_t));
+  return 0;
+}
+
+// stage-level: fix-up on a caller-provided primitive array with caller-provided flags
+int oracle_fixup(oracle_handle h, double* prim, const int32_t* flag) {
+  Ctx& c = h->c;
+  c.flag.assign(flag, flag + c.nz);
+  fixup(c, prim);
+  return 0;
+}
+
+}  // extern "C"
