@@ -90,3 +90,26 @@ def random_smooth(shape, rng, nmodes=3):
 
 def rng(seed=SEED):
     return np.random.Generator(np.random.PCG64(seed))
+
+
+def fast_wave(p, direction=0, bdir=1, amp=1e-6, rho0=1.0, u0=0.3, B0=0.5, t=0.0):
+    """Right-going linear fast magnetosonic wave, wave vector along `direction`, uniform field B0 along
+    `bdir` (perpendicular), fluid at rest.  Returns prim and the phase speed
+    c_f = sqrt((gam p + b^2)/(w + b^2)) (eq. 18 of the paper for k perpendicular to B)."""
+    assert bdir != direction
+    gam = p["gam"]
+    pg = (gam - 1.0) * u0
+    w = rho0 + u0 + pg
+    bsq = B0 * B0
+    cf = np.sqrt((gam * pg + bsq) / (w + bsq))
+    x = centres(p, direction)
+    L = p["xmax"][direction] - p["xmin"][direction]
+    shape = [1, 1, 1]
+    shape[direction] = -1
+    ph = np.sin(2.0 * np.pi * (x - cf * t) / L).reshape(shape)
+    prim = empty_prim(p)
+    prim[0] = rho0 * (1.0 + amp * ph)
+    prim[1] = u0 * (1.0 + gam * amp * ph)
+    prim[2 + direction] = cf * amp * ph
+    prim[5 + bdir] = B0 * (1.0 + amp * ph)
+    return prim, cf
