@@ -1,0 +1,284 @@
+#!/usr/bin/env python
+"""bench.py — zone-cycles/s of the full RK2 step (the whole hot path) on the headline workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--impl ours|reference] [--graph 0|1]
+
+One JSON line on stdout (rank 0).  Workload: BASELINE.json configs[3] = C4, the 256^3 MKS Fishbone-Moncrief
+torus, PPM + LLF, fp64 (seeded synthetic stand-in for the paper's initial data).
+N > 1 (torchrun): the path does not shard in this build ("replicas only"): every rank steps its own
+copy, no data-path collective; value = N x zones x K / max-over-ranks time.
+
+--impl reference: the CPU oracle as it stands, on the host cores, on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "zone-cycles/s per full RK2 step at 256^3 fp64 (1 B200); % of HBM roofline"
+UNIT = "zone-cycles/s"
+B_ALG = 1218.0          # algorithmic bytes per zone-cycle
+# algorithmic bytes per zone and launch of each kernel class: flux: read P 64, write 7 comps 56;
+# emf: read 6 B-fluxes 48, write 3 EMFs 24; update: P^n 64 + hydro fluxes 120 + EMFs 24 (+ P-half 64 in the
+# corrector, averaged: +32) in, 64 + 4 (flag) out
+KERNEL_BYTES = {"flux1": 120.0, "flux2": 120.0, "flux3": 120.0, "emf": 72.0, "update": 308.0}
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", d
+    return 6650.0, "fallback (B200_PROFILING.md)", {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_workload(name, **kw):
+    from workloads import config
+    from workloads.params import TORUS
+    from workloads.torus import fm_torus
+    p = config(name, **kw)
+    prim, info = fm_torus(p, **TORUS[name])
+    return p, prim
+
+
+def oracle_sample(name, steps, n3_sample=8, threads=None):
+    """The oracle as it stands on a phi-slab of the same torus (same (r,theta) grid and scheme, n3 = n3_sample):
+    returns (zone-cycles/s, cores, description, seconds)."""
+    import oracle
+    p, prim = make_workload(name, n3=n3_sample)
+    if threads:
+        oracle.set_threads(threads)
+    g = oracle.Grid(p)
+    g.bind(prim)
+    dt = g.cfl_dt(0.45)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        g.step(dt)
+    sec = time.perf_counter() - t0
+    zones = p["n1"] * p["n2"] * p["n3"]
+    return zones * steps / sec, oracle.get_threads(), f"{name} torus, {p['n1']}x{p['n2']}x{p['n3']} phi-slab of the {name} grid, {steps} RK2 steps", sec
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    per_step = []
+    p = None
+    import oracle
+    p, prim = make_workload(args.config, n3=args.ref_n3)
+    g = oracle.Grid(p)
+    g.bind(prim)
+    dt = g.cfl_dt(0.45)
+    zones = p["n1"] * p["n2"] * p["n3"]
+    for _ in range(args.warmup):
+        g.step(dt)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        g.step(dt)
+    sec = time.perf_counter() - t0
+    val = zones * args.steps / sec
+    sample = f"{args.config} torus, {p['n1']}x{p['n2']}x{p['n3']} phi-slab of the {args.config} grid per step"
+    out = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": 1e3 * sec / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic", "impl": "reference",
+           "config": {"workload": f"{args.config}: {sample} (CPU oracle, bounded sample)", "recon": p["recon"], "riemann": p["riemann"]},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import paper_2205_02484_b200 as cu
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the library has no CPU path)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    p, prim_host = make_workload(args.config)
+    zones = p["n1"] * p["n2"] * p["n3"]
+    prim_pinned = torch.from_numpy(prim_host).pin_memory()
+    s = cu.Solver(p, prim_pinned, device=f"cuda:{local}")
+    dt = s.cfl_dt(0.45)                                   # fixed dt chosen beforehand (eq. 26, xi = 0.45)
+    if args.graph:
+        s.use_graph(True)
+    for _ in range(args.warmup):
+        s.step(dt)
+    barrier()
+
+    # ---- timed region: K steps, device-resident inputs, CUDA events on the library's stream -----------------
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    if not args.graph:
+        s.set_timing(True)
+    l0 = s.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        s.step(dt)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = s.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    timing = s.get_timing() if not args.graph else {}
+    s.set_timing(False)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * zones * args.steps / (ms * 1e-3)
+    divb = s.divb()[1]
+    stats = s.stats()
+
+    # ---- e2e: the same step through the public API with HOST buffers: H2D of the primitives from pinned memory,
+    # one step, D2H of the result, every step inside the timed region ----------------------------------------
+    e2e_steps = max(1, min(args.e2e_steps, args.steps))
+    out_pinned = torch.empty_like(prim_pinned)
+    barrier()
+    e0.record()
+    for _ in range(e2e_steps):
+        s.load(prim_pinned)          # H2D + ghost fill
+        s.step(dt)
+        out_pinned.copy_(s.prim, non_blocking=True)
+    e1.record()
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    e2e_val = world * zones * e2e_steps / (ms_e2e * 1e-3)
+    nbytes = prim_pinned.numel() * 8
+
+    if rank == 0:
+        peak, peak_src, pk = peaks()
+        # dominant kernel class by measured device time
+        roof = None
+        shares = {}
+        if timing:
+            tot = sum(v[0] for v in timing.values())
+            shares = {k: round(v[0] / tot, 4) for k, v in timing.items() if v[1]}
+            dom = max((k for k in KERNEL_BYTES if timing[k][1]), key=lambda k: timing[k][0])
+            per_launch_ms = timing[dom][0] / timing[dom][1]
+            achieved = KERNEL_BYTES[dom] * zones / (per_launch_ms * 1e-3) / 1e9
+            roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                    "kernel_ms_per_launch": per_launch_ms, "kernel_time_shares": shares,
+                    "step_frac_of_hbm_roofline": value / world * B_ALG / (peak * 1e9),
+                    "note": "achieved = algorithmic bytes of the dominant kernel class per launch / its mean "
+                            "CUDA-event duration in the timed region; step_frac = zone-cycles/s x 1218 B / peak"}
+        else:
+            roof = {"bound": "hbm", "kernel": "whole step (graph replay)", "achieved": value / world * B_ALG / 1e9,
+                    "peak": peak, "unit": "GB/s", "frac": value / world * B_ALG / (peak * 1e9), "traffic": None,
+                    "peak_source": peak_src}
+        cpu = None
+        if not args.no_cpu:
+            v, cores, sample, sec = oracle_sample(args.config, args.cpu_steps, args.ref_n3)
+            cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": sec}
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+               "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+               "dtype": "f64", "data": "synthetic",
+               "config": {"workload": f"{args.config}: {p['n1']}x{p['n2']}x{p['n3']} MKS Fishbone-Moncrief torus, "
+                                      f"a={p['a']}, gam={p['gam']:.4f}, recon={'PPM' if p['recon'] else 'PLM-MC'}, "
+                                      f"riemann={'HLL' if p['riemann'] else 'LLF'}, fixed dt from cfl_dt(0.45)",
+                          "l2": "inputs larger than L2 (prim 1.15 GB, fluxes 3 GB per substep vs 126 MB L2)",
+                          "parallelism": "replicas only" if world > 1 else "single GPU", "graph": bool(args.graph),
+                          "dt": dt},
+               "clocks": clocks, "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": nbytes,
+                                         "d2h_bytes_per_step": nbytes, "steps": e2e_steps},
+               "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
+               "checks": {"divb_norm": divb, "stats": stats}}
+        print(json.dumps(out), flush=True)
+    s.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C4")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--graph", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-steps", type=int, default=3)
+    ap.add_argument("--ref-n3", type=int, default=32)
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

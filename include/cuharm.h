@@ -1,0 +1,159 @@
+/* cuharm.h — C ABI of libcuharm.so: the per-zone HARM conservative update of ideal GR-MHD on a fixed
+ * Kerr-Schild / modified-Kerr-Schild grid (cuHARM, arXiv 2205.02484), fp64, one NVIDIA B200 (sm_100a).
+ *
+ * Citations: "P:L<n>" = line n of the paper text with the equation it falls in; "A<n>" = a
+ * reading of the paper listed in DESIGN.md where the text is silent, garbled or self-contradictory.
+ *
+ * General rules
+ *   - Every function returns int: 0 = OK, <0 = one of the CUHARM_E* codes.  Nothing throws or aborts.
+ *     Physics trouble (a failed inversion, a floor hit) is NOT an error: see cuharm_get_stats.
+ *   - Pointers named d_* are DEVICE pointers, everything else is a HOST pointer.
+ *   - The caller owns every device byte.  The library borrows d_prim / d_workspace from cuharm_bind until
+ *     cuharm_destroy or the next cuharm_bind; it never allocates or frees device memory.
+ *   - All work is enqueued on the CUDA stream given to cuharm_grid_init.  Only the calls that return host
+ *     scalars (cuharm_cfl_dt, cuharm_last_cfl_dt, cuharm_divb, cuharm_get_stats) synchronise that stream.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns CUHARM_ECUDA.
+ *
+ * Array layout (device, fp64, C order, the last index fastest):
+ *   prim[8][n1+2ng][n2+2ng][n3+2ng], variables (rho, u, utilde^1, utilde^2, utilde^3, B^1, B^2, B^3)
+ *   (eq. 10).  All vector components are coordinate components in (X^1, X^2, X^3).  Zone (I,J,K) has its
+ *   centre at X^d = X^d_min + (index + 1/2) dx^d; array index = zone index + ng.
+ */
+#ifndef CUHARM_H
+#define CUHARM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CUHARM_OK 0
+#define CUHARM_EINVAL (-1) /* bad argument / shape / struct size            */
+#define CUHARM_ESTATE (-2) /* called out of order (e.g. step before bind)   */
+#define CUHARM_ECUDA (-3)  /* a CUDA call failed; text via cuharm_strerror  */
+#define CUHARM_ENOMEM (-4) /* workspace too small                           */
+
+typedef struct cuharm_ctx* cuharm_handle; /* opaque, host side; owns no device memory */
+
+/* Plain-old-data parameter block; struct_bytes = sizeof(cuharm_params) guards against layout drift. */
+typedef struct {
+  int32_t struct_bytes;
+  int32_t n1, n2, n3, ng; /* interior zones per direction (n3 == 1 allowed); ghost layers, ng >= 3          */
+  int32_t coords;         /* 0 = MKS (eq. 39; A14); 1 = Minkowski-Cartesian (tests; A39)        */
+  double a, gam;          /* black-hole spin (eq. 38); adiabatic index of p = (gam-1) u     */
+  double r_in, r_out, R0, hslope; /* MKS: X1 in [ln(r_in-R0), ln(r_out-R0)], X2 in [-1,1], X3 in [0,2pi)    */
+  double xmin[3], xmax[3];        /* Minkowski box                                                          */
+  int32_t recon;   /* 0 = PLM + MC limiter (eqs. 15-16; A2); 1 = PPM (A20)              */
+  int32_t riemann; /* 0 = local Lax-Friedrichs (eq. 17); 1 = HLL (eq. 20)                   */
+  int32_t bc_x1, bc_x2, bc_x3; /* 0 outflow (+ inflow check in MKS X1; A15), 1 periodic, 2 polar reflection
+                                  with utilde^2, B^2 sign flip, 3 fixed (ghosts never overwritten) */
+  double rho_fl_coef, rho_fl_pow, rho_fl_abs; /* rho >= max(abs, coef * r^pow)  (eq. 35; A9)    */
+  double u_fl_coef, u_fl_pow, u_fl_abs;       /* u   >= max(abs, coef * r^pow)                              */
+  double sigma_max, b2_over_u_max, gamma_max; /* b^2/rho, b^2/u ceilings (eqs. 36-37; A10, A11) and Lorentz
+                                                 factor cap (A12); <= 0 disables                    */
+  double newton_tol;                          /* |dW/W| criterion of the 2D Newton-Raphson (A8)     */
+  int32_t newton_maxit, newton_extra;         /* iteration cap; extra iterations after the criterion is met */
+  int32_t fixup_max_passes;                   /* Jacobi passes of the eq. 34 repair (A13)                   */
+  int32_t reserved;
+} cuharm_params;
+
+/* Create a context for the grid and scheme described by *p (the statement of the problem: spin a, adiabatic
+ * index, MKS parameters, resolution — P:L285-311).  cuda_stream is a cudaStream_t (NULL = default stream).
+ * Errors: EINVAL (null pointers, struct_bytes mismatch, n < 1, ng < 3, bad enum, polar reflection with n2 < ng),
+ * ECUDA (no usable device). */
+int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stream);
+
+/* Bytes of device workspace cuharm_bind needs: geometry tables, face fluxes F^1..3, edge EMFs, the half-step
+ * primitives, the fail mask, counters.  0 if h is NULL. */
+size_t cuharm_workspace_bytes(cuharm_handle h);
+
+/* Borrow the caller's primitive array d_prim (layout above) and workspace (256-byte aligned, ws_bytes >=
+ * cuharm_workspace_bytes).  If the geometry is already computed the ghost zones of d_prim are filled.
+ * Errors: EINVAL (null / misaligned), ENOMEM (ws_bytes too small). */
+int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_bytes);
+
+/* Geometry precompute (eqs. 38-39): g_cov, g_con, sqrt(-g), lapse at zone centres, 1-faces and
+ * 2-faces (3-faces equal centres: the metric is phi-independent), and the connection coefficients at
+ * centres from closed-form derivatives (A19), plus the floor profiles of eq. 35.  Then fills the ghost
+ * zones of the bound d_prim.  Errors: ESTATE (not bound). */
+int cuharm_metric_precompute(cuharm_handle h);
+
+/* One full RK2 (midpoint predictor / corrector) step of size dt, in place (eq. 25; A5): each substep
+ * = reconstruction (eqs. 15-16 / PPM) -> LLF/HLL face fluxes (eqs. 17-20) -> flux-CT (eqs. 21-22; A3) -> source
+ * (eq. 14) -> update -> Noble 2D inversion (eqs. 27-31; A6-A8) -> floors (eqs. 35-37) -> ghost fill -> repair of
+ * failed zones (eq. 34; A13) -> ghost fill.  d_prim has valid ghosts on entry and on exit.  Asynchronous.
+ * Errors: ESTATE (not bound / no geometry), EINVAL (dt not finite or <= 0). */
+int cuharm_step(cuharm_handle h, double dt);
+
+/* Pure inversion (eqs. 27-31) on full-grid arrays of the prim layout: d_U holds the 8 conserved variables
+ * sqrt(-g)(rho u^t, T^t_t, T^t_i, B^i) (A18); d_prim_inout carries the Newton guess in and the answer out;
+ * d_flag[zone] (int32, [n1g][n2g][n3g], may be NULL) = 0 ok, 1 D<=0 / non-finite input, 2 no convergence,
+ * 3 W<=0 or non-finite, 4 v^2 outside [0,1), 5 rho<=0, 6 u<0.  No floors, no repairs.  Asynchronous. */
+int cuharm_cons_to_prim(cuharm_handle h, const double* d_U, double* d_prim_inout, int32_t* d_flag);
+
+/* Primitive -> conserved on full-grid arrays.  Test helper.  Asynchronous. */
+int cuharm_prim_to_cons(cuharm_handle h, const double* d_prim, double* d_U);
+
+/* Time step of eq. 26 (A17) from the bound primitives: dt^l = xi dx^l / max_faces c_w^l,
+ * 1/dt = sum_l 1/dt^l.  Overwrites the flux workspace.  Synchronises. */
+int cuharm_cfl_dt(cuharm_handle h, double xi, double* dt_out);
+
+/* Same formula from the face speeds the predictor of the last cuharm_step saw ("the next time step",
+ * P:L198) — costs one 24-byte read-back, no extra kernel.  Synchronises.  ESTATE before the first step. */
+int cuharm_last_cfl_dt(cuharm_handle h, double xi, double* dt_out);
+
+/* Corner-centred discrete divergence of sqrt(-g) B (eq. 23; A4) over the corners whose cells are
+ * interior: *max_abs = max |D|, *max_norm = max |D| / (sum of the magnitudes of D's own terms).  Synchronises. */
+int cuharm_divb(cuharm_handle h, double* max_abs, double* max_norm);
+
+/* Copy a geometry table to a caller array d_out[comp][n1g][n2g]: loc 0 centre, 1 = 1-face (I-1/2,J), 2 = 2-face
+ * (I,J-1/2): 22 comps = g_cov (00 01 02 03 11 12 13 22 23 33), g_con (same order), sqrt(-g), lapse; loc 3: the 40
+ * connection coefficients Gamma^l_{nk}, l-major, (n,k) in the same 10-pair order.  Test helper.  Asynchronous. */
+int cuharm_get_geom(cuharm_handle h, int32_t loc, double* d_out);
+
+/* Fill the ghost zones of an arbitrary primitive array of the bound shape.  Asynchronous. */
+int cuharm_apply_bc(cuharm_handle h, double* d_prim);
+
+/* Stage-level test helpers (asynchronous; arrays have the prim layout unless stated):
+ * face fluxes of direction dir (1..3) BEFORE flux-CT, d_F[8][zones] stored at the zone whose LOWER dir-face it
+ * is, valid on faces 0..N_dir and transverse zones -1..N (eqs. 15-20); d_cw[zones] (may be NULL) = c_w. */
+int cuharm_flux_dir(cuharm_handle h, const double* d_prim, int32_t dir, double* d_F, double* d_cw);
+
+/* out[8] (HOST): 0 failed inversions, 1 zones repaired, 2 rho-floor hits, 3 u-floor hits, 4 ceilings applied,
+ * 5 Lorentz caps, 6 Newton iterations, 7 zones repaired by the last-resort rule.  Synchronises. */
+int cuharm_get_stats(cuharm_handle h, int64_t out[8]);
+
+/* Record the two substeps of cuharm_step into a CUDA graph and replay it on later calls (on != 0), or go back
+ * to plain launches (on == 0).  Purely a launch-overhead optimisation; results are identical. */
+int cuharm_use_graph(cuharm_handle h, int32_t on);
+
+/* Number of kernel launches the library has enqueued since grid_init (graph replays count their nodes). */
+int64_t cuharm_launch_count(cuharm_handle h);
+
+/* Kernel classes of the per-class timing below. */
+#define CUHARM_K_FLUX1 0  /* reconstruct + flux, direction 1 */
+#define CUHARM_K_FLUX2 1
+#define CUHARM_K_FLUX3 2
+#define CUHARM_K_EMF 3    /* flux-CT edge EMFs               */
+#define CUHARM_K_UPDATE 4 /* source + update + inversion + floors */
+#define CUHARM_K_BC 5     /* one ghost fill (up to 3 launches)    */
+#define CUHARM_K_FIXUP 6  /* eq. 34 repair                        */
+#define CUHARM_NCLASS 8
+
+/* Measurement aid: when on, a pair of CUDA events on the library's stream brackets every launch of the classes
+ * above (plain launches only; ignored while a graph replays).  cuharm_get_timing synchronises and returns, per
+ * class, the summed device milliseconds and the number of bracketed launches since cuharm_set_timing(h, 1). */
+int cuharm_set_timing(cuharm_handle h, int32_t on);
+int cuharm_get_timing(cuharm_handle h, double ms[CUHARM_NCLASS], int64_t count[CUHARM_NCLASS]);
+
+int cuharm_destroy(cuharm_handle h);
+
+/* Static text for a CUHARM_E* code; for CUHARM_ECUDA the text of the last CUDA error seen by this thread. */
+const char* cuharm_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CUHARM_H */

@@ -1,0 +1,524 @@
+// cuharm_api.cu — host side of libcuharm.so: the C ABI of include/cuharm.h, workspace carving, launch
+// sequencing of one RK2 step (eq. 25), optional CUDA-graph replay.  No torch types, no device
+// allocation: the caller owns every device byte.  There is no CPU path: without a device every call fails.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/cuharm.h"
+#include "cuharm_geom.cuh"
+#include "cuharm_kernels.cuh"
+
+using namespace cuharm;
+
+namespace {
+
+thread_local char g_errtext[256] = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e, const char* what) {
+  snprintf(g_errtext, sizeof(g_errtext), "%s: %s", what, cudaGetErrorString(e));
+  (void)cudaGetLastError();  // clear the non-sticky error state so that later calls report their own
+  return CUHARM_ECUDA;
+}
+#define CK(call)                                          \
+  do {                                                    \
+    cudaError_t e_ = (call);                              \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call);   \
+  } while (0)
+
+size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// counters block (unsigned long long slots)
+enum { CNT_STATS = 0, CNT_NFAIL = 8, CNT_CWPRED = 10, CNT_CWSCR = 13, CNT_DIVB = 16, CNT_TOTAL = 32 };
+
+}  // namespace
+
+struct cuharm_ctx {
+  cuharm_params p;
+  Dims d;
+  cudaStream_t stream;
+  double dx[3], x0[3];
+  // borrowed device memory
+  double* prim = nullptr;
+  char* ws = nullptr;
+  Geom *gC = nullptr, *gF1 = nullptr, *gF2 = nullptr;
+  double *conn = nullptr, *floors = nullptr, *F[3] = {nullptr, nullptr, nullptr}, *E = nullptr, *Phalf = nullptr;
+  int *flag = nullptr, *list = nullptr;
+  unsigned long long* cnt = nullptr;
+  bool bound = false, have_geom = false, stepped = false;
+  int64_t launches = 0;
+  // optional per-kernel-class timing with CUDA events on the library's stream (cuharm_set_timing)
+  bool timing = false, capturing = false;
+  std::vector<cudaEvent_t> ev;
+  std::vector<int> ev_cat;
+  size_t ev_used = 0;
+  double t_ms[CUHARM_NCLASS] = {0};
+  int64_t t_n[CUHARM_NCLASS] = {0};
+  // graph
+  bool use_graph = false;
+  cudaGraphExec_t gexec = nullptr;
+  cudaStream_t cap_stream = nullptr;
+  double graph_dt = 0.0;
+  int64_t graph_nodes = 0;
+};
+
+namespace {
+
+struct WsLayout {
+  size_t gC, gF1, gF2, conn, floors, F[3], E, Phalf, flag, list, cnt, total;
+};
+
+WsLayout layout(const Dims& d) {
+  WsLayout L;
+  size_t off = 0;
+  const size_t ncol = (size_t)d.n1g * d.n2g, nz = (size_t)d.nz;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+  L.gC = take(ncol * sizeof(Geom));
+  L.gF1 = take(ncol * sizeof(Geom));
+  L.gF2 = take(ncol * sizeof(Geom));
+  L.conn = take(ncol * 40 * sizeof(double));
+  L.floors = take(ncol * 2 * sizeof(double));
+  for (int k = 0; k < 3; k++) L.F[k] = take(7 * nz * sizeof(double));
+  L.E = take(3 * nz * sizeof(double));
+  L.Phalf = take(8 * nz * sizeof(double));
+  L.flag = take(nz * sizeof(int));
+  L.list = take(nz * sizeof(int));
+  L.cnt = take(CNT_TOTAL * sizeof(unsigned long long));
+  L.total = off;
+  return L;
+}
+
+NewtonCfg newton_cfg(const cuharm_params& p) { return NewtonCfg{p.newton_tol, p.newton_maxit, p.newton_extra}; }
+FloorCfg floor_cfg(const cuharm_params& p) { return FloorCfg{p.sigma_max, p.b2_over_u_max, p.gamma_max}; }
+
+// RAII pair of events around one launch (or one group of launches) of a kernel class
+struct Timed {
+  cuharm_ctx* h;
+  bool live;
+  Timed(cuharm_ctx* h_, int cat) : h(h_), live(false) {
+    if (!h->timing || h->capturing || h->ev_used + 2 > h->ev.size()) return;
+    if (cudaEventRecord(h->ev[h->ev_used], h->stream) != cudaSuccess) return;
+    h->ev_cat.push_back(cat);
+    live = true;
+  }
+  ~Timed() {
+    if (!live) return;
+    cudaEventRecord(h->ev[h->ev_used + 1], h->stream);
+    h->ev_used += 2;
+  }
+};
+
+int launch_bc(cuharm_ctx* h, double* P, const unsigned long long* gate) {
+  Timed t_(h, CUHARM_K_BC);
+  const Dims& d = h->d;
+  BcArgs a{d, P, h->gC, 0, h->p.coords, h->p.gamma_max, gate};
+  const int T = 128;
+  if (h->p.bc_x1 != 3) {
+    a.kind = h->p.bc_x1;
+    bc_x1_kernel<<<dim3((d.n3g + T - 1) / T, d.n2g, 2 * d.ng), T, 0, h->stream>>>(a);
+    h->launches++;
+  }
+  if (h->p.bc_x2 != 3) {
+    a.kind = h->p.bc_x2;
+    bc_x2_kernel<<<dim3((d.n3g + T - 1) / T, d.n1g, 2 * d.ng), T, 0, h->stream>>>(a);
+    h->launches++;
+  }
+  if (h->p.bc_x3 != 3) {
+    a.kind = h->p.bc_x3;
+    const long long n = (long long)d.n1g * d.n2g * 2 * d.ng;
+    bc_x3_kernel<<<(unsigned)((n + T - 1) / T), T, 0, h->stream>>>(a);
+    h->launches++;
+  }
+  CK(cudaGetLastError());
+  return CUHARM_OK;
+}
+
+template <int DIR, bool STAGE>
+void launch_flux_t(cuharm_ctx* h, const FluxArgs& a, dim3 grid) {
+  const int rc = h->p.recon, rm = h->p.riemann;
+  if (rc == 0 && rm == 0) flux_kernel<DIR, 0, 0, STAGE><<<grid, 128, 0, h->stream>>>(a);
+  else if (rc == 0 && rm == 1) flux_kernel<DIR, 0, 1, STAGE><<<grid, 128, 0, h->stream>>>(a);
+  else if (rc == 1 && rm == 0) flux_kernel<DIR, 1, 0, STAGE><<<grid, 128, 0, h->stream>>>(a);
+  else flux_kernel<DIR, 1, 1, STAGE><<<grid, 128, 0, h->stream>>>(a);
+}
+
+// fluxes of direction dir (1..3) of the primitive array P into F (and c_w max into cwmax)
+template <bool STAGE>
+int launch_flux(cuharm_ctx* h, const double* P, int dir, double* F, double* cw, unsigned long long* cwmax) {
+  const Dims& d = h->d;
+  int lo[3], hi[3];
+  const int n[3] = {d.n1, d.n2, d.n3};
+  for (int c = 0; c < 3; c++) {
+    lo[c] = (c == dir - 1) ? d.ng : d.ng - 1;
+    hi[c] = d.ng + n[c];
+  }
+  Timed t_(h, CUHARM_K_FLUX1 + dir - 1);
+  FluxArgs a{d, P, dir == 1 ? h->gF1 : (dir == 2 ? h->gF2 : h->gC), F, cw, cwmax, h->p.gam, lo[0], lo[1], lo[2], hi[2]};
+  dim3 grid((hi[2] - lo[2] + 1 + 127) / 128, hi[1] - lo[1] + 1, hi[0] - lo[0] + 1);
+  if (dir == 1) launch_flux_t<1, STAGE>(h, a, grid);
+  else if (dir == 2) launch_flux_t<2, STAGE>(h, a, grid);
+  else launch_flux_t<3, STAGE>(h, a, grid);
+  h->launches++;
+  CK(cudaGetLastError());
+  return CUHARM_OK;
+}
+
+// one RK2 substep (A34 order): fluxes -> EMFs -> update+inversion+floors -> ghost fill -> repair -> ghost fill
+int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pout, double dtau, int which) {
+  const Dims& d = h->d;
+  unsigned long long* cwmax = h->cnt + (which == 0 ? CNT_CWPRED : CNT_CWSCR);
+  for (int dir = 1; dir <= 3; dir++) {
+    int rc = launch_flux<false>(h, Pflux, dir, h->F[dir - 1], nullptr, cwmax + (dir - 1));
+    if (rc) return rc;
+  }
+  {
+    Timed t_(h, CUHARM_K_EMF);
+    EmfArgs a{d, h->F[0], h->F[1], h->F[2], h->E};
+    emf_kernel<<<dim3((d.n3 + 1 + 127) / 128, d.n2 + 1, d.n1 + 1), 128, 0, h->stream>>>(a);
+    h->launches++;
+  }
+  unsigned long long* nfail = h->cnt + CNT_NFAIL + which;
+  {
+    Timed t_(h, CUHARM_K_UPDATE);
+    UpdArgs a{d, Pbase, Pflux, Pout, h->F[0], h->F[1], h->F[2], h->E, h->gC, h->conn, h->floors, h->flag, h->list,
+              nfail, h->cnt + CNT_STATS, dtau, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], h->p.gam,
+              newton_cfg(h->p), floor_cfg(h->p)};
+    dim3 grid((d.n3 + 127) / 128, d.n2, d.n1);
+    if (Pflux == Pbase) update_kernel<true><<<grid, 128, 0, h->stream>>>(a);
+    else update_kernel<false><<<grid, 128, 0, h->stream>>>(a);
+    h->launches++;
+  }
+  CK(cudaGetLastError());
+  int rc = launch_bc(h, Pout, nullptr);
+  if (rc) return rc;
+  {
+    Timed t_(h, CUHARM_K_FIXUP);
+    FixArgs a{d, Pout, h->flag, h->list, nfail, h->cnt + CNT_STATS, h->gC, h->floors, h->p.fixup_max_passes, h->p.gam,
+              newton_cfg(h->p), floor_cfg(h->p)};
+    fixup_kernel<<<1, 1024, 0, h->stream>>>(a);
+    h->launches++;
+  }
+  CK(cudaGetLastError());
+  return launch_bc(h, Pout, nfail);
+}
+
+int enqueue_step(cuharm_ctx* h, double dt) {
+  // per-step counters: failure counts of the two substeps, the c_w maxima of predictor and corrector
+  CK(cudaMemsetAsync(h->cnt + CNT_NFAIL, 0, (CNT_DIVB - CNT_NFAIL) * sizeof(unsigned long long), h->stream));
+  int rc = substep(h, h->prim, h->prim, h->Phalf, 0.5 * dt, 0);  // predictor: fluxes and source from P^n
+  if (rc) return rc;
+  return substep(h, h->Phalf, h->prim, h->prim, dt, 1);          // corrector: from the half-step state, in place
+}
+
+int check_params(const cuharm_params* p) {
+  if (p->struct_bytes != (int32_t)sizeof(cuharm_params)) return CUHARM_EINVAL;
+  if (p->n1 < 1 || p->n2 < 1 || p->n3 < 1 || p->ng < 3 || p->ng > 8) return CUHARM_EINVAL;
+  if (p->coords < 0 || p->coords > 1 || p->recon < 0 || p->recon > 1 || p->riemann < 0 || p->riemann > 1) return CUHARM_EINVAL;
+  const int bcs[3] = {p->bc_x1, p->bc_x2, p->bc_x3};
+  for (int c = 0; c < 3; c++)
+    if (bcs[c] < 0 || bcs[c] > 3) return CUHARM_EINVAL;
+  if (p->bc_x1 == 2 || p->bc_x3 == 2) return CUHARM_EINVAL;  // the polar reflection belongs to X2
+  if (p->bc_x2 == 2 && p->n2 < p->ng) return CUHARM_EINVAL;  // a mirror image needs ng interior zones
+  if (!(p->gam > 1.0) || !(p->newton_tol > 0.0) || p->newton_maxit < 1 || p->newton_extra < 0 || p->fixup_max_passes < 0)
+    return CUHARM_EINVAL;
+  if (p->coords == 0) {
+    if (!(p->r_in - p->R0 > 0.0) || !(p->r_out > p->r_in) || !(std::fabs(p->a) <= 1.0)) return CUHARM_EINVAL;
+  } else {
+    for (int c = 0; c < 3; c++)
+      if (!(p->xmax[c] > p->xmin[c])) return CUHARM_EINVAL;
+  }
+  if ((long long)(p->n1 + 2 * p->ng) * (p->n2 + 2 * p->ng) * (p->n3 + 2 * p->ng) > 2000000000LL) return CUHARM_EINVAL;
+  return CUHARM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stream) {
+  if (!out || !p) return CUHARM_EINVAL;
+  int rc = check_params(p);
+  if (rc) return rc;
+  int ndev = 0;
+  CK(cudaGetDeviceCount(&ndev));
+  if (ndev < 1) return cuda_fail(cudaErrorNoDevice, "cuharm_grid_init");
+  cuharm_ctx* h = new (std::nothrow) cuharm_ctx();
+  if (!h) return CUHARM_ENOMEM;
+  h->p = *p;
+  h->stream = (cudaStream_t)cuda_stream;
+  Dims& d = h->d;
+  d.n1 = p->n1; d.n2 = p->n2; d.n3 = p->n3; d.ng = p->ng;
+  d.n1g = p->n1 + 2 * p->ng; d.n2g = p->n2 + 2 * p->ng; d.n3g = p->n3 + 2 * p->ng;
+  d.s2 = d.n3g; d.s1 = (long long)d.n2g * d.n3g; d.nz = (long long)d.n1g * d.s1;
+  if (p->coords == 0) {  // eq. 39: uniform in X1 = ln(r - R0), X2 in [-1,1], X3 in [0, 2 pi)
+    const double PI = 3.14159265358979323846;
+    h->x0[0] = std::log(p->r_in - p->R0);
+    h->dx[0] = (std::log(p->r_out - p->R0) - std::log(p->r_in - p->R0)) / p->n1;
+    h->x0[1] = -1.0; h->dx[1] = 2.0 / p->n2;
+    h->x0[2] = 0.0;  h->dx[2] = 2.0 * PI / p->n3;
+  } else {
+    const int n[3] = {p->n1, p->n2, p->n3};
+    for (int c = 0; c < 3; c++) { h->x0[c] = p->xmin[c]; h->dx[c] = (p->xmax[c] - p->xmin[c]) / n[c]; }
+  }
+  *out = h;
+  return CUHARM_OK;
+}
+
+size_t cuharm_workspace_bytes(cuharm_handle h) { return h ? layout(h->d).total : 0; }
+
+int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_bytes) {
+  if (!h || !d_prim || !d_workspace) return CUHARM_EINVAL;
+  if (((uintptr_t)d_workspace & 255) || ((uintptr_t)d_prim & 15)) return CUHARM_EINVAL;
+  const WsLayout L = layout(h->d);
+  if (ws_bytes < L.total) return CUHARM_ENOMEM;
+  const bool same_ws = h->ws == (char*)d_workspace;
+  h->prim = d_prim;
+  h->ws = (char*)d_workspace;
+  h->gC = (Geom*)(h->ws + L.gC); h->gF1 = (Geom*)(h->ws + L.gF1); h->gF2 = (Geom*)(h->ws + L.gF2);
+  h->conn = (double*)(h->ws + L.conn); h->floors = (double*)(h->ws + L.floors);
+  for (int k = 0; k < 3; k++) h->F[k] = (double*)(h->ws + L.F[k]);
+  h->E = (double*)(h->ws + L.E); h->Phalf = (double*)(h->ws + L.Phalf);
+  h->flag = (int*)(h->ws + L.flag); h->list = (int*)(h->ws + L.list);
+  h->cnt = (unsigned long long*)(h->ws + L.cnt);
+  if (!same_ws) h->have_geom = false;
+  if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+  h->bound = true;
+  h->stepped = false;
+  CK(cudaMemsetAsync(h->flag, 0, (size_t)h->d.nz * sizeof(int), h->stream));  // ghost zones always count as good
+  CK(cudaMemsetAsync(h->cnt, 0, CNT_TOTAL * sizeof(unsigned long long), h->stream));
+  if (h->have_geom) {
+    int rc = launch_bc(h, h->prim, nullptr);
+    if (rc) return rc;
+    // the half-step array keeps the caller's ghost values where a boundary is `fixed`
+    CK(cudaMemcpyAsync(h->Phalf, h->prim, 8 * (size_t)h->d.nz * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+  }
+  return CUHARM_OK;
+}
+
+int cuharm_metric_precompute(cuharm_handle h) {
+  if (!h) return CUHARM_EINVAL;
+  if (!h->bound) return CUHARM_ESTATE;
+  const cuharm_params& p = h->p;
+  const Dims& d = h->d;
+  GeomArgs a{d.n1g, d.n2g, d.ng, d.n2, p.coords, (p.coords == 0 && p.bc_x2 == 2) ? 1 : 0, p.a, p.R0, p.hslope,
+             h->x0[0], h->x0[1], h->dx[0], h->dx[1], p.rho_fl_coef, p.rho_fl_pow, p.rho_fl_abs, p.u_fl_coef,
+             p.u_fl_pow, p.u_fl_abs, h->gC, h->gF1, h->gF2, h->conn, h->floors};
+  const int n = d.n1g * d.n2g;
+  geom_kernel<<<(n + 63) / 64, 64, 0, h->stream>>>(a);
+  h->launches++;
+  CK(cudaGetLastError());
+  h->have_geom = true;
+  int rc = launch_bc(h, h->prim, nullptr);
+  if (rc) return rc;
+  CK(cudaMemcpyAsync(h->Phalf, h->prim, 8 * (size_t)d.nz * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+  return CUHARM_OK;
+}
+
+int cuharm_step(cuharm_handle h, double dt) {
+  if (!h) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  if (!(dt > 0.0) || !std::isfinite(dt)) return CUHARM_EINVAL;
+  h->stepped = true;
+  if (!h->use_graph) return enqueue_step(h, dt);
+  if (!h->gexec || h->graph_dt != dt) {  // (re)capture: dt is baked into the kernel arguments
+    if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+    cudaGraph_t g = nullptr;
+    const int64_t before = h->launches;
+    // record on a private stream (the caller's may be the legacy default stream, which cannot be captured);
+    // the instantiated graph is then launched on the caller's stream
+    if (!h->cap_stream) CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+    cudaStream_t user = h->stream;
+    CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+    h->stream = h->cap_stream;
+    h->capturing = true;
+    int rc = enqueue_step(h, dt);
+    h->capturing = false;
+    h->stream = user;
+    cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
+    h->graph_nodes = h->launches - before;
+    h->launches = before;
+    if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+    if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+    e = cudaGraphInstantiate(&h->gexec, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { h->gexec = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
+    h->graph_dt = dt;
+  }
+  CK(cudaGraphLaunch(h->gexec, h->stream));
+  h->launches += h->graph_nodes;
+  return CUHARM_OK;
+}
+
+int cuharm_use_graph(cuharm_handle h, int32_t on) {
+  if (!h) return CUHARM_EINVAL;
+  h->use_graph = on != 0;
+  if (!on && h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+  return CUHARM_OK;
+}
+
+int64_t cuharm_launch_count(cuharm_handle h) { return h ? h->launches : 0; }
+
+int cuharm_set_timing(cuharm_handle h, int32_t on) {
+  if (!h) return CUHARM_EINVAL;
+  if (on && h->ev.empty()) {
+    h->ev.resize(2 * 8192);
+    for (auto& e : h->ev) CK(cudaEventCreate(&e));
+  }
+  h->timing = on != 0;
+  h->ev_used = 0;
+  h->ev_cat.clear();
+  for (int c = 0; c < CUHARM_NCLASS; c++) { h->t_ms[c] = 0.0; h->t_n[c] = 0; }
+  return CUHARM_OK;
+}
+
+int cuharm_get_timing(cuharm_handle h, double ms[CUHARM_NCLASS], int64_t count[CUHARM_NCLASS]) {
+  if (!h || !ms || !count) return CUHARM_EINVAL;
+  CK(cudaStreamSynchronize(h->stream));
+  for (size_t q = 0; q + 1 < h->ev_used; q += 2) {
+    float t = 0.f;
+    CK(cudaEventElapsedTime(&t, h->ev[q], h->ev[q + 1]));
+    const int c = h->ev_cat[q / 2];
+    h->t_ms[c] += t;
+    h->t_n[c] += 1;
+  }
+  h->ev_used = 0;
+  h->ev_cat.clear();
+  for (int c = 0; c < CUHARM_NCLASS; c++) { ms[c] = h->t_ms[c]; count[c] = h->t_n[c]; }
+  return CUHARM_OK;
+}
+
+int cuharm_cons_to_prim(cuharm_handle h, const double* d_U, double* d_prim_inout, int32_t* d_flag) {
+  if (!h || !d_U || !d_prim_inout) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  const Dims& d = h->d;
+  ConvArgs a{d, d_U, d_prim_inout, d_flag, h->gC, h->p.gam, newton_cfg(h->p)};
+  cons_to_prim_kernel<<<dim3((d.n3g + 127) / 128, d.n2g, d.n1g), 128, 0, h->stream>>>(a);
+  h->launches++;
+  CK(cudaGetLastError());
+  return CUHARM_OK;
+}
+
+int cuharm_prim_to_cons(cuharm_handle h, const double* d_prim, double* d_U) {
+  if (!h || !d_prim || !d_U) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  const Dims& d = h->d;
+  ConvArgs a{d, d_prim, d_U, nullptr, h->gC, h->p.gam, newton_cfg(h->p)};
+  prim_to_cons_kernel<<<dim3((d.n3g + 127) / 128, d.n2g, d.n1g), 128, 0, h->stream>>>(a);
+  h->launches++;
+  CK(cudaGetLastError());
+  return CUHARM_OK;
+}
+
+static int dt_from_cw(cuharm_handle h, const unsigned long long* d_cw, double xi, double* dt_out) {
+  unsigned long long m[3];
+  CK(cudaMemcpyAsync(m, d_cw, sizeof(m), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  double inv = 0.0;
+  for (int c = 0; c < 3; c++) {
+    double cw;
+    std::memcpy(&cw, &m[c], sizeof(double));
+    const double dtl = xi * h->dx[c] / cw;  // dt^l = xi dx^l / max c_w
+    inv += 1.0 / dtl;                       // eq. 26
+  }
+  *dt_out = 1.0 / inv;
+  return CUHARM_OK;
+}
+
+int cuharm_cfl_dt(cuharm_handle h, double xi, double* dt_out) {
+  if (!h || !dt_out || !(xi > 0.0)) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  unsigned long long* cw = h->cnt + CNT_CWSCR;
+  CK(cudaMemsetAsync(cw, 0, 3 * sizeof(unsigned long long), h->stream));
+  for (int dir = 1; dir <= 3; dir++) {
+    int rc = launch_flux<false>(h, h->prim, dir, h->F[dir - 1], nullptr, cw + (dir - 1));
+    if (rc) return rc;
+  }
+  return dt_from_cw(h, cw, xi, dt_out);
+}
+
+int cuharm_last_cfl_dt(cuharm_handle h, double xi, double* dt_out) {
+  if (!h || !dt_out || !(xi > 0.0)) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom || !h->stepped) return CUHARM_ESTATE;
+  return dt_from_cw(h, h->cnt + CNT_CWPRED, xi, dt_out);
+}
+
+int cuharm_divb(cuharm_handle h, double* max_abs, double* max_norm) {
+  if (!h || !max_abs || !max_norm) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  const Dims& d = h->d;
+  const bool two_d = d.n3 == 1;
+  const int khi = two_d ? d.ng : ((h->p.bc_x3 == 1) ? d.ng + d.n3 - 1 : d.ng + d.n3 - 2);
+  unsigned long long* out = h->cnt + CNT_DIVB;
+  CK(cudaMemsetAsync(out, 0, 2 * sizeof(unsigned long long), h->stream));
+  if (d.n1 >= 2 && d.n2 >= 2 && khi >= d.ng) {
+    DivbArgs a{d, h->prim, h->gC, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], khi, out};
+    divb_kernel<<<dim3((khi - d.ng + 1 + 127) / 128, d.n2 - 1, d.n1 - 1), 128, 0, h->stream>>>(a);
+    h->launches++;
+    CK(cudaGetLastError());
+  }
+  unsigned long long m[2];
+  CK(cudaMemcpyAsync(m, out, sizeof(m), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  std::memcpy(max_abs, &m[0], sizeof(double));
+  std::memcpy(max_norm, &m[1], sizeof(double));
+  return CUHARM_OK;
+}
+
+int cuharm_get_geom(cuharm_handle h, int32_t loc, double* d_out) {
+  if (!h || !d_out || loc < 0 || loc > 3) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  const int n = h->d.n1g * h->d.n2g;
+  const Geom* tab = loc == 1 ? h->gF1 : (loc == 2 ? h->gF2 : h->gC);
+  geom_export_kernel<<<(n + 127) / 128, 128, 0, h->stream>>>(tab, h->conn, loc, n, d_out);
+  h->launches++;
+  CK(cudaGetLastError());
+  return CUHARM_OK;
+}
+
+int cuharm_apply_bc(cuharm_handle h, double* d_prim) {
+  if (!h || !d_prim) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  return launch_bc(h, d_prim, nullptr);
+}
+
+int cuharm_flux_dir(cuharm_handle h, const double* d_prim, int32_t dir, double* d_F, double* d_cw) {
+  if (!h || !d_prim || !d_F || dir < 1 || dir > 3) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  CK(cudaMemsetAsync(d_F, 0, 8 * (size_t)h->d.nz * sizeof(double), h->stream));
+  if (d_cw) CK(cudaMemsetAsync(d_cw, 0, (size_t)h->d.nz * sizeof(double), h->stream));
+  return launch_flux<true>(h, d_prim, dir, d_F, d_cw, h->cnt + CNT_CWSCR + (dir - 1));
+}
+
+int cuharm_get_stats(cuharm_handle h, int64_t out[8]) {
+  if (!h || !out) return CUHARM_EINVAL;
+  if (!h->bound) return CUHARM_ESTATE;
+  CK(cudaMemcpyAsync(out, h->cnt + CNT_STATS, 8 * sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return CUHARM_OK;
+}
+
+int cuharm_destroy(cuharm_handle h) {
+  if (!h) return CUHARM_EINVAL;
+  if (h->gexec) cudaGraphExecDestroy(h->gexec);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  for (auto& e : h->ev) cudaEventDestroy(e);
+  delete h;
+  return CUHARM_OK;
+}
+
+const char* cuharm_strerror(int code) {
+  switch (code) {
+    case CUHARM_OK: return "ok";
+    case CUHARM_EINVAL: return "invalid argument";
+    case CUHARM_ESTATE: return "call out of order (bind / metric_precompute / step)";
+    case CUHARM_ECUDA: return g_errtext;
+    case CUHARM_ENOMEM: return "workspace too small";
+    default: return "unknown error code";
+  }
+}
+
+}  // extern "C"
