@@ -93,7 +93,10 @@ WsLayout layout(const Dims& d) {
 }
 
 NewtonCfg newton_cfg(const cuharm_params& p) { return NewtonCfg{p.newton_tol, p.newton_maxit, p.newton_extra}; }
-FloorCfg floor_cfg(const cuharm_params& p) { return FloorCfg{p.sigma_max, p.b2_over_u_max, p.gamma_max}; }
+FloorCfg floor_cfg(const cuharm_params& p) {
+  return FloorCfg{p.sigma_max, p.b2_over_u_max, p.gamma_max, p.sigma_max > 0.0 ? 1.0 / p.sigma_max : 0.0,
+                  p.b2_over_u_max > 0.0 ? 1.0 / p.b2_over_u_max : 0.0};
+}
 
 // RAII pair of events around one launch (or one group of launches) of a kernel class
 struct Timed {
@@ -137,13 +140,32 @@ int launch_bc(cuharm_ctx* h, double* P, const unsigned long long* gate) {
   return CUHARM_OK;
 }
 
-template <int DIR, bool STAGE>
-void launch_flux_t(cuharm_ctx* h, const FluxArgs& a, dim3 grid) {
-  const int rc = h->p.recon, rm = h->p.riemann;
-  if (rc == 0 && rm == 0) flux_kernel<DIR, 0, 0, STAGE><<<grid, 128, 0, h->stream>>>(a);
-  else if (rc == 0 && rm == 1) flux_kernel<DIR, 0, 1, STAGE><<<grid, 128, 0, h->stream>>>(a);
-  else if (rc == 1 && rm == 0) flux_kernel<DIR, 1, 0, STAGE><<<grid, 128, 0, h->stream>>>(a);
-  else flux_kernel<DIR, 1, 1, STAGE><<<grid, 128, 0, h->stream>>>(a);
+// number of marching segments per column: enough warps for several waves over the 148 SMs, segments not shorter
+// than 16 faces (the prologue of a segment reconstructs one extra cell)
+int march_seg(long long columns, int nfaces) {
+  const long long warps = (columns + 31) / 32;
+  int nseg = (int)((148LL * 16 * 6 + warps - 1) / warps);
+  const int maxseg = (nfaces + 15) / 16;
+  if (nseg > maxseg) nseg = maxseg;
+  if (nseg < 1) nseg = 1;
+  return (nfaces + nseg - 1) / nseg;  // faces per segment
+}
+
+template <int RECON, int RIEMANN, bool STAGE>
+void launch_flux_t(cuharm_ctx* h, FluxArgs& a, int dir) {
+  const int ni = a.hi1 - a.lo1 + 1, nj = a.hi2 - a.lo2 + 1, nk = a.hi3 - a.lo3 + 1;
+  if (dir == 3) {
+    const int fpw = FluxK<RECON>::FPW;
+    const long long warps = (long long)ni * nj * ((nk + fpw - 1) / fpw);
+    flux_k_kernel<RECON, RIEMANN, STAGE><<<(unsigned)((warps + 3) / 4), 128, 0, h->stream>>>(a);
+  } else {
+    const long long cols = (long long)(dir == 1 ? nj : ni) * nk;
+    const int nf = dir == 1 ? ni : nj;
+    a.seg = march_seg(cols, nf);
+    const dim3 grid((unsigned)((cols + 127) / 128), (unsigned)((nf + a.seg - 1) / a.seg));
+    if (dir == 1) flux_march_kernel<1, RECON, RIEMANN, STAGE><<<grid, 128, 0, h->stream>>>(a);
+    else flux_march_kernel<2, RECON, RIEMANN, STAGE><<<grid, 128, 0, h->stream>>>(a);
+  }
 }
 
 // fluxes of direction dir (1..3) of the primitive array P into F (and c_w max into cwmax)
@@ -157,11 +179,13 @@ int launch_flux(cuharm_ctx* h, const double* P, int dir, double* F, double* cw, 
     hi[c] = d.ng + n[c];
   }
   Timed t_(h, CUHARM_K_FLUX1 + dir - 1);
-  FluxArgs a{d, P, dir == 1 ? h->gF1 : (dir == 2 ? h->gF2 : h->gC), F, cw, cwmax, h->p.gam, lo[0], lo[1], lo[2], hi[2]};
-  dim3 grid((hi[2] - lo[2] + 1 + 127) / 128, hi[1] - lo[1] + 1, hi[0] - lo[0] + 1);
-  if (dir == 1) launch_flux_t<1, STAGE>(h, a, grid);
-  else if (dir == 2) launch_flux_t<2, STAGE>(h, a, grid);
-  else launch_flux_t<3, STAGE>(h, a, grid);
+  FluxArgs a{d, P, dir == 1 ? h->gF1 : (dir == 2 ? h->gF2 : h->gC), F, cw, cwmax, h->p.gam,
+             lo[0], lo[1], lo[2], hi[0], hi[1], hi[2], 0};
+  const int rc = h->p.recon, rm = h->p.riemann;
+  if (rc == 0 && rm == 0) launch_flux_t<0, 0, STAGE>(h, a, dir);
+  else if (rc == 0 && rm == 1) launch_flux_t<0, 1, STAGE>(h, a, dir);
+  else if (rc == 1 && rm == 0) launch_flux_t<1, 0, STAGE>(h, a, dir);
+  else launch_flux_t<1, 1, STAGE>(h, a, dir);
   h->launches++;
   CK(cudaGetLastError());
   return CUHARM_OK;

@@ -39,6 +39,7 @@ __device__ inline void flat_geom(Geom& G) {
   G.g00 = -1.0; G.g01 = 0.0; G.g03 = 0.0; G.g11 = 1.0; G.g13 = 0.0; G.g22 = 1.0; G.g33 = 1.0;
   G.c00 = -1.0; G.c01 = 0.0; G.c03 = 0.0; G.c11 = 1.0; G.c13 = 0.0; G.c22 = 1.0; G.c33 = 1.0;
   G.sg = 1.0; G.alpha = 1.0;
+  G.ialpha = 1.0; G.ac01 = 0.0; G.isg = 1.0; G.pad = 0.0;
 }
 
 // eq. 38 with Sigma = r^2 + a^2 cos^2(theta), transformed by J = diag(1, r', theta', 1)
@@ -67,6 +68,10 @@ __device__ inline void mks_geom(const GeomArgs& A, double X1, double X2, bool on
   G.c33 = 1.0 / (Sig * s2f);
   G.sg = on_axis ? 0.0 : Sig * fabs(sn) * fabs(p.rp) * fabs(p.thp);
   G.alpha = 1.0 / sqrt(-G.c00);
+  G.ialpha = sqrt(-G.c00);
+  G.ac01 = G.alpha * G.c01;
+  G.isg = G.sg > 0.0 ? 1.0 / G.sg : 0.0;
+  G.pad = 0.0;
 }
 
 // Gamma^l_{nk} = 1/2 g^{ls} (d_n g_{sk} + d_k g_{sn} - d_s g_{nk}); the metric depends on X1, X2 only.

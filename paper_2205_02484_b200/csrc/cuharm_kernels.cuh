@@ -1,33 +1,11 @@
-// cuharm_kernels.cuh — grid kernels of the hot path (S1-S11 of DESIGN.md): ghost fill, reconstruct+flux per
-// direction, flux-CT EMFs, fused source+update+inversion+floors, repair of failed zones, CFL and div B
+// cuharm_kernels.cuh — grid kernels of the hot path (S1-S11 of DESIGN.md) other than the flux kernels
+// (cuharm_flux.cuh): ghost fill, flux-CT EMFs, fused source+update+inversion+floors, repair of failed zones, CFL and div B
 // reductions.  fp64, SoA prim[8][n1g][n2g][n3g] with k (phi) fastest: a warp runs along k at fixed (i,j), so
 // every geometry read is a broadcast (the metric is phi-independent).
 #pragma once
-#include "cuharm_phys.cuh"
+#include "cuharm_flux.cuh"
 
 namespace cuharm {
-
-struct Dims {
-  int n1, n2, n3, ng;
-  int n1g, n2g, n3g;
-  long long s1, s2;  // element strides of i and j (k has stride 1)
-  long long nz;      // zones per variable, ghosts included
-};
-
-__device__ __forceinline__ unsigned long long warp_max_ull(unsigned long long v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    const unsigned long long w = __shfl_xor_sync(0xffffffffu, v, o);
-    v = w > v ? w : v;
-  }
-  return v;
-}
-
-// max of non-negative doubles through their order-preserving integer image; no floating-point atomics anywhere
-__device__ __forceinline__ void atomic_max_nonneg(unsigned long long* addr, double v) {
-  const unsigned long long m = warp_max_ull((unsigned long long)__double_as_longlong(v >= 0.0 ? v : 0.0));
-  if ((threadIdx.x & 31) == 0 && m > *reinterpret_cast<volatile unsigned long long*>(addr)) atomicMax(addr, m);
-}
 
 // ---------------------------------------------------------------------------------------------------------
 // S1  Boundary conditions (A15).  Order X1, X2, X3, each over the full extended range of the others.
@@ -134,66 +112,6 @@ __global__ void bc_x3_kernel(BcArgs a) {
   const long long base = (long long)col * d.n3g;
 #pragma unroll
   for (int v = 0; v < 8; v++) a.P[v * d.nz + base + kg] = a.P[v * d.nz + base + ks];
-}
-
-// ---------------------------------------------------------------------------------------------------------
-// S2+S3  Reconstruction + Riemann flux of one direction, one thread per face (eqs. 15-20).
-// Face (i,j,k) = LOWER DIR-face of zone (i,j,k); computed on faces ng..ng+N_DIR and transverse zones
-// ng-1..ng+N (one ghost layer, for the EMF average).  Output: F[c][zone], c = 0..4 hydro components,
-// c = 5,6 the induction fluxes of B^{DIR+1}, B^{DIR+2} (cyclic); the flux of B^{DIR} is identically replaced by
-// zero in flux-CT (eq. 22) and never stored.  STAGE = true (test helper): all 8 components + c_w per face.
-// cwmax: running max of c_w over the faces of this launch (S10 by-product).
-// ---------------------------------------------------------------------------------------------------------
-struct FluxArgs {
-  Dims d;
-  const double* P;
-  const Geom* Gf;  // geometry at this direction's faces
-  double* F;       // [7][nz] (or [8][nz] if STAGE)
-  double* cw;      // STAGE only
-  unsigned long long* cwmax;
-  double gam;
-  int lo1, lo2, lo3, hi3;
-};
-
-template <int DIR, int RECON, int RIEMANN, bool STAGE>
-__global__ void __launch_bounds__(128) flux_kernel(FluxArgs a) {
-  const Dims& d = a.d;
-  const int k = a.lo3 + blockIdx.x * 128 + threadIdx.x;
-  const int j = a.lo2 + blockIdx.y, i = a.lo1 + blockIdx.z;
-  double cwv = 0.0;
-  if (k <= a.hi3) {
-    const long long sd = DIR == 1 ? d.s1 : (DIR == 2 ? d.s2 : 1);
-    const long long idx = i * d.s1 + j * d.s2 + k;
-    double pl[8], pr[8];
-#pragma unroll
-    for (int v = 0; v < 8; v++) {
-      const double* y = a.P + v * d.nz + idx;
-      double dum;
-      if (RECON == 0) {
-        const double ym2 = y[-2 * sd], ym1 = y[-sd], y0 = y[0], y1 = y[sd];
-        recon_cell<0>(0.0, ym2, ym1, y0, 0.0, dum, pl[v]);
-        recon_cell<0>(0.0, ym1, y0, y1, 0.0, pr[v], dum);
-      } else {
-        const double ym3 = y[-3 * sd], ym2 = y[-2 * sd], ym1 = y[-sd], y0 = y[0], y1 = y[sd], y2 = y[2 * sd];
-        recon_cell<1>(ym3, ym2, ym1, y0, y1, dum, pl[v]);  // q^l = upper-face value of the left zone
-        recon_cell<1>(ym2, ym1, y0, y1, y2, pr[v], dum);   // q^r = lower-face value of the right zone
-      }
-    }
-    const Geom G = load_geom(a.Gf, i * d.n2g + j);
-    double F[8];
-    face_flux<DIR, RIEMANN>(pl, pr, G, a.gam, F, cwv);
-    if (STAGE) {
-#pragma unroll
-      for (int v = 0; v < 8; v++) a.F[v * d.nz + idx] = F[v];
-      if (a.cw) a.cw[idx] = cwv;
-    } else {
-#pragma unroll
-      for (int v = 0; v < 5; v++) a.F[v * d.nz + idx] = F[v];
-      a.F[5 * d.nz + idx] = F[5 + (DIR % 3)];        // B^{DIR+1}
-      a.F[6 * d.nz + idx] = F[5 + ((DIR + 1) % 3)];  // B^{DIR+2}
-    }
-  }
-  atomic_max_nonneg(a.cwmax, cwv);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -304,7 +222,7 @@ __global__ void __launch_bounds__(128) update_kernel(UpdArgs a) {
     for (int v = 0; v < 8; v++) pn[v] = pb[v];  // A35: the guess is P^n
     const int flag = invert_2d(U, G, a.gam, pn, a.nc, c_its);
     if (flag == 0) {
-      const int m = apply_floors(pn, G, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), a.fc, a.gam, a.nc);
+      const int m = apply_floors(pn, G, a.C + q2, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), a.fc, a.gam, a.nc);
       c_rho = m & 1; c_u = (m >> 1) & 1; c_ceil = (m >> 2) & 1; c_cap = (m >> 3) & 1;
     } else {
       const unsigned long long pos = atomicAdd(a.nfail, 1ull);
@@ -414,7 +332,7 @@ __global__ void __launch_bounds__(1024) fixup_kernel(FixArgs a) {
       for (int v = 5; v < 8; v++) q[v] = a.P[v * d.nz + idx];
       const int q2 = (int)(idx / d.s2);  // = i * n2g + j
       const Geom G = load_geom(a.C, q2);
-      apply_floors(q, G, a.floors[2 * q2], a.floors[2 * q2 + 1], a.fc, a.gam, a.nc);
+      apply_floors(q, G, a.C + q2, a.floors[2 * q2], a.floors[2 * q2 + 1], a.fc, a.gam, a.nc);
 #pragma unroll
       for (int v = 0; v < 5; v++) a.P[v * d.nz + idx] = q[v];
       a.flag[idx] = -(pass + 1);

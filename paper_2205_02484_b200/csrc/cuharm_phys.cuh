@@ -4,21 +4,24 @@
 // Shares nothing with oracle/ (the CPU checker): no header, table, constant generator or helper.
 //
 // Metric storage.  In Kerr-Schild coordinates and under the diagonal MKS Jacobian (eqs. 38-39) the covariant and
-// the contravariant metric have the same zero pattern: the (0,2), (1,2), (2,3) entries vanish.  Only the seven
-// entries 00 01 03 11 13 22 33 of each are stored and every contraction below skips the structural zeros (adding
-// an exact zero never changes a sum, so this is the same arithmetic as the full 4x4 contraction).
+// the contravariant metric have the same zero pattern: the (0,2), (1,2), (2,3) entries vanish, and g^{t phi} = 0 as
+// well.  Only the seven entries 00 01 03 11 13 22 33 of each are stored and every contraction below skips the
+// structural zeros (adding an exact zero never changes a sum: the same arithmetic as the full 4x4 contraction).
 #pragma once
 #include <cstdint>
 
 namespace cuharm {
 
-// one geometry record: 16 doubles = one 128-byte line, read as a warp-wide broadcast
+// one geometry record: 20 doubles = 160 bytes, read as a warp-wide broadcast.  g^{t phi} vanishes identically in
+// Kerr-Schild coordinates (and in Minkowski), so c03 is kept only for the export helper; the arithmetic skips it.
 struct Geom {
   double g00, g01, g03, g11, g13, g22, g33;  // g_{mu nu}
   double c00, c01, c03, c11, c13, c22, c33;  // g^{mu nu}
   double sg, alpha;                          // sqrt(-g), lapse 1/sqrt(-g^tt)
+  double ialpha, ac01;                       // 1/alpha, alpha g^{t1} = -beta^1/alpha
+  double isg, pad;                           // 1/sqrt(-g) (0 where sqrt(-g) = 0: the polar faces, A32)
 };
-static_assert(sizeof(Geom) == 128, "Geom must be one cache line");
+static_assert(sizeof(Geom) == 160, "Geom is 20 doubles");
 
 __device__ __forceinline__ Geom load_geom(const Geom* __restrict__ tab, int q) {
   const double2* s = reinterpret_cast<const double2*>(tab + q);
@@ -32,7 +35,30 @@ __device__ __forceinline__ Geom load_geom(const Geom* __restrict__ tab, int q) {
   v = __ldg(s + 5); G.c11 = v.x; G.c13 = v.y;
   v = __ldg(s + 6); G.c22 = v.x; G.c33 = v.y;
   v = __ldg(s + 7); G.sg = v.x; G.alpha = v.y;
+  v = __ldg(s + 8); G.ialpha = v.x; G.ac01 = v.y;
+  v = __ldg(s + 9); G.isg = v.x; G.pad = 0.0;
   return G;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Reciprocal and reciprocal square root for the hot path: the hardware seed (MUFU.RCP64H / MUFU.RSQ64H, about 20
+// good bits) plus ONE third-order Newton step, no special-case path.  Result within 2 ulp for normal, finite
+// arguments; callers guarantee that (x > 0 where a root is taken, |x| far from the subnormal range).  The IEEE
+// division sequence nvcc emits costs three times the fp64 instructions and enters a ~100-instruction slow path
+// whenever the NUMERATOR is zero — which it is (B = 0) in 90 % of the zones of a torus workload.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double frcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  const double e = fma(-x, r, 1.0);     // 1 - x r, |e| <~ 2^-20
+  return fma(r, fma(e, e, e), r);       // r (1 + e + e^2): error e^3
+}
+
+__device__ __forceinline__ double frsqrt(double x) {
+  double r;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  const double e = fma(-x * r, r, 1.0);               // 1 - x r^2
+  return fma(r, e * fma(0.375, e, 0.5), r);           // r (1 + e/2 + 3 e^2/8): error 5 e^3/16
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -61,22 +87,22 @@ __device__ __forceinline__ void lower(const Geom& G, double v0, double v1, doubl
 }
 
 __device__ __forceinline__ void fluid_state(const double q[8], const Geom& G, State& S) {
-  const double lor = sqrt(1.0 + gamma_sq_minus_one(q, G));  // Gamma
+  const double x = 1.0 + gamma_sq_minus_one(q, G);
+  const double ilor = frsqrt(x);
+  const double lor = x * ilor;  // Gamma = sqrt(1 + q^2)
   S.lor = lor;
-  const double a = G.alpha;
-  S.u0 = lor / a;
-  // beta^i / alpha = alpha g^{ti};  u^i = ut^i - Gamma beta^i / alpha  (eq. 10)
-  const double la = lor * a;
-  S.u1 = q[2] - la * G.c01;
+  S.u0 = lor * G.ialpha;
+  // beta^i / alpha = -alpha g^{ti};  u^i = ut^i - Gamma beta^i / alpha  (eq. 10);  g^{t2} = g^{t3} = 0
+  S.u1 = fma(-lor, G.ac01, q[2]);
   S.u2 = q[3];
-  S.u3 = q[4] - la * G.c03;
+  S.u3 = q[4];
   lower(G, S.u0, S.u1, S.u2, S.u3, S.l0, S.l1, S.l2, S.l3);
   const double bt = q[5] * S.l1 + q[6] * S.l2 + q[7] * S.l3;  // b^t = B^i u_i
-  const double iu0 = 1.0 / S.u0;
+  const double iu0 = G.alpha * ilor;
   S.b0 = bt;
-  S.b1 = (q[5] + bt * S.u1) * iu0;  // b^i = (B^i + b^t u^i) / u^t
-  S.b2 = (q[6] + bt * S.u2) * iu0;
-  S.b3 = (q[7] + bt * S.u3) * iu0;
+  S.b1 = fma(bt, S.u1, q[5]) * iu0;  // b^i = (B^i + b^t u^i) / u^t
+  S.b2 = fma(bt, S.u2, q[6]) * iu0;
+  S.b3 = fma(bt, S.u3, q[7]) * iu0;
   lower(G, S.b0, S.b1, S.b2, S.b3, S.m0, S.m1, S.m2, S.m3);
   S.bsq = S.b0 * S.m0 + S.b1 * S.m1 + S.b2 * S.m2 + S.b3 * S.m3;
 }
@@ -86,19 +112,19 @@ __device__ __forceinline__ double pick(int d, double a0, double a1, double a2, d
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Conserved variables (DIR = 0) and fluxes (DIR = 1,2,3): eqs. 5-8.
-//   [0] sqrt(-g) rho u^d   [1..4] sqrt(-g) T^d_nu   [5..7] sqrt(-g)(b^i u^d - b^d u^i)   (A1: sign; A18)
+// Conserved variables (DIR = 0) and fluxes (DIR = 1,2,3) DIVIDED BY sqrt(-g): eqs. 5-8.
+//   [0] rho u^d   [1..4] T^d_nu   [5..7] b^i u^d - b^d u^i   (A1: sign; A18)
+// For DIR = 0 the last three are B^i themselves: b^i u^t - b^t u^i = B^i by the definition of b^i.
 // ---------------------------------------------------------------------------------------------------------
 template <int DIR>
-__device__ __forceinline__ void flux_vector(const double q[8], const State& S, const Geom& G, double gam, double out[8]) {
+__device__ __forceinline__ void flux_hat(const double q[8], const State& S, double gam, double out[8]) {
   const double pg = (gam - 1.0) * q[1];
   const double w = q[0] + q[1] + pg;        // enthalpy density
   const double ud = pick(DIR, S.u0, S.u1, S.u2, S.u3);
   const double bd = pick(DIR, S.b0, S.b1, S.b2, S.b3);
   const double eta = (w + S.bsq) * ud;
-  const double ptot = pg + 0.5 * S.bsq;
-  const double sg = G.sg;
-  out[0] = sg * (q[0] * ud);
+  const double ptot = fma(0.5, S.bsq, pg);
+  out[0] = q[0] * ud;
   double t0 = eta * S.l0 - bd * S.m0;
   double t1 = eta * S.l1 - bd * S.m1;
   double t2 = eta * S.l2 - bd * S.m2;
@@ -107,117 +133,114 @@ __device__ __forceinline__ void flux_vector(const double q[8], const State& S, c
   if (DIR == 1) t1 += ptot;
   if (DIR == 2) t2 += ptot;
   if (DIR == 3) t3 += ptot;
-  out[1] = sg * t0;
-  out[2] = sg * t1;
-  out[3] = sg * t2;
-  out[4] = sg * t3;
-  out[5] = sg * (S.b1 * ud - bd * S.u1);
-  out[6] = sg * (S.b2 * ud - bd * S.u2);
-  out[7] = sg * (S.b3 * ud - bd * S.u3);
+  out[1] = t0;
+  out[2] = t1;
+  out[3] = t2;
+  out[4] = t3;
+  if (DIR == 0) {
+    out[5] = q[5]; out[6] = q[6]; out[7] = q[7];
+  } else {
+    out[5] = DIR == 1 ? 0.0 : S.b1 * ud - bd * S.u1;
+    out[6] = DIR == 2 ? 0.0 : S.b2 * ud - bd * S.u2;
+    out[7] = DIR == 3 ? 0.0 : S.b3 * ud - bd * S.u3;
+  }
+}
+
+template <int DIR>
+__device__ __forceinline__ void flux_vector(const double q[8], const State& S, const Geom& G, double gam, double out[8]) {
+  flux_hat<DIR>(q, S, gam, out);
+#pragma unroll
+  for (int v = 0; v < 8; v++) out[v] *= G.sg;
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Fast-magnetosonic bounds from the quadratic dispersion relation (eqs. 18-19): roots of
-// A v^2 + B v + C = 0, c1 >= c2.  A29: a negative discriminant is clamped to zero.
+// Fast-magnetosonic bounds from the quadratic dispersion relation (eqs. 18-19): the roots
+// cp >= cm of A v^2 + B v + C = 0.  c_ms^2 = v_a^2 + c_s^2 (1 - v_a^2) = (b^2 + gam p) / (b^2 + w).
+// A = (u^t)^2 (1 - c_ms^2) - c_ms^2 g^tt > 0 because g^tt < 0 everywhere in Kerr-Schild coordinates, so the
+// "+" root is the larger one.  A29: a negative discriminant is clamped to zero.
 // ---------------------------------------------------------------------------------------------------------
 template <int DIR>
-__device__ __forceinline__ void wave_speeds(const double q[8], const State& S, const Geom& G, double gam, double& c1,
-                                            double& c2) {
+__device__ __forceinline__ void wave_speeds(const double q[8], const State& S, const Geom& G, double gam, double& cp,
+                                            double& cm) {
   const double pg = (gam - 1.0) * q[1];
   const double w = q[0] + q[1] + pg;
-  const double cs2 = gam * pg / w;               // eq. 19
-  const double va2 = S.bsq / (S.bsq + w);
-  const double cms2 = va2 + cs2 * (1.0 - va2);   // eq. 18
+  const double cms2 = fma(gam, pg, S.bsq) * frcp(S.bsq + w);  // eqs. 18-19
   const double ut = S.u0;
   const double ud = pick(DIR, S.u0, S.u1, S.u2, S.u3);
-  const double gtd = DIR == 1 ? G.c01 : (DIR == 3 ? G.c03 : 0.0);
+  const double gtd = DIR == 1 ? G.c01 : 0.0;
   const double gdd = DIR == 1 ? G.c11 : (DIR == 2 ? G.c22 : G.c33);
-  const double A = ut * ut - cms2 * (G.c00 + ut * ut);
-  const double B = -2.0 * (ut * ud - cms2 * (gtd + ut * ud));
-  const double C = ud * ud - cms2 * (gdd + ud * ud);
-  double disc = B * B - 4.0 * A * C;
-  disc = disc < 0.0 ? 0.0 : disc;
-  const double sq = sqrt(disc);
-  const double i2A = 1.0 / (2.0 * A);
-  const double ra = (-B + sq) * i2A;
-  const double rb = (-B - sq) * i2A;
-  c1 = ra > rb ? ra : rb;
-  c2 = ra > rb ? rb : ra;
+  const double utt = ut * ut, utd = ut * ud, udd = ud * ud;
+  const double A = fma(-cms2, G.c00 + utt, utt);
+  const double hB = fma(-cms2, gtd + utd, utd);  // = -B/2
+  const double C = fma(-cms2, gdd + udd, udd);
+  double disc = fma(hB, hB, -A * C);             // (B^2 - 4AC)/4
+  disc = disc > 1e-300 ? disc : 1e-300;
+  const double sq = disc * frsqrt(disc);
+  const double iA = frcp(A);
+  cp = (hB + sq) * iA;
+  cm = (hB - sq) * iA;
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Reconstruction.  MC-limited slope, eq. 15 (A2: the last branch is signed).
+// Reconstruction.  MC-limited slope, eq. 15 (A2: the last branch is signed): for dm, dp of one sign the
+// one of {2 dm, 2 dp, (dm+dp)/2} of smallest magnitude, else 0.
 // ---------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double slope_mc(double qm, double q0, double qp) {
   const double dm = q0 - qm, dp = qp - q0;
   const double dc = 0.5 * (qp - qm);
-  const double am = 2.0 * fabs(dm), ap = 2.0 * fabs(dp), ac = fabs(dc);
-  // for dm, dp of one sign |dc| is the mean of |dm|, |dp|: at most one of the one-sided tests can hold
-  double s = dc;
-  s = (ap < ac) ? 2.0 * dp : s;
-  s = (am < ac && fabs(dm) < fabs(dp)) ? 2.0 * dm : s;
+  const double one = fabs(dm) < fabs(dp) ? dm : dp;  // the smaller one-sided difference
+  const double two = one + one;
+  const double s = fabs(two) < fabs(dc) ? two : dc;
   return (dm * dp < 0.0) ? 0.0 : s;
 }
 
-// Values at the lower (ql) and upper (qr) face of the cell y2 from the cell values y0..y4 around it.
-// RECON 0: piecewise linear, eq. 16.  RECON 1: piecewise parabolic (A20): MC-limited
-// slopes, 4th-order interface values, monotonisation; no steepening, no flattening.
-template <int RECON>
-__device__ __forceinline__ void recon_cell(double y0, double y1, double y2, double y3, double y4, double& ql, double& qr) {
-  if (RECON == 0) {
-    const double dq = slope_mc(y1, y2, y3);
-    ql = y2 - 0.5 * dq;
-    qr = y2 + 0.5 * dq;
-  } else {
-    const double dm = slope_mc(y0, y1, y2);
-    const double d0 = slope_mc(y1, y2, y3);
-    const double dp = slope_mc(y2, y3, y4);
-    double l = 0.5 * (y1 + y2) - (d0 - dm) / 6.0;
-    double r = 0.5 * (y2 + y3) - (dp - d0) / 6.0;
-    if ((r - y2) * (y2 - l) <= 0.0) {
-      l = y2;
-      r = y2;
-    } else {
-      const double d = r - l;
-      const double m6 = d * (y2 - 0.5 * (l + r));
-      const double lim = d * d / 6.0;
-      if (m6 > lim) l = 3.0 * y2 - 2.0 * r;
-      else if (m6 < -lim) r = 3.0 * y2 - 2.0 * l;
-    }
-    ql = l;
-    qr = r;
-  }
+// PPM (A20): 4th-order edge value between cells 0 and 1 from their values and MC slopes ...
+__device__ __forceinline__ double ppm_edge(double y0, double y1, double s0, double s1) {
+  return fma(-1.0 / 6.0, s1 - s0, 0.5 * (y0 + y1));
+}
+
+// ... and the monotonisation of the parabola of a cell with value y and edge values l (lower), r (upper).
+__device__ __forceinline__ void ppm_mono(double y, double& l, double& r) {
+  const double d = r - l;
+  const double m6 = d * (y - 0.5 * (l + r));
+  const double lim = d * d * (1.0 / 6.0);
+  const double l2 = fma(-2.0, r, 3.0 * y), r2 = fma(-2.0, l, 3.0 * y);
+  const bool flat = (r - y) * (y - l) <= 0.0;
+  const bool lo = m6 > lim, hi = m6 < -lim;
+  l = flat ? y : (lo ? l2 : l);
+  r = flat ? y : ((!lo && hi) ? r2 : r);
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // Riemann flux at one face from the two reconstructed states and the FACE metric.
 // RIEMANN 0: local Lax-Friedrichs, eq. 17.  RIEMANN 1: HLL, eq. 20 (A30: guarded denominator).
+// sqrt(-g) multiplies the combination once (it is common to U^l, U^r, F^l, F^r at a face).
 // ---------------------------------------------------------------------------------------------------------
 template <int DIR, int RIEMANN>
 __device__ __forceinline__ void face_flux(const double pl[8], const double pr[8], const Geom& G, double gam, double F[8],
                                           double& cw) {
-  State S;
-  double Ul[8], Fl[8], c1l, c2l;
-  fluid_state(pl, G, S);
-  flux_vector<0>(pl, S, G, gam, Ul);
-  flux_vector<DIR>(pl, S, G, gam, Fl);
-  wave_speeds<DIR>(pl, S, G, gam, c1l, c2l);
-  double Ur[8], Fr[8], c1r, c2r;
-  fluid_state(pr, G, S);
-  flux_vector<0>(pr, S, G, gam, Ur);
-  flux_vector<DIR>(pr, S, G, gam, Fr);
-  wave_speeds<DIR>(pr, S, G, gam, c1r, c2r);
-  const double cmax = fmax(0.0, fmax(c1r, c1l));
-  const double cmin = fmax(0.0, fmax(-c2r, -c2l));
+  State Sl, Sr;
+  double Ul[8], Fl[8], Ur[8], Fr[8], cpl, cml, cpr, cmr;
+  fluid_state(pl, G, Sl);
+  fluid_state(pr, G, Sr);
+  flux_hat<0>(pl, Sl, gam, Ul);
+  flux_hat<0>(pr, Sr, gam, Ur);
+  flux_hat<DIR>(pl, Sl, gam, Fl);
+  flux_hat<DIR>(pr, Sr, gam, Fr);
+  wave_speeds<DIR>(pl, Sl, G, gam, cpl, cml);
+  wave_speeds<DIR>(pr, Sr, G, gam, cpr, cmr);
+  const double cmax = fmax(0.0, fmax(cpr, cpl));
+  const double cmin = fmax(0.0, fmax(-cmr, -cml));
   cw = fmax(cmax, cmin);
   if (RIEMANN == 0) {
+    const double hsg = 0.5 * G.sg;
 #pragma unroll
-    for (int v = 0; v < 8; v++) F[v] = 0.5 * (Fl[v] + Fr[v] - cw * (Ur[v] - Ul[v]));
+    for (int v = 0; v < 8; v++) F[v] = hsg * fma(-cw, Ur[v] - Ul[v], Fl[v] + Fr[v]);
   } else {
-    const double iden = 1.0 / fmax(cmax + cmin, 1e-300);
+    const double sc = G.sg * frcp(fmax(cmax + cmin, 1e-300));
     const double cc = cmax * cmin;
 #pragma unroll
-    for (int v = 0; v < 8; v++) F[v] = (cmax * Fl[v] + cmin * Fr[v] - cc * (Ur[v] - Ul[v])) * iden;
+    for (int v = 0; v < 8; v++) F[v] = sc * fma(-cc, Ur[v] - Ul[v], fma(cmax, Fl[v], cmin * Fr[v]));
   }
 }
 
@@ -225,7 +248,7 @@ __device__ __forceinline__ void face_flux(const double pl[8], const double pr[8]
 // Geometric source S_nu = sqrt(-g) T^kappa_lambda Gamma^lambda_{nu kappa} (eq. 7; eq. 14).
 // conn: 40 doubles, Gamma^l_{nk} with l-major and the (n,k) pair order 00 01 02 03 11 12 13 22 23 33.
 // ---------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ int pair_index(int n, int k) {
+__device__ __forceinline__ constexpr int pair_index(int n, int k) {
   // index of the unordered pair (n,k) in 00 01 02 03 11 12 13 22 23 33
   const int lo = n < k ? n : k, hi = n < k ? k : n;
   return lo * 4 - (lo * (lo - 1)) / 2 + (hi - lo);
@@ -236,23 +259,27 @@ __device__ __forceinline__ void source_term(const double q[8], const State& S, c
   const double pg = (gam - 1.0) * q[1];
   const double w = q[0] + q[1] + pg;
   const double eta = w + S.bsq;
-  const double ptot = pg + 0.5 * S.bsq;
+  const double ptot = fma(0.5, S.bsq, pg);
   const double uc[4] = {S.u0, S.u1, S.u2, S.u3}, ul[4] = {S.l0, S.l1, S.l2, S.l3};
   const double bc[4] = {S.b0, S.b1, S.b2, S.b3}, bl[4] = {S.m0, S.m1, S.m2, S.m3};
-  double T[4][4];  // T^k_l
+  double cn[40];
+  const double2* c2 = reinterpret_cast<const double2*>(conn);
 #pragma unroll
-  for (int k = 0; k < 4; k++)
+  for (int s = 0; s < 20; s++) { const double2 v = __ldg(c2 + s); cn[2 * s] = v.x; cn[2 * s + 1] = v.y; }
+  double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
 #pragma unroll
-    for (int l = 0; l < 4; l++) T[k][l] = eta * uc[k] * ul[l] + (k == l ? ptot : 0.0) - bc[k] * bl[l];
+  for (int k = 0; k < 4; k++) {
+    const double eu = eta * uc[k];
 #pragma unroll
-  for (int nu = 0; nu < 4; nu++) {
-    double s = 0.0;
-#pragma unroll
-    for (int k = 0; k < 4; k++)
-#pragma unroll
-      for (int l = 0; l < 4; l++) s += T[k][l] * __ldg(conn + l * 10 + pair_index(nu, k));
-    src[nu] = G.sg * s;
+    for (int l = 0; l < 4; l++) {
+      const double T = fma(eu, ul[l], -bc[k] * bl[l]) + (k == l ? ptot : 0.0);  // T^k_l
+      s0 = fma(T, cn[l * 10 + pair_index(0, k)], s0);
+      s1 = fma(T, cn[l * 10 + pair_index(1, k)], s1);
+      s2 = fma(T, cn[l * 10 + pair_index(2, k)], s2);
+      s3 = fma(T, cn[l * 10 + pair_index(3, k)], s3);
+    }
   }
+  src[0] = G.sg * s0; src[1] = G.sg * s1; src[2] = G.sg * s2; src[3] = G.sg * s3;
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -265,10 +292,10 @@ struct NewtonCfg {
   int maxit, extra;
 };
 
-__device__ __noinline__ int invert_2d(const double U[8], const Geom& G, double gam, double q[8], NewtonCfg nc, int& iters) {
+__device__ __forceinline__ int invert_2d(const double U[8], const Geom& G, double gam, double q[8], NewtonCfg nc, int& iters) {
   iters = 0;
   const double a = G.alpha;
-  const double isg = 1.0 / G.sg;
+  const double isg = G.isg;
   const double B1 = U[5] * isg, B2 = U[6] * isg, B3 = U[7] * isg;
   const double g1 = q[2], g2 = q[3], g3 = q[4];  // guess velocity
   const double grho = q[0], gu = q[1];
@@ -279,61 +306,65 @@ __device__ __noinline__ int invert_2d(const double U[8], const Geom& G, double g
   const double Bc1 = a * B1, Bc2 = a * B2, Bc3 = a * B3;                                  // script-B^i
   const bool fin = isfinite(D) && isfinite(Q0) && isfinite(Q1) && isfinite(Q2) && isfinite(Q3) && isfinite(Bc1) &&
                    isfinite(Bc2) && isfinite(Bc3);
-  if (!fin || !(D > 0.0)) return 1;
-  // Q^mu = g^{mu nu} Q_nu
-  const double Qc0 = G.c00 * Q0 + G.c01 * Q1 + G.c03 * Q3;
+  if (!fin || !(D > 0.0) || !(isg > 0.0)) return 1;
+  // Q^mu = g^{mu nu} Q_nu  (g^{t phi} = 0)
+  const double Qc0 = G.c00 * Q0 + G.c01 * Q1;
   const double Qc1 = G.c01 * Q0 + G.c11 * Q1 + G.c13 * Q3;
   const double Qc2 = G.c22 * Q2;
-  const double Qc3 = G.c03 * Q0 + G.c13 * Q1 + G.c33 * Q3;
+  const double Qc3 = G.c13 * Q1 + G.c33 * Q3;
   const double Bsq = G.g11 * Bc1 * Bc1 + G.g22 * Bc2 * Bc2 + G.g33 * Bc3 * Bc3 + 2.0 * (G.g13 * Bc1 * Bc3);
   const double QdB = Q1 * Bc1 + Q2 * Bc2 + Q3 * Bc3;
   // n_mu = (-alpha,0,0,0); n^mu = (1/alpha, -alpha g^{ti})
-  const double n0 = 1.0 / a, n1 = -a * G.c01, n3 = -a * G.c03;
-  const double Qdn = Q0 * n0 + Q1 * n1 + Q3 * n3;
+  const double n1 = -G.ac01;
+  const double Qdn = fma(Q0, G.ialpha, Q1 * n1);
   const double Qsq = Qc0 * Q0 + Qc1 * Q1 + Qc2 * Q2 + Qc3 * Q3;
-  const double Qtsq = Qsq + Qdn * Qdn;
+  const double Qtsq = fma(Qdn, Qdn, Qsq);
   const double QdB2 = QdB * QdB;
-  const double gfac = (gam - 1.0) / gam;
+  const double igam = frcp(gam);
+  const double gfac = (gam - 1.0) * igam;
   // initial guess: W = Gamma^2 w from the guess, v^2 from eq. 29 at that W
   const double qsq = G.g11 * g1 * g1 + G.g22 * g2 * g2 + G.g33 * g3 * g3 + 2.0 * (G.g13 * g1 * g3);
-  double W = (1.0 + qsq) * (grho + gam * gu);
+  double W = (1.0 + qsq) * fma(gam, gu, grho);
+  if (!(W > 0.0) || !isfinite(W)) return 3;
   double v2 = 0.0;
   for (int t = 0; t < 400; t++) {
-    v2 = (Qtsq + QdB2 * (Bsq + 2.0 * W) / (W * W)) / ((Bsq + W) * (Bsq + W));
-    if (v2 < 1.0) break;
+    const double iW = frcp(W), iBW = frcp(Bsq + W);
+    v2 = fma(QdB2 * fma(2.0, W, Bsq), iW * iW, Qtsq) * (iBW * iBW);
+    if (v2 < 1.0 || !(W < 1e300)) break;
     W *= 10.0;
   }
-  if (!(v2 < 1.0) || !(W > 0.0)) return 3;
+  if (!(v2 < 1.0)) return 3;
   v2 = v2 < 0.0 ? 0.0 : v2;
   bool converged = false;
   int extra_left = -1;
   int it;
   for (it = 1; it <= nc.maxit; it++) {
-    const double iW = 1.0 / W;
+    const double iW = frcp(W);
     const double iW2 = iW * iW, iW3 = iW2 * iW;
     const double omv = 1.0 - v2;
-    const double sq = sqrt(omv);
+    const double isq = frsqrt(omv);
+    const double sq = omv * isq;
     const double BW = Bsq + W;
-    const double pg = gfac * (W * omv - D * sq);                                   // eq. 31
-    const double f1 = Qtsq - v2 * BW * BW + QdB2 * (Bsq + 2.0 * W) * iW2;          // eq. 29
-    const double f2 = -Qdn - 0.5 * Bsq * (1.0 + v2) + 0.5 * QdB2 * iW2 - W + pg;   // eq. 30 (A6)
-    const double j11 = -2.0 * BW * (v2 + QdB2 * iW3);
+    const double pg = gfac * fma(W, omv, -D * sq);                                  // eq. 31
+    const double f1 = fma(QdB2 * fma(2.0, W, Bsq), iW2, fma(-v2 * BW, BW, Qtsq));    // eq. 29
+    const double f2 = fma(0.5 * QdB2, iW2, fma(-0.5 * Bsq, 1.0 + v2, -Qdn)) - W + pg;  // eq. 30 (A6)
+    const double j11 = -2.0 * BW * fma(QdB2, iW3, v2);
     const double j12 = -BW * BW;
-    const double j21 = -1.0 - QdB2 * iW3 + gfac * omv;
-    const double j22 = -0.5 * Bsq + gfac * (-W + D / (2.0 * sq));
-    const double idet = 1.0 / (j11 * j22 - j12 * j21);
-    const double dW = (-f1 * j22 + f2 * j12) * idet;
-    const double dv = (-f2 * j11 + f1 * j21) * idet;
+    const double j21 = fma(gfac, omv, fma(-QdB2, iW3, -1.0));
+    const double j22 = fma(gfac, fma(0.5 * D, isq, -W), -0.5 * Bsq);
+    const double idet = frcp(fma(j11, j22, -j12 * j21));
+    const double dW = fma(f2, j12, -f1 * j22) * idet;
+    const double dv = fma(f1, j21, -f2 * j11) * idet;
     const double Wn = fabs(W + dW);
     double vn = v2 + dv;
     vn = vn < 0.0 ? 0.0 : vn;
     vn = vn > 1.0 - 1e-15 ? 1.0 - 1e-15 : vn;
-    const double err = (Wn == 0.0) ? fabs(dW) : fabs(dW / Wn);
+    const bool small = (Wn == 0.0) ? (fabs(dW) <= nc.tol) : (fabs(dW) <= nc.tol * Wn);  // |dW/W| <= tol
     W = Wn;
     v2 = vn;
-    if (!isfinite(W) || !isfinite(v2)) { iters = it; return 3; }
+    if (!isfinite(W) || !isfinite(v2) || W == 0.0) { iters = it; return 3; }
     if (extra_left < 0) {
-      if (err <= nc.tol) extra_left = nc.extra;
+      if (small) extra_left = nc.extra;
     } else {
       extra_left--;
     }
@@ -343,20 +374,28 @@ __device__ __noinline__ int invert_2d(const double U[8], const Geom& G, double g
   if (!converged) return 2;
   if (!(W > 0.0)) return 3;
   if (!(v2 >= 0.0 && v2 < 1.0)) return 4;
-  const double lor = 1.0 / sqrt(1.0 - v2);
-  const double rho = D / lor;
-  const double w = W * (1.0 - v2);
-  const double u = (w - rho) / gam;
+  const double omv = 1.0 - v2;
+  const double lor = frsqrt(omv);
+  const double rho = D * (omv * lor);  // D / Gamma
+  const double w = W * omv;
+  const double u = (w - rho) * igam;
   if (!(rho > 0.0)) return 5;
   if (!(u >= 0.0)) return 6;
   q[0] = rho;
   q[1] = u;
-  const double f = lor / (W + Bsq);
-  const double QdBW = QdB / W;
-  q[2] = f * (Qc1 + n1 * Qdn + QdBW * Bc1);  // ut^i = Gamma [Qt^i + (Q.B) B^i / W] / (W + B^2)
-  q[3] = f * (Qc2 + QdBW * Bc2);
-  q[4] = f * (Qc3 + n3 * Qdn + QdBW * Bc3);
+  const double f = lor * frcp(W + Bsq);
+  const double QdBW = QdB * frcp(W);
+  q[2] = f * (fma(n1, Qdn, Qc1) + QdBW * Bc1);  // ut^i = Gamma [Qt^i + (Q.B) B^i / W] / (W + B^2)
+  q[3] = f * fma(QdBW, Bc2, Qc2);
+  q[4] = f * fma(QdBW, Bc3, Qc3);
   return 0;
+}
+
+// out-of-line copy for rare paths (the ceiling re-inversion)
+__device__ __noinline__ int invert_2d_cold(const double* U, const Geom* Gp, double gam, double* q, NewtonCfg nc) {
+  int its;
+  const Geom G = load_geom(Gp, 0);
+  return invert_2d(U, G, gam, q, nc, its);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -365,54 +404,67 @@ __device__ __noinline__ int invert_2d(const double U[8], const Geom& G, double g
 // ---------------------------------------------------------------------------------------------------------
 struct FloorCfg {
   double sigma_max, b2_over_u_max, gamma_max;
+  double isigma, ib2u;  // reciprocals of the two ceilings (host-computed; 0 when the ceiling is disabled)
 };
 
-__device__ __forceinline__ int apply_floors(double q[8], const Geom& G, double rfl, double ufl, FloorCfg fc, double gam,
-                                            NewtonCfg nc) {
+// rare path of the ceilings: mass / energy injected at rest in the normal-observer frame, re-inversion (A11)
+__device__ __noinline__ int apply_ceilings_cold(double* q, const Geom* Gp, double drho, double du, FloorCfg fc, double gam,
+                                                NewtonCfg nc) {
+  const Geom G = load_geom(Gp, 0);
+  int mask = 4;
+  State S;
+  fluid_state(q, G, S);
+  double U[8], Ua[8];
+  flux_vector<0>(q, S, G, gam, U);
+  double qa[8] = {drho, du, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+  State Sa;
+  fluid_state(qa, G, Sa);
+  flux_vector<0>(qa, Sa, G, gam, Ua);
+  for (int v = 0; v < 8; v++) U[v] += Ua[v];
+  double t[8];
+  for (int v = 0; v < 8; v++) t[v] = q[v];
+  const int flag = invert_2d_cold(U, Gp, gam, t, nc);
+  if (flag == 0) {
+    for (int v = 0; v < 5; v++) q[v] = t[v];
+  } else {
+    q[0] += drho;
+    q[1] += du;
+    mask |= 16;
+  }
+  State S2;
+  fluid_state(q, G, S2);
+  if (fc.sigma_max > 0.0) q[0] = fmax(q[0], S2.bsq * fc.isigma);
+  if (fc.b2_over_u_max > 0.0) q[1] = fmax(q[1], S2.bsq * fc.ib2u);
+  return mask;
+}
+
+__device__ __forceinline__ int apply_floors(double q[8], const Geom& G, const Geom* Gp, double rfl, double ufl, FloorCfg fc,
+                                            double gam, NewtonCfg nc) {
   int mask = 0;
   if (q[0] < rfl) { q[0] = rfl; mask |= 1; }
   if (q[1] < ufl) { q[1] = ufl; mask |= 2; }
+  const double qsq = gamma_sq_minus_one(q, G);
   if (fc.sigma_max > 0.0 || fc.b2_over_u_max > 0.0) {
-    // b^2 by the identity b^2 = (B^2 + (B.u)^2) / Gamma^2 would be cheaper, but the state is needed below anyway
-    State S;
-    fluid_state(q, G, S);
+    // b^2 = (g_ij B^i B^j + (b^t)^2) / (u^t)^2 with b^t = B^i u_i  (from b^i = (B^i + b^t u^i)/u^t and b.u = 0)
+    const double lor2 = 1.0 + qsq;
+    const double lor = lor2 * frsqrt(lor2);
+    const double u0 = lor * G.ialpha;
+    const double u1 = fma(-lor, G.ac01, q[2]);
+    const double l1 = G.g01 * u0 + G.g11 * u1 + G.g13 * q[4];
+    const double l2 = G.g22 * q[3];
+    const double l3 = G.g03 * u0 + G.g13 * u1 + G.g33 * q[4];
+    const double bt = q[5] * l1 + q[6] * l2 + q[7] * l3;
+    const double B2 = G.g11 * q[5] * q[5] + G.g22 * q[6] * q[6] + G.g33 * q[7] * q[7] + 2.0 * (G.g13 * q[5] * q[7]);
+    const double bsq = fma(bt, bt, B2) * (G.alpha * G.alpha) * frcp(lor2);
     double drho = 0.0, du = 0.0;
-    if (fc.sigma_max > 0.0) drho = fmax(0.0, S.bsq / fc.sigma_max - q[0]);
-    if (fc.b2_over_u_max > 0.0) du = fmax(0.0, S.bsq / fc.b2_over_u_max - q[1]);
-    if (drho > 0.0 || du > 0.0) {  // rare: mass/energy injected at rest in the normal-observer frame (A11)
-      mask |= 4;
-      double U[8], Ua[8];
-      flux_vector<0>(q, S, G, gam, U);
-      double qa[8] = {drho, du, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-      State Sa;
-      fluid_state(qa, G, Sa);
-      flux_vector<0>(qa, Sa, G, gam, Ua);
-#pragma unroll
-      for (int v = 0; v < 8; v++) U[v] += Ua[v];
-      double t[8];
-#pragma unroll
-      for (int v = 0; v < 8; v++) t[v] = q[v];
-      int its;
-      const int flag = invert_2d(U, G, gam, t, nc, its);
-      if (flag == 0) {
-#pragma unroll
-        for (int v = 0; v < 5; v++) q[v] = t[v];
-      } else {
-        q[0] += drho;
-        q[1] += du;
-        mask |= 16;
-      }
-      State S2;
-      fluid_state(q, G, S2);
-      if (fc.sigma_max > 0.0) q[0] = fmax(q[0], S2.bsq / fc.sigma_max);
-      if (fc.b2_over_u_max > 0.0) q[1] = fmax(q[1], S2.bsq / fc.b2_over_u_max);
-    }
+    if (fc.sigma_max > 0.0) drho = fmax(0.0, fma(bsq, fc.isigma, -q[0]));
+    if (fc.b2_over_u_max > 0.0) du = fmax(0.0, fma(bsq, fc.ib2u, -q[1]));
+    if (drho > 0.0 || du > 0.0) mask |= apply_ceilings_cold(q, Gp, drho, du, fc, gam, nc);
   }
   if (fc.gamma_max > 0.0) {
-    const double qsq = gamma_sq_minus_one(q, G);
-    const double lor = sqrt(1.0 + qsq);
-    if (lor > fc.gamma_max) {
-      const double f = sqrt((fc.gamma_max * fc.gamma_max - 1.0) / (lor * lor - 1.0));  // A12
+    const double q2 = (mask & 4) ? gamma_sq_minus_one(q, G) : qsq;
+    if (q2 > fc.gamma_max * fc.gamma_max - 1.0) {
+      const double f = sqrt((fc.gamma_max * fc.gamma_max - 1.0) / q2);  // A12
       q[2] *= f; q[3] *= f; q[4] *= f;
       mask |= 8;
     }
