@@ -59,6 +59,8 @@ struct cuharm_ctx {
   double t_ms[CUHARM_NCLASS] = {0};
   int64_t t_n[CUHARM_NCLASS] = {0};
   // graph
+  bool upd_tma = false;  // update_tma_kernel usable (shared-memory opt-in succeeded)
+  int upd_blocks = 0;    // its persistent grid size
   bool use_graph = false;
   cudaGraphExec_t gexec = nullptr;
   cudaStream_t cap_stream = nullptr;
@@ -156,8 +158,8 @@ void launch_flux_t(cuharm_ctx* h, FluxArgs& a, int dir) {
   const int ni = a.hi1 - a.lo1 + 1, nj = a.hi2 - a.lo2 + 1, nk = a.hi3 - a.lo3 + 1;
   if (dir == 3) {
     const int fpw = FluxK<RECON>::FPW;
-    const long long warps = (long long)ni * nj * ((nk + fpw - 1) / fpw);
-    flux_k_kernel<RECON, RIEMANN, STAGE><<<(unsigned)((warps + 3) / 4), 128, 0, h->stream>>>(a);
+    const dim3 grid((unsigned)((nk + fpw - 1) / fpw), (unsigned)((nj + 3) / 4), (unsigned)ni);
+    flux_k_kernel<RECON, RIEMANN, STAGE><<<grid, 128, 0, h->stream>>>(a);
   } else {
     const long long cols = (long long)(dir == 1 ? nj : ni) * nk;
     const int nf = dir == 1 ? ni : nj;
@@ -212,8 +214,22 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
               nfail, h->cnt + CNT_STATS, dtau, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], h->p.gam,
               newton_cfg(h->p), floor_cfg(h->p)};
     dim3 grid((d.n3 + 127) / 128, d.n2, d.n1);
-    if (Pflux == Pbase) update_kernel<true><<<grid, 128, 0, h->stream>>>(a);
-    else update_kernel<false><<<grid, 128, 0, h->stream>>>(a);
+    // bulk-copy (TMA) staging needs 16-byte aligned row segments: even n3g and 16-byte aligned arrays
+    const uintptr_t al = (uintptr_t)Pbase | (uintptr_t)Pflux | (uintptr_t)h->F[0] | (uintptr_t)h->F[1] |
+                         (uintptr_t)h->F[2] | (uintptr_t)h->E;
+    const bool tma = h->upd_tma && (d.n3g % 2 == 0) && (al % 16 == 0);
+    const size_t smem = (size_t)UPD_NROW * UPD_ROW * sizeof(double);
+    if (tma) {
+      const int nch = (d.n3 + 127) / 128;
+      const long long nt = (long long)d.n1 * d.n2 * nch;
+      const int ntiles = (int)nt;
+      const int nb = (int)std::min<long long>(nt, h->upd_blocks);
+      if (Pflux == Pbase) update_tma_kernel<true><<<nb, 128, smem, h->stream>>>(a, ntiles, nch);
+      else update_tma_kernel<false><<<nb, 128, smem, h->stream>>>(a, ntiles, nch);
+    } else {
+      if (Pflux == Pbase) update_kernel<true><<<grid, 128, 0, h->stream>>>(a);
+      else update_kernel<false><<<grid, 128, 0, h->stream>>>(a);
+    }
     h->launches++;
   }
   CK(cudaGetLastError());
@@ -287,6 +303,24 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
   } else {
     const int n[3] = {p->n1, p->n2, p->n3};
     for (int c = 0; c < 3; c++) { h->x0[c] = p->xmin[c]; h->dx[c] = (p->xmax[c] - p->xmin[c]) / n[c]; }
+  }
+  {  // opt in to the dynamic shared memory of the bulk-copy update kernel (51.7 KB per block)
+    const int smem = UPD_NROW * UPD_ROW * (int)sizeof(double);
+    const cudaError_t e1 = cudaFuncSetAttribute(update_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    const cudaError_t e2 = cudaFuncSetAttribute(update_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    h->upd_tma = (e1 == cudaSuccess && e2 == cudaSuccess);
+    if (h->upd_tma) {  // persistent grid: every SM filled with as many blocks as fit
+      int dev = 0, sms = 0, per = 0;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, update_tma_kernel<false>, 128, smem) != cudaSuccess || per < 1)
+        h->upd_tma = false;
+      h->upd_blocks = sms * per;
+    }
+    if (!h->upd_tma) cudaGetLastError();
+#ifdef CUHARM_NO_TMA
+    h->upd_tma = false;
+#endif
   }
   *out = h;
   return CUHARM_OK;

@@ -12,7 +12,8 @@
 //     MC slope, the unlimited PPM edge value and the limited upper-edge state of the previous cell in registers;
 //     k is the lane index, so every load and store is coalesced and the face geometry is a broadcast;
 //   direction 3: a lane owns one cell along k; the neighbour's slope, edge value and limited state arrive by warp
-//     shuffle; a warp of 32 cells yields 29 (PPM) or 31 (PLM) faces, consecutive warps overlap by the difference.
+//     shuffle; a warp of 32 cells yields 29 (PPM) or 31 (PLM) faces, consecutive warps overlap by the difference;
+//     the 4 warps of a block take 4 consecutive rows j at the same position along k.
 #pragma once
 #include "cuharm_phys.cuh"
 
@@ -70,9 +71,33 @@ __device__ __forceinline__ void store_flux(const FluxArgs& a, long long idx, con
 
 // ---------------------------------------------------------------------------------------------------------
 // Directions 1 and 2: marching.  grid.x covers the flattened (transverse index, k) plane, grid.y the segments.
+// Per variable a thread carries, for the face f it is about to do: yc = y_f, yn = y_{f+1}, dn = y_{f+1} - y_f,
+// the doubled MC slope sc of cell f, the unlimited edge value elo at f-1/2, the limited upper-edge state rprev of
+// cell f-1, and `pre` = y_{f+2}, loaded one iteration ahead so that its DRAM latency hides behind a whole face.
 // ---------------------------------------------------------------------------------------------------------
+#ifndef CUHARM_MARCH_PF
+#define CUHARM_MARCH_PF 1   // software prefetch distance (faces beyond the register look-ahead); 0 = off
+#endif
+#ifndef CUHARM_PF_LEVEL
+#define CUHARM_PF_LEVEL 1
+#endif
+__device__ __forceinline__ void prefetch_l1(const void* p) {
+#if CUHARM_PF_LEVEL == 1
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+#else
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+#endif
+}
+
+#ifndef CUHARM_MARCH_UNROLL
+#define CUHARM_MARCH_UNROLL 2
+#endif
+#ifndef CUHARM_MARCH_MINB
+#define CUHARM_MARCH_MINB 2
+#endif
+
 template <int DIR, int RECON, int RIEMANN, bool STAGE>
-__global__ void __launch_bounds__(128) flux_march_kernel(FluxArgs a) {
+__global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(FluxArgs a) {
   static_assert(DIR == 1 || DIR == 2, "marching kernel: directions 1 and 2");
   const Dims& d = a.d;
   const int nk = a.hi3 - a.lo3 + 1;
@@ -87,53 +112,87 @@ __global__ void __launch_bounds__(128) flux_march_kernel(FluxArgs a) {
     const int flo = DIR == 1 ? a.lo1 : a.lo2, fhi = DIR == 1 ? a.hi1 : a.hi2;
     const int fa = flo + blockIdx.y * a.seg;
     const int fb = min(fa + a.seg, fhi + 1);
+    const int nd = DIR == 1 ? d.n1g : d.n2g;  // extent of the marching direction (for the look-ahead clamp)
     // element offset of cell fa in this column; geometry index of face fa and its stride
-    const double* y = a.P + (DIR == 1 ? (long long)t * d.s2 : (long long)t * d.s1) + k + (long long)fa * sd;
     long long idx = (DIR == 1 ? (long long)t * d.s2 : (long long)t * d.s1) + k + (long long)fa * sd;
+    const double* y = a.P + idx;
     int gq = DIR == 1 ? fa * d.n2g + t : t * d.n2g + fa;
     const int gstep = DIR == 1 ? d.n2g : 1;
-    double rprev[8], sc[8], elo[8];
-    // prologue: limited upper-edge state of cell fa-1 (and, for PPM, slope of cell fa and edge value fa-1/2)
+    double yc[8], yn[8], dn[8], sc[8], elo[8], rprev[8], pre[8];
+    // prologue: state of the carried quantities at face fa
 #pragma unroll
     for (int v = 0; v < 8; v++) {
       const double* yv = y + v * nz;
       if (RECON == 0) {
-        const double ym2 = yv[-2 * sd], ym1 = yv[-sd], y0 = yv[0];
-        rprev[v] = fma(0.5, slope_mc(ym2, ym1, y0), ym1);
+        const double ym2 = yv[-2 * sd], ym1 = yv[-sd];
+        yc[v] = yv[0];
+        yn[v] = yv[sd];
+        double l;
+        plm_faces(ym1, slope2_mc(ym1 - ym2, yc[v] - ym1), l, rprev[v]);
+        dn[v] = yc[v] - ym1;  // PLM carries the LOWER difference of cell f
+        pre[v] = yv[(fa + 2 < nd ? 2 : 1) * sd];
       } else {
-        const double ym3 = yv[-3 * sd], ym2 = yv[-2 * sd], ym1 = yv[-sd], y0 = yv[0], y1 = yv[sd];
-        const double sm2 = slope_mc(ym3, ym2, ym1), sm1 = slope_mc(ym2, ym1, y0);
-        sc[v] = slope_mc(ym1, y0, y1);
+        const double ym3 = yv[-3 * sd], ym2 = yv[-2 * sd], ym1 = yv[-sd];
+        yc[v] = yv[0];
+        yn[v] = yv[sd];
+        const double d32 = ym2 - ym3, d21 = ym1 - ym2, d10 = yc[v] - ym1;
+        dn[v] = yn[v] - yc[v];
+        const double sm2 = slope2_mc(d32, d21), sm1 = slope2_mc(d21, d10);
+        sc[v] = slope2_mc(d10, dn[v]);
         double l = ppm_edge(ym2, ym1, sm2, sm1);
-        double r = ppm_edge(ym1, y0, sm1, sc[v]);
+        double r = ppm_edge(ym1, yc[v], sm1, sc[v]);
         elo[v] = r;
         ppm_mono(ym1, l, r);
         rprev[v] = r;
+        pre[v] = yv[2 * sd];
       }
     }
+    constexpr int UNR = CUHARM_MARCH_UNROLL;
+#pragma unroll UNR
     for (int f = fa; f < fb; f++) {
       double pl[8], pr[8];
+      // look-ahead load for the next face (clamped at the end of the array; the clamped value is never used)
+      const long long ahead = (f + 3 < nd ? 3 : 2) * sd;
+#if CUHARM_MARCH_PF
+      {
+        const long long far = (f + 3 + CUHARM_MARCH_PF < nd ? 3 + CUHARM_MARCH_PF : 2) * sd;
+#pragma unroll
+        for (int v = 0; v < 8; v++) prefetch_l1(y + v * nz + far);
+        prefetch_l1(reinterpret_cast<const char*>(a.Gf + gq + gstep));
+        prefetch_l1(reinterpret_cast<const char*>(a.Gf + gq + gstep) + 128);
+      }
+#endif
 #pragma unroll
       for (int v = 0; v < 8; v++) {
-        const double* yv = y + v * nz;
+        const double nxt = y[v * nz + ahead];
         if (RECON == 0) {
-          const double ym1 = yv[-sd], y0 = yv[0], y1 = yv[sd];
-          const double hs = 0.5 * slope_mc(ym1, y0, y1);  // eq. 16
+          // cell f: slope from (y_f - y_{f-1}, y_{f+1} - y_f)
+          const double dp = yn[v] - yc[v];
+          double l, r;
+          plm_faces(yc[v], slope2_mc(dn[v], dp), l, r);
           pl[v] = rprev[v];
-          pr[v] = y0 - hs;
-          rprev[v] = y0 + hs;
+          pr[v] = l;
+          rprev[v] = r;
+          dn[v] = dp;
+          yc[v] = yn[v];
+          yn[v] = pre[v];
         } else {
-          const double y0 = yv[0], y1 = yv[sd], y2 = yv[2 * sd];
-          const double s1 = slope_mc(y0, y1, y2);
-          const double ehi = ppm_edge(y0, y1, sc[v], s1);
+          const double y2 = pre[v];
+          const double d2 = y2 - yn[v];
+          const double s1 = slope2_mc(dn[v], d2);            // cell f+1
+          const double ehi = ppm_edge(yc[v], yn[v], sc[v], s1);  // edge f+1/2
           double l = elo[v], r = ehi;
-          ppm_mono(y0, l, r);
+          ppm_mono(yc[v], l, r);
           pl[v] = rprev[v];
           pr[v] = l;
           rprev[v] = r;
           sc[v] = s1;
           elo[v] = ehi;
+          dn[v] = d2;
+          yc[v] = yn[v];
+          yn[v] = y2;
         }
+        pre[v] = nxt;
       }
       const Geom G = load_geom(a.Gf, gq);
       double F[8], c;
@@ -158,23 +217,24 @@ struct FluxK {
   static constexpr int FPW = RECON == 0 ? 31 : 29;  // faces per warp
 };
 
+#ifndef CUHARM_FLUXK_MINB
+#define CUHARM_FLUXK_MINB 4
+#endif
+
 template <int RECON, int RIEMANN, bool STAGE>
-__global__ void __launch_bounds__(128) flux_k_kernel(FluxArgs a) {
+__global__ void __launch_bounds__(128, CUHARM_FLUXK_MINB) flux_k_kernel(FluxArgs a) {
   const Dims& d = a.d;
   constexpr int HALO = FluxK<RECON>::HALO, FPW = FluxK<RECON>::FPW;
   const unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31;
-  const int nfaces = a.hi3 - a.lo3 + 1;
-  const int wpr = (nfaces + FPW - 1) / FPW;  // warps per row
-  const int nj = a.hi2 - a.lo2 + 1;
-  const long long nrows = (long long)(a.hi1 - a.lo1 + 1) * nj;
-  const long long gw = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
-  if (gw >= nrows * wpr) return;  // whole warp
-  const int row = (int)(gw / wpr), w = (int)(gw % wpr);
-  const int i = a.lo1 + row / nj, j = a.lo2 + row % nj;
+  // grid: x = warp slot along the row, y = groups of 4 rows j (one per warp of the block), z = i: no divisions
+  const int w = blockIdx.x;
+  const int j = a.lo2 + blockIdx.y * 4 + (threadIdx.x >> 5);
+  const int i = a.lo1 + blockIdx.z;
+  if (j > a.hi2) return;  // whole warp
   const int f0 = a.lo3 + w * FPW;
   const int c = f0 - HALO + lane;  // this lane's cell = the cell whose lower face is face c
-  const int cc = min(max(c, 1), d.n3g - 2);  // clamped for loads; clamped lanes never produce output
+  const int cc = min(max(c, 1), d.n3g - 2);  // clamped for the loads; clamped lanes never produce output
   const long long nz = d.nz;
   const long long rowoff = i * d.s1 + j * d.s2;
   const double* y = a.P + rowoff + cc;
@@ -183,11 +243,10 @@ __global__ void __launch_bounds__(128) flux_k_kernel(FluxArgs a) {
   for (int v = 0; v < 8; v++) {
     const double* yv = y + v * nz;
     const double ym1 = yv[-1], y0 = yv[0], y1 = yv[1];
-    const double s = slope_mc(ym1, y0, y1);
+    const double s = slope2_mc(y0 - ym1, y1 - y0);
     double l, r;
     if (RECON == 0) {
-      l = fma(-0.5, s, y0);
-      r = fma(0.5, s, y0);
+      plm_faces(y0, s, l, r);
     } else {
       const double sup = __shfl_down_sync(FULL, s, 1);   // slope of cell c+1 (lane 31: garbage)
       const double ehi = ppm_edge(y0, y1, s, sup);
@@ -199,9 +258,9 @@ __global__ void __launch_bounds__(128) flux_k_kernel(FluxArgs a) {
     pl[v] = __shfl_up_sync(FULL, r, 1);  // upper-edge state of cell c-1
     pr[v] = l;
   }
-  const bool valid = lane >= HALO && lane < HALO + FPW && c <= a.hi3;
+  const bool ok = lane >= HALO && lane < HALO + FPW && c <= a.hi3;
   double cwv = 0.0;
-  if (valid) {
+  if (ok) {
     const Geom G = load_geom(a.Gf, i * d.n2g + j);
     double F[8];
     face_flux<3, RIEMANN>(pl, pr, G, a.gam, F, cwv);

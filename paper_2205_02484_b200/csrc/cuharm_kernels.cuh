@@ -161,95 +161,237 @@ struct UpdArgs {
   FloorCfg fc;
 };
 
+#ifndef CUHARM_UPD_MINB
+#define CUHARM_UPD_MINB 3
+#endif
+
+// Per-zone work once the streamed operands are in registers.  pb = P^n, pf = the state the fluxes were built from
+// (pf is pb in the predictor), fx[6v..6v+5] = F1[i+1], F1[i], F2[j+1], F2[j], F3[k+1], F3[k] of hydro component v,
+// ex = E1 at (0, +j, +k, +j+k), E2 at (0, +i, +k, +i+k), E3 at (0, +i, +j, +i+j).
 template <bool SAME>
-__global__ void __launch_bounds__(128) update_kernel(UpdArgs a) {
+__device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8], const double pf[8], const double fx[30],
+                                            const double ex[12], long long idx, int q2, bool live, int cnt[5]) {
   const Dims& d = a.d;
-  const int k = d.ng + blockIdx.x * 128 + threadIdx.x;
-  const int j = d.ng + blockIdx.y, i = d.ng + blockIdx.z;
-  int c_rho = 0, c_u = 0, c_ceil = 0, c_cap = 0, c_its = 0;
-  if (k < d.ng + d.n3) {
-    const long long idx = i * d.s1 + j * d.s2 + k;
-    const int q2 = i * d.n2g + j;
-    const Geom G = load_geom(a.C, q2);
-    double pb[8];
+  double dU[8];  // -div F (eq. 25)
 #pragma unroll
-    for (int v = 0; v < 8; v++) pb[v] = a.Pbase[v * d.nz + idx];
-    State S;
-    fluid_state(pb, G, S);
-    double U[8];
-    flux_vector<0>(pb, S, G, a.gam, U);
-    double src[4];
-    if (SAME) {
-      source_term(pb, S, G, a.conn + (size_t)q2 * 40, a.gam, src);
-    } else {
-      double pf[8];
+  for (int v = 0; v < 5; v++)
+    dU[v] = -fma(fx[6 * v] - fx[6 * v + 1], a.idx1,
+                 fma(fx[6 * v + 2] - fx[6 * v + 3], a.idx2, (fx[6 * v + 4] - fx[6 * v + 5]) * a.idx3));
+  // induction: flux-CT replacement fluxes from the edge EMFs (eq. 22; A3)
+  {
+    const double e1_00 = ex[0], e1_j = ex[1], e1_k = ex[2], e1_jk = ex[3];
+    const double e2_00 = ex[4], e2_i = ex[5], e2_k = ex[6], e2_ik = ex[7];
+    const double e3_00 = ex[8], e3_i = ex[9], e3_j = ex[10], e3_ij = ex[11];
+    // F~2(B1) = -1/2 (E3 + E3[i+1]) at faces j, j+1;  F~3(B1) = +1/2 (E2 + E2[i+1]) at faces k, k+1
+    const double divB1 = ((-0.5 * (e3_j + e3_ij)) - (-0.5 * (e3_00 + e3_i))) * a.idx2 +
+                         ((0.5 * (e2_k + e2_ik)) - (0.5 * (e2_00 + e2_i))) * a.idx3;
+    // F~1(B2) = +1/2 (E3 + E3[j+1]) at faces i, i+1;  F~3(B2) = -1/2 (E1 + E1[j+1]) at faces k, k+1
+    const double divB2 = ((0.5 * (e3_i + e3_ij)) - (0.5 * (e3_00 + e3_j))) * a.idx1 +
+                         ((-0.5 * (e1_k + e1_jk)) - (-0.5 * (e1_00 + e1_j))) * a.idx3;
+    // F~1(B3) = -1/2 (E2 + E2[k+1]) at faces i, i+1;  F~2(B3) = +1/2 (E1 + E1[k+1]) at faces j, j+1
+    const double divB3 = ((-0.5 * (e2_i + e2_ik)) - (-0.5 * (e2_00 + e2_k))) * a.idx1 +
+                         ((0.5 * (e1_j + e1_jk)) - (0.5 * (e1_00 + e1_k))) * a.idx2;
+    dU[5] = -divB1;
+    dU[6] = -divB2;
+    dU[7] = -divB3;
+  }
+  // per-(i,j) tables (broadcast loads, L1/L2 resident), U^n, source, update
+  const Geom G = load_geom(a.C, q2);
+  State S;
+  fluid_state(pb, G, S);
+  double U[8];
+  flux_vector<0>(pb, S, G, a.gam, U);
+  double src[4];
+  if (SAME) {
+    source_term(pb, S, G, a.conn + (size_t)q2 * 40, a.gam, src);
+  } else {
+    fluid_state(pf, G, S);
+    source_term(pf, S, G, a.conn + (size_t)q2 * 40, a.gam, src);
+  }
+  U[0] = fma(a.dtau, dU[0], U[0]);
 #pragma unroll
-      for (int v = 0; v < 8; v++) pf[v] = a.Pflux[v * d.nz + idx];
-      fluid_state(pf, G, S);
-      source_term(pf, S, G, a.conn + (size_t)q2 * 40, a.gam, src);
-    }
-    // hydrodynamic components: face-flux differences (eq. 25)
+  for (int v = 1; v < 5; v++) U[v] = fma(a.dtau, src[v - 1] + dU[v], U[v]);
 #pragma unroll
-    for (int v = 0; v < 5; v++) {
-      const double* f1 = a.F1 + v * d.nz + idx;
-      const double* f2 = a.F2 + v * d.nz + idx;
-      const double* f3 = a.F3 + v * d.nz + idx;
-      const double div = (f1[d.s1] - f1[0]) * a.idx1 + (f2[d.s2] - f2[0]) * a.idx2 + (f3[1] - f3[0]) * a.idx3;
-      const double s = (v >= 1) ? src[v - 1] : 0.0;
-      U[v] = U[v] + a.dtau * (s - div);
-    }
-    // induction: flux-CT replacement fluxes from the edge EMFs (eq. 22; A3)
-    {
-      const double* E1 = a.E + idx; const double* E2 = a.E + d.nz + idx; const double* E3 = a.E + 2 * d.nz + idx;
-      const double e1_00 = E1[0], e1_j = E1[d.s2], e1_k = E1[1], e1_jk = E1[d.s2 + 1];
-      const double e2_00 = E2[0], e2_i = E2[d.s1], e2_k = E2[1], e2_ik = E2[d.s1 + 1];
-      const double e3_00 = E3[0], e3_i = E3[d.s1], e3_j = E3[d.s2], e3_ij = E3[d.s1 + d.s2];
-      // F~2(B1) = -1/2 (E3 + E3[i+1]) at faces j, j+1;  F~3(B1) = +1/2 (E2 + E2[i+1]) at faces k, k+1
-      const double divB1 = ((-0.5 * (e3_j + e3_ij)) - (-0.5 * (e3_00 + e3_i))) * a.idx2 +
-                           ((0.5 * (e2_k + e2_ik)) - (0.5 * (e2_00 + e2_i))) * a.idx3;
-      // F~1(B2) = +1/2 (E3 + E3[j+1]) at faces i, i+1;  F~3(B2) = -1/2 (E1 + E1[j+1]) at faces k, k+1
-      const double divB2 = ((0.5 * (e3_i + e3_ij)) - (0.5 * (e3_00 + e3_j))) * a.idx1 +
-                           ((-0.5 * (e1_k + e1_jk)) - (-0.5 * (e1_00 + e1_j))) * a.idx3;
-      // F~1(B3) = -1/2 (E2 + E2[k+1]) at faces i, i+1;  F~2(B3) = +1/2 (E1 + E1[k+1]) at faces j, j+1
-      const double divB3 = ((-0.5 * (e2_i + e2_ik)) - (-0.5 * (e2_00 + e2_k))) * a.idx1 +
-                           ((0.5 * (e1_j + e1_jk)) - (0.5 * (e1_00 + e1_k))) * a.idx2;
-      U[5] = U[5] - a.dtau * divB1;
-      U[6] = U[6] - a.dtau * divB2;
-      U[7] = U[7] - a.dtau * divB3;
-    }
-    double pn[8];
+  for (int v = 5; v < 8; v++) U[v] = fma(a.dtau, dU[v], U[v]);
+  double pn[8];
 #pragma unroll
-    for (int v = 0; v < 8; v++) pn[v] = pb[v];  // A35: the guess is P^n
-    const int flag = invert_2d(U, G, a.gam, pn, a.nc, c_its);
-    if (flag == 0) {
-      const int m = apply_floors(pn, G, a.C + q2, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), a.fc, a.gam, a.nc);
-      c_rho = m & 1; c_u = (m >> 1) & 1; c_ceil = (m >> 2) & 1; c_cap = (m >> 3) & 1;
-    } else {
-      const unsigned long long pos = atomicAdd(a.nfail, 1ull);
-      a.list[pos] = (int)idx;
-    }
+  for (int v = 0; v < 8; v++) pn[v] = pb[v];  // A35: the guess is P^n
+  int its = 0;
+  const int flag = invert_2d(U, G, a.gam, pn, a.nc, its);
+  int m = 0;
+  if (flag == 0) {
+    m = apply_floors(pn, G, a.C + q2, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), a.fc, a.gam, a.nc);
+  } else if (live) {
+    const unsigned long long pos = atomicAdd(a.nfail, 1ull);
+    a.list[pos] = (int)idx;
+  }
+  if (live) {
     a.flag[idx] = flag;
 #pragma unroll
     for (int v = 0; v < 8; v++) a.Pout[v * d.nz + idx] = pn[v];
+    cnt[0] = m & 1; cnt[1] = (m >> 1) & 1; cnt[2] = (m >> 2) & 1; cnt[3] = (m >> 3) & 1; cnt[4] = its;
   }
-  // statistics: warp sums, one atomic per warp and counter, zeros skipped
-  c_rho = __reduce_add_sync(0xffffffffu, c_rho);
-  c_u = __reduce_add_sync(0xffffffffu, c_u);
-  c_ceil = __reduce_add_sync(0xffffffffu, c_ceil);
-  c_cap = __reduce_add_sync(0xffffffffu, c_cap);
-  c_its = __reduce_add_sync(0xffffffffu, c_its);
+}
+
+// statistics: warp sums, one shared-memory atomic per warp and counter, one global atomic per block and counter
+__device__ __forceinline__ void update_stats(const UpdArgs& a, const int cnt[5]) {
   __shared__ int sh[5];
   if (threadIdx.x < 5) sh[threadIdx.x] = 0;
   __syncthreads();
-  if ((threadIdx.x & 31) == 0) {
-    if (c_rho) atomicAdd(&sh[0], c_rho);
-    if (c_u) atomicAdd(&sh[1], c_u);
-    if (c_ceil) atomicAdd(&sh[2], c_ceil);
-    if (c_cap) atomicAdd(&sh[3], c_cap);
-    if (c_its) atomicAdd(&sh[4], c_its);
+#pragma unroll
+  for (int c = 0; c < 5; c++) {
+    const int s = __reduce_add_sync(0xffffffffu, cnt[c]);
+    if ((threadIdx.x & 31) == 0 && s) atomicAdd(&sh[c], s);
   }
   __syncthreads();
   if (threadIdx.x < 5 && sh[threadIdx.x]) atomicAdd(a.stats + 2 + threadIdx.x, (unsigned long long)sh[threadIdx.x]);
+}
+
+// Generic kernel: per-thread loads (any n3, any alignment).  One thread per interior zone; out-of-range lanes of the
+// ragged tail work on a clamped copy of the last zone and store nothing.
+template <bool SAME>
+__global__ void __launch_bounds__(128, CUHARM_UPD_MINB) update_kernel(UpdArgs a) {
+  const Dims& d = a.d;
+  const int k = d.ng + blockIdx.x * 128 + threadIdx.x;
+  const int j = d.ng + blockIdx.y, i = d.ng + blockIdx.z;
+  const bool live = k < d.ng + d.n3;
+  const int kc = live ? k : d.ng + d.n3 - 1;
+  const long long idx = i * d.s1 + j * d.s2 + kc;
+  const int q2 = i * d.n2g + j;
+  double pb[8], pf[8], fx[30], ex[12];
+#pragma unroll
+  for (int v = 0; v < 8; v++) pb[v] = a.Pbase[v * d.nz + idx];
+#pragma unroll
+  for (int v = 0; v < 8; v++) pf[v] = SAME ? pb[v] : a.Pflux[v * d.nz + idx];
+#pragma unroll
+  for (int v = 0; v < 5; v++) {
+    const double* f1 = a.F1 + v * d.nz + idx;
+    const double* f2 = a.F2 + v * d.nz + idx;
+    const double* f3 = a.F3 + v * d.nz + idx;
+    fx[6 * v + 0] = __ldg(f1 + d.s1); fx[6 * v + 1] = __ldg(f1);
+    fx[6 * v + 2] = __ldg(f2 + d.s2); fx[6 * v + 3] = __ldg(f2);
+    fx[6 * v + 4] = __ldg(f3 + 1);    fx[6 * v + 5] = __ldg(f3);
+  }
+  {
+    const double* E1 = a.E + idx; const double* E2 = a.E + d.nz + idx; const double* E3 = a.E + 2 * d.nz + idx;
+    ex[0] = __ldg(E1); ex[1] = __ldg(E1 + d.s2); ex[2] = __ldg(E1 + 1); ex[3] = __ldg(E1 + d.s2 + 1);
+    ex[4] = __ldg(E2); ex[5] = __ldg(E2 + d.s1); ex[6] = __ldg(E2 + 1); ex[7] = __ldg(E2 + d.s1 + 1);
+    ex[8] = __ldg(E3); ex[9] = __ldg(E3 + d.s1); ex[10] = __ldg(E3 + d.s2); ex[11] = __ldg(E3 + d.s1 + d.s2);
+  }
+  int cnt[5] = {0, 0, 0, 0, 0};
+  update_zone<SAME>(a, pb, pf, fx, ex, idx, q2, live, cnt);
+  update_stats(a, cnt);
+}
+
+// TMA kernel (n3g even, 16-byte aligned arrays).  The streamed operands of the 128 zones of a block are 49 row
+// segments (41 in the predictor) of UPD_ROW doubles each, contiguous along k: lanes of warp 0 issue one 1D bulk copy
+// (cp.async.bulk, global -> shared, completion on an mbarrier) per row, so the whole DRAM footprint of the block
+// is in flight at once, holds no registers while it flies, and costs no per-thread address arithmetic.  Every
+// thread then reads its zone (and the k+1 neighbour) from shared memory.  Segment = zones k0-1 .. k0+UPD_ROW-2 of
+// the row (k0 = first zone of the block; the -1 makes the start even, i.e. 16-byte aligned, because ng is odd).
+constexpr int UPD_ROW = 132;   // doubles per staged row: 1 + 128 + 1 (k+1) + 2 pad -> 1056 B, a multiple of 16
+constexpr int UPD_NROW = 49;   // 8 P^n, 8 P-flux, 10 F1, 10 F2, 5 F3, 2 E1, 2 E2, 4 E3
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+// issue the bulk copies of one tile (rows of zones kb.. of row (i,j)) into one stage; called by threads 0..63
+template <bool SAME>
+__device__ __forceinline__ void upd_issue_tile(const UpdArgs& a, int tile, int nch, double* stage, unsigned bar) {
+  const Dims& d = a.d;
+  const int c = tile % nch, ij = tile / nch;
+  const int j = d.ng + ij % d.n2, i = d.ng + ij / d.n2;
+  const int kb = d.ng + c * 128 - 1;                      // first staged zone of the row (even)
+  const unsigned bytes = (unsigned)min(UPD_ROW - 2, d.n3g - kb) * 8u;  // staged zones per row: even count
+  const long long base = i * d.s1 + j * d.s2 + kb;       // element offset of the segment in every array
+  const int t = threadIdx.x;
+  if (t == 0) {
+    const unsigned total = bytes * (SAME ? UPD_NROW - 8 : UPD_NROW);
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(total) : "memory");
+  }
+  for (int r = t; r < UPD_NROW; r += 64) {
+    const double* src;
+    if (r < 8) src = a.Pbase + r * d.nz;
+    else if (r < 16) { if (SAME) continue; src = a.Pflux + (r - 8) * d.nz; }
+    else if (r < 26) src = a.F1 + ((r - 16) >> 1) * d.nz + (((r - 16) & 1) ? 0 : d.s1);
+    else if (r < 36) src = a.F2 + ((r - 26) >> 1) * d.nz + (((r - 26) & 1) ? 0 : d.s2);
+    else if (r < 41) src = a.F3 + (r - 36) * d.nz;
+    else if (r < 43) src = a.E + (r - 41) * d.s2;
+    else if (r < 45) src = a.E + d.nz + (r - 43) * d.s1;
+    else src = a.E + 2 * d.nz + ((r - 45) & 1) * d.s1 + ((r - 45) >> 1) * d.s2;
+    src += base;
+    const unsigned dst = smem_u32(stage + r * UPD_ROW);
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+  }
+}
+
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  unsigned done = 0;
+  while (!done) {
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(done)
+                 : "r"(bar), "r"(parity)
+                 : "memory");
+  }
+}
+
+// Persistent blocks: block b takes tiles b, b + gridDim.x, ...; tile = (i, j, 128-zone chunk of the row), chunk
+// fastest.  One stage per block: the stage is free again as soon as every thread has moved its operands to
+// registers, which is the first thing a tile does, so the copies of tile n+1 fly during the whole of tile n's
+// arithmetic; CUHARM_UPD_TMA_MINB blocks per SM keep that many tiles in flight and enough warps for the
+// (serial) Newton iteration.
+#ifndef CUHARM_UPD_TMA_MINB
+#define CUHARM_UPD_TMA_MINB 3
+#endif
+template <bool SAME>
+__global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(UpdArgs a, int ntiles, int nch) {
+  extern __shared__ __align__(128) double rows[];  // [UPD_NROW][UPD_ROW]
+  __shared__ __align__(8) unsigned long long mbar;
+  const Dims& d = a.d;
+  const int t = threadIdx.x;
+  const int G = gridDim.x;
+  const unsigned bar0 = smem_u32(&mbar);
+  if (t == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar0));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  int tile = blockIdx.x;
+  if (t < 64 && tile < ntiles) upd_issue_tile<SAME>(a, tile, nch, rows, bar0);
+  int cnt_acc[5] = {0, 0, 0, 0, 0};
+  for (int n = 0; tile < ntiles; tile += G, n++) {
+    const int c = tile % nch, ij = tile / nch;
+    const int j = d.ng + ij % d.n2, i = d.ng + ij / d.n2;
+    const int k0 = d.ng + c * 128;
+    const bool live = k0 + t < d.ng + d.n3;
+    const int tc = live ? t : d.ng + d.n3 - 1 - k0;  // clamped lane position
+    const long long idx = i * d.s1 + j * d.s2 + k0 + tc;
+    const int q2 = i * d.n2g + j;
+    mbar_wait(bar0, n & 1);
+    const double* z = rows + 1 + tc;  // this zone in row 0 of the stage
+    double pb[8], pf[8], fx[30], ex[12];
+#pragma unroll
+    for (int v = 0; v < 8; v++) pb[v] = z[v * UPD_ROW];
+#pragma unroll
+    for (int v = 0; v < 8; v++) pf[v] = SAME ? pb[v] : z[(8 + v) * UPD_ROW];
+#pragma unroll
+    for (int v = 0; v < 5; v++) {
+      fx[6 * v + 0] = z[(16 + 2 * v) * UPD_ROW]; fx[6 * v + 1] = z[(17 + 2 * v) * UPD_ROW];
+      fx[6 * v + 2] = z[(26 + 2 * v) * UPD_ROW]; fx[6 * v + 3] = z[(27 + 2 * v) * UPD_ROW];
+      fx[6 * v + 4] = z[(36 + v) * UPD_ROW + 1]; fx[6 * v + 5] = z[(36 + v) * UPD_ROW];
+    }
+    ex[0] = z[41 * UPD_ROW]; ex[1] = z[42 * UPD_ROW]; ex[2] = z[41 * UPD_ROW + 1]; ex[3] = z[42 * UPD_ROW + 1];
+    ex[4] = z[43 * UPD_ROW]; ex[5] = z[44 * UPD_ROW]; ex[6] = z[43 * UPD_ROW + 1]; ex[7] = z[44 * UPD_ROW + 1];
+    ex[8] = z[45 * UPD_ROW]; ex[9] = z[46 * UPD_ROW]; ex[10] = z[47 * UPD_ROW]; ex[11] = z[48 * UPD_ROW];
+    __syncthreads();  // every thread holds its operands: the stage can be refilled
+    if (t < 64 && tile + G < ntiles) upd_issue_tile<SAME>(a, tile + G, nch, rows, bar0);
+    int cnt[5] = {0, 0, 0, 0, 0};
+    update_zone<SAME>(a, pb, pf, fx, ex, idx, q2, live, cnt);
+#pragma unroll
+    for (int q = 0; q < 5; q++) cnt_acc[q] += cnt[q];
+  }
+  update_stats(a, cnt_acc);
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -87,24 +87,30 @@ __device__ __forceinline__ void lower(const Geom& G, double v0, double v1, doubl
 }
 
 __device__ __forceinline__ void fluid_state(const double q[8], const Geom& G, State& S) {
-  const double x = 1.0 + gamma_sq_minus_one(q, G);
+  // covariant spatial components: u_i = g_ij utilde^j exactly, because g_ij beta^j = g_ti (the shift lowered by the
+  // spatial metric) cancels the u^t term of u_i = g_it u^t + g_ij u^j; likewise u_t = -alpha Gamma + beta^i u_i with
+  // beta^1 = alpha (alpha g^{t1}) the only non-zero shift component in Kerr-Schild coordinates.
+  S.l1 = fma(G.g11, q[2], G.g13 * q[4]);
+  S.l2 = G.g22 * q[3];
+  S.l3 = fma(G.g13, q[2], G.g33 * q[4]);
+  const double x = 1.0 + fma(S.l1, q[2], fma(S.l2, q[3], S.l3 * q[4]));  // Gamma^2 = 1 + g_ij ut^i ut^j
   const double ilor = frsqrt(x);
   const double lor = x * ilor;  // Gamma = sqrt(1 + q^2)
   S.lor = lor;
   S.u0 = lor * G.ialpha;
-  // beta^i / alpha = -alpha g^{ti};  u^i = ut^i - Gamma beta^i / alpha  (eq. 10);  g^{t2} = g^{t3} = 0
+  // beta^i / alpha = alpha g^{ti};  u^i = ut^i - Gamma beta^i / alpha  (eq. 10);  g^{t2} = g^{t3} = 0
   S.u1 = fma(-lor, G.ac01, q[2]);
   S.u2 = q[3];
   S.u3 = q[4];
-  lower(G, S.u0, S.u1, S.u2, S.u3, S.l0, S.l1, S.l2, S.l3);
-  const double bt = q[5] * S.l1 + q[6] * S.l2 + q[7] * S.l3;  // b^t = B^i u_i
+  S.l0 = G.alpha * fma(G.ac01, S.l1, -lor);
+  const double bt = fma(q[5], S.l1, fma(q[6], S.l2, q[7] * S.l3));  // b^t = B^i u_i
   const double iu0 = G.alpha * ilor;
   S.b0 = bt;
   S.b1 = fma(bt, S.u1, q[5]) * iu0;  // b^i = (B^i + b^t u^i) / u^t
   S.b2 = fma(bt, S.u2, q[6]) * iu0;
   S.b3 = fma(bt, S.u3, q[7]) * iu0;
   lower(G, S.b0, S.b1, S.b2, S.b3, S.m0, S.m1, S.m2, S.m3);
-  S.bsq = S.b0 * S.m0 + S.b1 * S.m1 + S.b2 * S.m2 + S.b3 * S.m3;
+  S.bsq = fma(S.b0, S.m0, fma(S.b1, S.m1, fma(S.b2, S.m2, S.b3 * S.m3)));
 }
 
 __device__ __forceinline__ double pick(int d, double a0, double a1, double a2, double a3) {
@@ -162,17 +168,18 @@ __device__ __forceinline__ void flux_vector(const double q[8], const State& S, c
 template <int DIR>
 __device__ __forceinline__ void wave_speeds(const double q[8], const State& S, const Geom& G, double gam, double& cp,
                                             double& cm) {
+  // c_ms^2 = N / D with N = b^2 + gam p, D = b^2 + w (eqs. 18-19).  The quadratic is homogeneous in its
+  // coefficients, so it is scaled by D > 0 and c_ms^2 is never formed: A = (D - N) (u^t)^2 - N g^tt, ...
   const double pg = (gam - 1.0) * q[1];
   const double w = q[0] + q[1] + pg;
-  const double cms2 = fma(gam, pg, S.bsq) * frcp(S.bsq + w);  // eqs. 18-19
+  const double N = fma(gam, pg, S.bsq);
+  const double DmN = (S.bsq + w) - N;
   const double ut = S.u0;
   const double ud = pick(DIR, S.u0, S.u1, S.u2, S.u3);
-  const double gtd = DIR == 1 ? G.c01 : 0.0;
   const double gdd = DIR == 1 ? G.c11 : (DIR == 2 ? G.c22 : G.c33);
-  const double utt = ut * ut, utd = ut * ud, udd = ud * ud;
-  const double A = fma(-cms2, G.c00 + utt, utt);
-  const double hB = fma(-cms2, gtd + utd, utd);  // = -B/2
-  const double C = fma(-cms2, gdd + udd, udd);
+  const double A = fma(DmN * ut, ut, -N * G.c00);
+  const double hB = DIR == 1 ? fma(DmN * ut, ud, -N * G.c01) : (DmN * ut) * ud;  // = -B/2; g^{t2} = g^{t3} = 0
+  const double C = fma(DmN * ud, ud, -N * gdd);
   double disc = fma(hB, hB, -A * C);             // (B^2 - 4AC)/4
   disc = disc > 1e-300 ? disc : 1e-300;
   const double sq = disc * frsqrt(disc);
@@ -182,33 +189,51 @@ __device__ __forceinline__ void wave_speeds(const double q[8], const State& S, c
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Reconstruction.  MC-limited slope, eq. 15 (A2: the last branch is signed): for dm, dp of one sign the
-// one of {2 dm, 2 dp, (dm+dp)/2} of smallest magnitude, else 0.
+// Reconstruction.  The fp64 pipe and the issue slots bound the flux kernels, so the limiter
+// is written for the fewest fp64 instructions; every form below equals the paper's in exact arithmetic and
+// differs from the literal transcription by rounding only.
+//
+// MC-limited slope, eq. 15 (A2: the last branch is signed), from the two one-sided differences
+// dm = q_I - q_{I-1}, dp = q_{I+1} - q_I.  Returned DOUBLED: 2 dq = minmod(4 dm, 4 dp, dm + dp)  (scaling by a
+// power of two is exact).  "dm dp < 0" is read off the sign bits; when one of them is zero the minmod is zero anyway.
 // ---------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double slope_mc(double qm, double q0, double qp) {
-  const double dm = q0 - qm, dp = qp - q0;
-  const double dc = 0.5 * (qp - qm);
-  const double one = fabs(dm) < fabs(dp) ? dm : dp;  // the smaller one-sided difference
-  const double two = one + one;
-  const double s = fabs(two) < fabs(dc) ? two : dc;
-  return (dm * dp < 0.0) ? 0.0 : s;
+__device__ __forceinline__ double same_sign_factor(double a, double b, int hi_one) {
+  // the double whose high word is hi_one (low word 0) if a and b carry the same sign bit, else +0.0
+  const int x = __double2hiint(a) ^ __double2hiint(b);
+  return __hiloint2double(~(x >> 31) & hi_one, 0);
 }
 
-// PPM (A20): 4th-order edge value between cells 0 and 1 from their values and MC slopes ...
-__device__ __forceinline__ double ppm_edge(double y0, double y1, double s0, double s1) {
-  return fma(-1.0 / 6.0, s1 - s0, 0.5 * (y0 + y1));
+__device__ __forceinline__ double slope2_mc(double dm, double dp) {
+  const double sum = dm + dp;
+  const double one = fabs(dm) < fabs(dp) ? dm : dp;              // the smaller one-sided difference
+  const double four = one * same_sign_factor(dm, dp, 0x40100000);  // 4 one, or 0 at an extremum
+  return fabs(four) < fabs(sum) ? four : sum;
+}
+
+// PLM face values of a cell from its doubled slope (eq. 16): q -+ dq/2
+__device__ __forceinline__ void plm_faces(double y, double s2, double& l, double& r) {
+  l = fma(-0.25, s2, y);
+  r = fma(0.25, s2, y);
+}
+
+// PPM (A20): 4th-order edge value between cells 0 and 1 from their values and DOUBLED MC slopes:
+// (y0 + y1)/2 - (dq1 - dq0)/6 ...
+__device__ __forceinline__ double ppm_edge(double y0, double y1, double s20, double s21) {
+  return fma(-1.0 / 12.0, s21 - s20, 0.5 * (y0 + y1));
 }
 
 // ... and the monotonisation of the parabola of a cell with value y and edge values l (lower), r (upper).
+// With a = r - y, b = y - l the three cases of Colella-Woodward eq. 1.10 are: a b <= 0 -> l = r = y;
+// |b| > 2|a| -> l = 3y - 2r = y - 2a;  |a| > 2|b| -> r = 3y - 2l = y + 2b.  Hence l = y - min(|b|, 2|a|) sgn(b),
+// r = y + min(|a|, 2|b|) sgn(a) for a b > 0 (a zero a or b gives l = r = y through the min), else l = r = y.
 __device__ __forceinline__ void ppm_mono(double y, double& l, double& r) {
-  const double d = r - l;
-  const double m6 = d * (y - 0.5 * (l + r));
-  const double lim = d * d * (1.0 / 6.0);
-  const double l2 = fma(-2.0, r, 3.0 * y), r2 = fma(-2.0, l, 3.0 * y);
-  const bool flat = (r - y) * (y - l) <= 0.0;
-  const bool lo = m6 > lim, hi = m6 < -lim;
-  l = flat ? y : (lo ? l2 : l);
-  r = flat ? y : ((!lo && hi) ? r2 : r);
+  const double a = r - y, b = y - l;
+  const double a2 = a + a, b2 = b + b;
+  const double bp = fabs(b) < fabs(a2) ? b : a2;
+  const double ap = fabs(a) < fabs(b2) ? a : b2;
+  const double f = same_sign_factor(a, b, 0x3ff00000);  // 1 or 0
+  l = fma(-f, bp, y);
+  r = fma(f, ap, y);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -216,31 +241,63 @@ __device__ __forceinline__ void ppm_mono(double y, double& l, double& r) {
 // RIEMANN 0: local Lax-Friedrichs, eq. 17.  RIEMANN 1: HLL, eq. 20 (A30: guarded denominator).
 // sqrt(-g) multiplies the combination once (it is common to U^l, U^r, F^l, F^r at a face).
 // ---------------------------------------------------------------------------------------------------------
+// One side's contribution F^d + c U (both divided by sqrt(-g)) formed in one go: with uh = u^d + c u^t and
+// bh = b^d + c b^t,  [0] rho uh;  [1..4] (w + b^2) uh u_nu + (p + b^2/2)(delta^d_nu + c delta^t_nu) - bh b_nu;
+// [5..7] b^i uh - bh u^i  (= c B^d for i = d).  Algebraically the same as flux_hat<DIR> + c flux_hat<0>.
+template <int DIR>
+__device__ __forceinline__ void side_flux(const double q[8], const State& S, double gam, double c, double out[8]) {
+  const double pg = (gam - 1.0) * q[1];
+  const double w = q[0] + q[1] + pg;
+  const double ptot = fma(0.5, S.bsq, pg);
+  const double ud = pick(DIR, S.u0, S.u1, S.u2, S.u3);
+  const double bd = pick(DIR, S.b0, S.b1, S.b2, S.b3);
+  const double uh = fma(c, S.u0, ud), bh = fma(c, S.b0, bd);
+  const double e = (w + S.bsq) * uh;
+  out[0] = q[0] * uh;
+  double t0 = fma(c, ptot, fma(e, S.l0, -bh * S.m0));
+  double t1 = fma(e, S.l1, -bh * S.m1);
+  double t2 = fma(e, S.l2, -bh * S.m2);
+  double t3 = fma(e, S.l3, -bh * S.m3);
+  if (DIR == 1) t1 += ptot;
+  if (DIR == 2) t2 += ptot;
+  if (DIR == 3) t3 += ptot;
+  out[1] = t0;
+  out[2] = t1;
+  out[3] = t2;
+  out[4] = t3;
+  out[5] = DIR == 1 ? c * q[5] : fma(S.b1, uh, -bh * S.u1);
+  out[6] = DIR == 2 ? c * q[6] : fma(S.b2, uh, -bh * S.u2);
+  out[7] = DIR == 3 ? c * q[7] : fma(S.b3, uh, -bh * S.u3);
+}
+
 template <int DIR, int RIEMANN>
 __device__ __forceinline__ void face_flux(const double pl[8], const double pr[8], const Geom& G, double gam, double F[8],
                                           double& cw) {
   State Sl, Sr;
-  double Ul[8], Fl[8], Ur[8], Fr[8], cpl, cml, cpr, cmr;
+  double Hl[8], Hr[8], cpl, cml, cpr, cmr;
   fluid_state(pl, G, Sl);
   fluid_state(pr, G, Sr);
-  flux_hat<0>(pl, Sl, gam, Ul);
-  flux_hat<0>(pr, Sr, gam, Ur);
-  flux_hat<DIR>(pl, Sl, gam, Fl);
-  flux_hat<DIR>(pr, Sr, gam, Fr);
   wave_speeds<DIR>(pl, Sl, G, gam, cpl, cml);
   wave_speeds<DIR>(pr, Sr, G, gam, cpr, cmr);
   const double cmax = fmax(0.0, fmax(cpr, cpl));
   const double cmin = fmax(0.0, fmax(-cmr, -cml));
   cw = fmax(cmax, cmin);
   if (RIEMANN == 0) {
+    // eq. 17: (F^l + F^r - c_w (U^r - U^l))/2 = ((F^l + c_w U^l) + (F^r - c_w U^r))/2
+    side_flux<DIR>(pl, Sl, gam, cw, Hl);
+    side_flux<DIR>(pr, Sr, gam, -cw, Hr);
     const double hsg = 0.5 * G.sg;
 #pragma unroll
-    for (int v = 0; v < 8; v++) F[v] = hsg * fma(-cw, Ur[v] - Ul[v], Fl[v] + Fr[v]);
+    for (int v = 0; v < 8; v++) F[v] = hsg * (Hl[v] + Hr[v]);
   } else {
+    // eq. 20: (c_max F^l + c_min F^r - c_max c_min (U^r - U^l)) / (c_max + c_min)
+    //       = (c_max (F^l + c_min U^l) + c_min (F^r - c_max U^r)) / (c_max + c_min)
+    side_flux<DIR>(pl, Sl, gam, cmin, Hl);
+    side_flux<DIR>(pr, Sr, gam, -cmax, Hr);
     const double sc = G.sg * frcp(fmax(cmax + cmin, 1e-300));
-    const double cc = cmax * cmin;
+    const double wl = sc * cmax, wr = sc * cmin;
 #pragma unroll
-    for (int v = 0; v < 8; v++) F[v] = sc * fma(-cc, Ur[v] - Ul[v], fma(cmax, Fl[v], cmin * Fr[v]));
+    for (int v = 0; v < 8; v++) F[v] = fma(wl, Hl[v], wr * Hr[v]);
   }
 }
 
