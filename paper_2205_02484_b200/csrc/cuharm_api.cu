@@ -61,6 +61,7 @@ struct cuharm_ctx {
   // graph
   bool upd_tma = false;  // update_tma_kernel usable (shared-memory opt-in succeeded)
   int upd_blocks = 0;    // its persistent grid size
+  int fluxk_blocks = 0;  // persistent grid size of flux_k_tma_kernel (0: not usable)
   bool use_graph = false;
   cudaGraphExec_t gexec = nullptr;
   cudaStream_t cap_stream = nullptr;
@@ -158,8 +159,17 @@ void launch_flux_t(cuharm_ctx* h, FluxArgs& a, int dir) {
   const int ni = a.hi1 - a.lo1 + 1, nj = a.hi2 - a.lo2 + 1, nk = a.hi3 - a.lo3 + 1;
   if (dir == 3) {
     const int fpw = FluxK<RECON>::FPW;
-    const dim3 grid((unsigned)((nk + fpw - 1) / fpw), (unsigned)((nj + 3) / 4), (unsigned)ni);
-    flux_k_kernel<RECON, RIEMANN, STAGE><<<grid, 128, 0, h->stream>>>(a);
+    const int wpr = (nk + fpw - 1) / fpw;
+    const Dims& d = a.d;
+    const bool tma = h->fluxk_blocks > 0 && (d.n3g % 2 == 0) && ((uintptr_t)a.P % 16 == 0);
+    if (tma) {
+      const long long items = (long long)ni * nj * wpr;
+      const int nb = (int)std::min<long long>((items + 3) / 4, h->fluxk_blocks);
+      flux_k_tma_kernel<RECON, RIEMANN, STAGE><<<nb, 128, 0, h->stream>>>(a, wpr);
+    } else {
+      const dim3 grid((unsigned)wpr, (unsigned)((nj + 3) / 4), (unsigned)ni);
+      flux_k_kernel<RECON, RIEMANN, STAGE><<<grid, 128, 0, h->stream>>>(a);
+    }
   } else {
     const long long cols = (long long)(dir == 1 ? nj : ni) * nk;
     const int nf = dir == 1 ? ni : nj;
@@ -318,8 +328,18 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
       h->upd_blocks = sms * per;
     }
     if (!h->upd_tma) cudaGetLastError();
+    {
+      int dev = 0, sms = 0, per = 0;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, flux_k_tma_kernel<1, 0, false>, 128, 0) == cudaSuccess && per > 0)
+        h->fluxk_blocks = sms * per;
+      else
+        cudaGetLastError();
+    }
 #ifdef CUHARM_NO_TMA
     h->upd_tma = false;
+    h->fluxk_blocks = 0;
 #endif
   }
   *out = h;

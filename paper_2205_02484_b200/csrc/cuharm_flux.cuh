@@ -42,6 +42,33 @@ __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* addr, doub
   if ((threadIdx.x & 31) == 0 && m > *reinterpret_cast<volatile unsigned long long*>(addr)) atomicMax(addr, m);
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Asynchronous 1D bulk copies global -> shared (the TMA engine's cp.async.bulk) completing on an mbarrier.
+// Source, destination and size must be multiples of 16 bytes.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  unsigned done = 0;
+  while (!done) {
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(done)
+                 : "r"(bar), "r"(parity)
+                 : "memory");
+  }
+}
+
 struct FluxArgs {
   Dims d;
   const double* P;
@@ -267,6 +294,115 @@ __global__ void __launch_bounds__(128, CUHARM_FLUXK_MINB) flux_k_kernel(FluxArgs
     store_flux<3, STAGE>(a, rowoff + c, F, cwv);
   }
   atomic_max_nonneg(a.cwmax, cwv);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Direction 3, bulk-copy version (n3g even, 16-byte aligned P): persistent warps, each with its own one-stage
+// pipeline.  Work item = (i, j, w) as above, w fastest; warp g takes items g, g + W, ...  The 34 cells x 8 variables
+// an item reads arrive as 8 bulk copies of KSEG doubles into the warp's stage; the stage is free again once the
+// lanes have moved their three cells per variable to registers, so the copies of the next item fly during the
+// whole of this item's arithmetic and no lane ever waits on DRAM with a scoreboard.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int KSEG = 36;  // doubles per staged row segment: 34 cells rounded up to an even start and count
+
+struct ItemIdx { int i, j, w; };
+
+#ifndef CUHARM_FLUXK_TMA_MINB
+#define CUHARM_FLUXK_TMA_MINB 4
+#endif
+
+template <int RECON, int RIEMANN, bool STAGE>
+__global__ void __launch_bounds__(128, CUHARM_FLUXK_TMA_MINB) flux_k_tma_kernel(FluxArgs a, int wpr) {
+  __shared__ __align__(128) double stage_all[4][8][KSEG];
+  __shared__ __align__(8) unsigned long long mbar_all[4];
+  const Dims& d = a.d;
+  constexpr int HALO = FluxK<RECON>::HALO, FPW = FluxK<RECON>::FPW;
+  const unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  double (*stage)[KSEG] = stage_all[wib];
+  const unsigned bar = smem_u32(&mbar_all[wib]);
+  const int ni = a.hi1 - a.lo1 + 1, nj = a.hi2 - a.lo2 + 1;
+  const long long nitems = (long long)ni * nj * wpr;
+  const long long W = (long long)gridDim.x * 4;
+  long long item = (long long)blockIdx.x * 4 + wib;
+  // decomposition of the first item and of the stride, then carried increments (no division in the loop)
+  ItemIdx cur, nxt, dlt;
+  {
+    long long r = item / wpr;
+    cur.w = (int)(item % wpr); cur.j = (int)(r % nj); cur.i = (int)(r / nj);
+    r = W / wpr;
+    dlt.w = (int)(W % wpr); dlt.j = (int)(r % nj); dlt.i = (int)(r / nj);
+  }
+  auto advance = [&](const ItemIdx& x) {
+    ItemIdx y{x.i + dlt.i, x.j + dlt.j, x.w + dlt.w};
+    if (y.w >= wpr) { y.w -= wpr; y.j++; }
+    if (y.j >= nj) { y.j -= nj; y.i++; }
+    return y;
+  };
+  // segment start (even, clamped) of an item's chunk
+  auto seg_start = [&](int w) {
+    int cs = a.lo3 + w * FPW - HALO - 1;
+    cs = cs < 0 ? 0 : cs & ~1;
+    return cs;
+  };
+  // lanes 0..7, one variable each: a single thread needs several hundred cycles per bulk copy it issues, eight
+  // lanes issue theirs concurrently
+  auto issue = [&](const ItemIdx& x) {
+    const int cs = seg_start(x.w);
+    const unsigned bytes = (unsigned)min(KSEG, d.n3g - cs) * 8u;
+    const double* src = a.P + (a.lo1 + x.i) * d.s1 + (a.lo2 + x.j) * d.s2 + cs + lane * d.nz;
+    if (lane == 0) mbar_expect_tx(bar, 8u * bytes);
+    __syncwarp(0xffu);
+    bulk_g2s(smem_u32(&stage[lane][0]), src, bytes, bar);
+  };
+  if (lane == 0) {
+    mbar_init(bar, 1);
+    mbar_fence_init();
+  }
+  __syncwarp();
+  if (lane < 8 && item < nitems) issue(cur);
+  double cwmax = 0.0;
+  for (unsigned n = 0; item < nitems; item += W, n++, cur = nxt) {
+    nxt = advance(cur);
+    const int i = a.lo1 + cur.i, j = a.lo2 + cur.j;
+    const int f0 = a.lo3 + cur.w * FPW;
+    const int c = f0 - HALO + lane;            // this lane's cell = the cell whose lower face is face c
+    const int cc = min(max(c, 1), d.n3g - 2);  // clamped for the reads; clamped lanes never produce output
+    const int o = cc - seg_start(cur.w);
+    mbar_wait(bar, n & 1);
+    double ym1[8], y0[8], y1[8];
+#pragma unroll
+    for (int v = 0; v < 8; v++) { ym1[v] = stage[v][o - 1]; y0[v] = stage[v][o]; y1[v] = stage[v][o + 1]; }
+    __syncwarp();  // all lanes hold their cells: the stage can be refilled
+    if (lane < 8 && item + W < nitems) issue(nxt);
+    double pl[8], pr[8];
+#pragma unroll
+    for (int v = 0; v < 8; v++) {
+      const double s = slope2_mc(y0[v] - ym1[v], y1[v] - y0[v]);
+      double l, r;
+      if (RECON == 0) {
+        plm_faces(y0[v], s, l, r);
+      } else {
+        const double sup = __shfl_down_sync(FULL, s, 1);   // slope of cell c+1 (lane 31: garbage)
+        const double ehi = ppm_edge(y0[v], y1[v], s, sup);
+        const double elo = __shfl_up_sync(FULL, ehi, 1);   // edge value c-1/2 (lane 0: garbage)
+        l = elo;
+        r = ehi;
+        ppm_mono(y0[v], l, r);
+      }
+      pl[v] = __shfl_up_sync(FULL, r, 1);  // upper-edge state of cell c-1
+      pr[v] = l;
+    }
+    const bool ok = lane >= HALO && lane < HALO + FPW && c <= a.hi3;
+    if (ok) {
+      const Geom G = load_geom(a.Gf, i * d.n2g + j);
+      double F[8], cwv;
+      face_flux<3, RIEMANN>(pl, pr, G, a.gam, F, cwv);
+      store_flux<3, STAGE>(a, i * d.s1 + j * d.s2 + c, F, cwv);
+      cwmax = fmax(cwmax, cwv);
+    }
+  }
+  atomic_max_nonneg(a.cwmax, cwmax);
 }
 
 }  // namespace cuharm

@@ -292,8 +292,6 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_MINB) update_kernel(UpdArgs a)
 constexpr int UPD_ROW = 132;   // doubles per staged row: 1 + 128 + 1 (k+1) + 2 pad -> 1056 B, a multiple of 16
 constexpr int UPD_NROW = 49;   // 8 P^n, 8 P-flux, 10 F1, 10 F2, 5 F3, 2 E1, 2 E2, 4 E3
 
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-
 // issue the bulk copies of one tile (rows of zones kb.. of row (i,j)) into one stage; called by threads 0..63
 template <bool SAME>
 __device__ __forceinline__ void upd_issue_tile(const UpdArgs& a, int tile, int nch, double* stage, unsigned bar) {
@@ -306,7 +304,7 @@ __device__ __forceinline__ void upd_issue_tile(const UpdArgs& a, int tile, int n
   const int t = threadIdx.x;
   if (t == 0) {
     const unsigned total = bytes * (SAME ? UPD_NROW - 8 : UPD_NROW);
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(total) : "memory");
+    mbar_expect_tx(bar, total);
   }
   for (int r = t; r < UPD_NROW; r += 64) {
     const double* src;
@@ -320,19 +318,7 @@ __device__ __forceinline__ void upd_issue_tile(const UpdArgs& a, int tile, int n
     else src = a.E + 2 * d.nz + ((r - 45) & 1) * d.s1 + ((r - 45) >> 1) * d.s2;
     src += base;
     const unsigned dst = smem_u32(stage + r * UPD_ROW);
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-                 "l"(src), "r"(bytes), "r"(bar)
-                 : "memory");
-  }
-}
-
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
-  unsigned done = 0;
-  while (!done) {
-    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                 : "=r"(done)
-                 : "r"(bar), "r"(parity)
-                 : "memory");
+    bulk_g2s(dst, src, bytes, bar);
   }
 }
 
@@ -353,8 +339,8 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(Up
   const int G = gridDim.x;
   const unsigned bar0 = smem_u32(&mbar);
   if (t == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar0));
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    mbar_init(bar0, 1);
+    mbar_fence_init();
   }
   __syncthreads();
   int tile = blockIdx.x;

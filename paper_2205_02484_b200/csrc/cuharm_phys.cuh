@@ -392,10 +392,8 @@ __device__ __forceinline__ int invert_2d(const double U[8], const Geom& G, doubl
   }
   if (!(v2 < 1.0)) return 3;
   v2 = v2 < 0.0 ? 0.0 : v2;
-  bool converged = false;
-  int extra_left = -1;
-  int it;
-  for (it = 1; it <= nc.maxit; it++) {
+  // One Newton update of (W, v^2); returns whether |dW/W| <= tol held for this update.
+  auto newton_step = [&]() {
     const double iW = frcp(W);
     const double iW2 = iW * iW, iW3 = iW2 * iW;
     const double omv = 1.0 - v2;
@@ -416,19 +414,27 @@ __device__ __forceinline__ int invert_2d(const double U[8], const Geom& G, doubl
     double vn = v2 + dv;
     vn = vn < 0.0 ? 0.0 : vn;
     vn = vn > 1.0 - 1e-15 ? 1.0 - 1e-15 : vn;
-    const bool small = (Wn == 0.0) ? (fabs(dW) <= nc.tol) : (fabs(dW) <= nc.tol * Wn);  // |dW/W| <= tol
     W = Wn;
     v2 = vn;
-    if (!isfinite(W) || !isfinite(v2) || W == 0.0) { iters = it; return 3; }
-    if (extra_left < 0) {
-      if (small) extra_left = nc.extra;
-    } else {
-      extra_left--;
-    }
-    if (extra_left == 0) { converged = true; break; }
+    return (Wn == 0.0) ? (fabs(dW) <= nc.tol) : (fabs(dW) <= nc.tol * Wn);  // |dW/W| <= tol
+  };
+  // iterate to the criterion (the only data-dependent branch), then `extra` more updates, all within maxit; a
+  // non-finite iterate never meets the criterion, so finiteness is tested once, after the loops
+  int it = 1;
+  bool small = false;
+  for (; it <= nc.maxit; it++) {
+    small = newton_step();
+    if (small) break;
+  }
+  int more = 0;
+  if (small) {
+    more = min(nc.extra, nc.maxit - it);
+    for (int e = 0; e < more; e++) newton_step();
+    it += more;
   }
   iters = it > nc.maxit ? nc.maxit : it;
-  if (!converged) return 2;
+  if (!isfinite(W) || !isfinite(v2) || W == 0.0) return 3;
+  if (!small || more < nc.extra) return 2;
   if (!(W > 0.0)) return 3;
   if (!(v2 >= 0.0 && v2 < 1.0)) return 4;
   const double omv = 1.0 - v2;
