@@ -293,11 +293,13 @@ constexpr int UPD_ROW = 132;   // doubles per staged row: 1 + 128 + 1 (k+1) + 2 
 constexpr int UPD_NROW = 49;   // 8 P^n, 8 P-flux, 10 F1, 10 F2, 5 F3, 2 E1, 2 E2, 4 E3
 
 // issue the bulk copies of one tile (rows of zones kb.. of row (i,j)) into one stage; called by threads 0..63
+struct TileIdx { int i, j, c; };  // zone-row (i, j) (interior numbering) and 128-zone chunk of a tile
+
 template <bool SAME>
-__device__ __forceinline__ void upd_issue_tile(const UpdArgs& a, int tile, int nch, double* stage, unsigned bar) {
+__device__ __forceinline__ void upd_issue_tile(const UpdArgs& a, TileIdx x, double* stage, unsigned bar) {
   const Dims& d = a.d;
-  const int c = tile % nch, ij = tile / nch;
-  const int j = d.ng + ij % d.n2, i = d.ng + ij / d.n2;
+  const int c = x.c;
+  const int j = d.ng + x.j, i = d.ng + x.i;
   const int kb = d.ng + c * 128 - 1;                      // first staged zone of the row (even)
   const unsigned bytes = (unsigned)min(UPD_ROW - 2, d.n3g - kb) * 8u;  // staged zones per row: even count
   const long long base = i * d.s1 + j * d.s2 + kb;       // element offset of the segment in every array
@@ -344,12 +346,26 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(Up
   }
   __syncthreads();
   int tile = blockIdx.x;
-  if (t < 64 && tile < ntiles) upd_issue_tile<SAME>(a, tile, nch, rows, bar0);
+  // decomposition of the first tile and of the stride, then carried increments (no division in the loop)
+  TileIdx cur, nxt, dlt;
+  {
+    int r = tile / nch;
+    cur.c = tile % nch; cur.j = r % d.n2; cur.i = r / d.n2;
+    r = G / nch;
+    dlt.c = G % nch; dlt.j = r % d.n2; dlt.i = r / d.n2;
+  }
+  auto advance = [&](const TileIdx& x) {
+    TileIdx y{x.i + dlt.i, x.j + dlt.j, x.c + dlt.c};
+    if (y.c >= nch) { y.c -= nch; y.j++; }
+    if (y.j >= d.n2) { y.j -= d.n2; y.i++; }
+    return y;
+  };
+  if (t < 64 && tile < ntiles) upd_issue_tile<SAME>(a, cur, rows, bar0);
   int cnt_acc[5] = {0, 0, 0, 0, 0};
-  for (int n = 0; tile < ntiles; tile += G, n++) {
-    const int c = tile % nch, ij = tile / nch;
-    const int j = d.ng + ij % d.n2, i = d.ng + ij / d.n2;
-    const int k0 = d.ng + c * 128;
+  for (int n = 0; tile < ntiles; tile += G, n++, cur = nxt) {
+    nxt = advance(cur);
+    const int j = d.ng + cur.j, i = d.ng + cur.i;
+    const int k0 = d.ng + cur.c * 128;
     const bool live = k0 + t < d.ng + d.n3;
     const int tc = live ? t : d.ng + d.n3 - 1 - k0;  // clamped lane position
     const long long idx = i * d.s1 + j * d.s2 + k0 + tc;
@@ -371,7 +387,7 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(Up
     ex[4] = z[43 * UPD_ROW]; ex[5] = z[44 * UPD_ROW]; ex[6] = z[43 * UPD_ROW + 1]; ex[7] = z[44 * UPD_ROW + 1];
     ex[8] = z[45 * UPD_ROW]; ex[9] = z[46 * UPD_ROW]; ex[10] = z[47 * UPD_ROW]; ex[11] = z[48 * UPD_ROW];
     __syncthreads();  // every thread holds its operands: the stage can be refilled
-    if (t < 64 && tile + G < ntiles) upd_issue_tile<SAME>(a, tile + G, nch, rows, bar0);
+    if (t < 64 && tile + G < ntiles) upd_issue_tile<SAME>(a, nxt, rows, bar0);
     int cnt[5] = {0, 0, 0, 0, 0};
     update_zone<SAME>(a, pb, pf, fx, ex, idx, q2, live, cnt);
 #pragma unroll
