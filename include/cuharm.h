@@ -105,7 +105,8 @@ int cuharm_cfl_dt(cuharm_handle h, double xi, double* dt_out);
 int cuharm_last_cfl_dt(cuharm_handle h, double xi, double* dt_out);
 
 /* Corner-centred discrete divergence of sqrt(-g) B (eq. 23; A4) over the corners whose cells are
- * interior: *max_abs = max |D|, *max_norm = max |D| / (sum of the magnitudes of D's own terms).  Synchronises. */
+ * interior: *max_abs = max |D|, *max_norm = max |D| / (sum of the magnitudes of D's own terms), the latter over
+ * the corners where that sum exceeds 1e-290 (below it the terms are in the subnormal range).  Synchronises. */
 int cuharm_divb(cuharm_handle h, double* max_abs, double* max_norm);
 
 /* Copy a geometry table to a caller array d_out[comp][n1g][n2g]: loc 0 centre, 1 = 1-face (I-1/2,J), 2 = 2-face

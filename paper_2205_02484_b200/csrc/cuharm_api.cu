@@ -211,7 +211,12 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
     int rc = launch_flux<false>(h, Pflux, dir, h->F[dir - 1], nullptr, cwmax + (dir - 1));
     if (rc) return rc;
   }
-  {
+  // bulk-copy (TMA) staging of the update kernel needs 16-byte aligned row segments: even n3g, aligned arrays.
+  // That kernel evaluates the edge EMFs itself (flux-CT fused); otherwise they go through emf_kernel and h->E.
+  const uintptr_t al = (uintptr_t)Pbase | (uintptr_t)Pflux | (uintptr_t)h->F[0] | (uintptr_t)h->F[1] |
+                       (uintptr_t)h->F[2] | (uintptr_t)h->E;
+  const bool tma = h->upd_tma && (d.n3g % 2 == 0) && (al % 16 == 0);
+  if (!tma) {
     Timed t_(h, CUHARM_K_EMF);
     EmfArgs a{d, h->F[0], h->F[1], h->F[2], h->E};
     emf_kernel<<<dim3((d.n3 + 1 + 127) / 128, d.n2 + 1, d.n1 + 1), 128, 0, h->stream>>>(a);
@@ -224,10 +229,6 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
               nfail, h->cnt + CNT_STATS, dtau, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], h->p.gam,
               newton_cfg(h->p), floor_cfg(h->p)};
     dim3 grid((d.n3 + 127) / 128, d.n2, d.n1);
-    // bulk-copy (TMA) staging needs 16-byte aligned row segments: even n3g and 16-byte aligned arrays
-    const uintptr_t al = (uintptr_t)Pbase | (uintptr_t)Pflux | (uintptr_t)h->F[0] | (uintptr_t)h->F[1] |
-                         (uintptr_t)h->F[2] | (uintptr_t)h->E;
-    const bool tma = h->upd_tma && (d.n3g % 2 == 0) && (al % 16 == 0);
     const size_t smem = (size_t)UPD_NROW * UPD_ROW * sizeof(double);
     if (tma) {
       const int nch = (d.n3 + 127) / 128;

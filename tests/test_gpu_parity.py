@@ -250,6 +250,12 @@ def test_cfl_dt_and_divb_values_match():
     s.load(bad)
     a, n = s.divb(); ar, nr = g.divb()
     assert abs(a / ar - 1) < 1e-12 and abs(n / nr - 1) < 1e-12 and nr > 1e-3
+    # the same pattern scaled into the subnormal range: skipped by the normalised measure on both sides (A4)
+    tiny = ref.copy(); tiny[5:8] = 1e-300 * r.uniform(0.5, 1.0, size=tiny[5:8].shape)
+    g.bind(tiny)
+    s.load(tiny)
+    a, n = s.divb(); ar, nr = g.divb()
+    assert n == 0.0 and nr == 0.0 and 0.0 < ar < 1e-290 and abs(a / ar - 1) < 1e-9
 
 
 # ------------------------------------------------------------------ S8: repair of failed zones (eq. 34)

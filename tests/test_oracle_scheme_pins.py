@@ -160,6 +160,25 @@ def test_cfl_closed_form_uniform_minkowski():
     assert abs(g.cfl_dt(xi) * inv - 1.0) < 1e-13
 
 
+def test_divb_normalised_measure_skips_subnormal_range_corners():
+    """A4 (addition): corners whose terms sum to < 1e-290 do not enter max |D| / sum|terms| (rounding is absolute in
+    the subnormal range, so the ratio is O(1) there for any field); max |D| still sees them, and a field of ordinary
+    magnitude with the same non-solenoidal pattern is reported as O(1)."""
+    p = minkowski_params(6, 5, 4)
+    prim = uniform_state(p, [1.0, 1.0, 0, 0, 0, 0, 0, 0])
+    rng = np.random.Generator(np.random.PCG64(7))
+    pattern = rng.uniform(0.5, 1.0, size=prim[5].shape)
+    prim[5] = 1e-300 * pattern          # not solenoidal, subnormal-range terms
+    g = oracle.Grid(p)
+    g.bind(prim)
+    mabs, mnorm = g.divb()
+    assert mnorm == 0.0 and 0.0 < mabs < 1e-295
+    prim[5] = 1e-3 * pattern
+    g.bind(prim)
+    mabs, mnorm = g.divb()
+    assert mnorm > 1e-2 and mabs > 1e-4
+
+
 # ------------------------------------------------------------------ pin 9: flux-CT keeps eq. 23 for ARBITRARY fluxes
 @pytest.mark.parametrize("kind", ["minkowski", "mks"])
 def test_flux_ct_preserves_divb_for_arbitrary_fluxes(kind):
