@@ -229,7 +229,7 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
               nfail, h->cnt + CNT_STATS, dtau, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], h->p.gam,
               newton_cfg(h->p), floor_cfg(h->p)};
     dim3 grid((d.n3 + 127) / 128, d.n2, d.n1);
-    const size_t smem = (size_t)UPD_NROW * UPD_ROW * sizeof(double);
+    const size_t smem = UPD_SMEM;
     if (tma) {
       const int nch = (d.n3 + 127) / 128;
       const long long nt = (long long)d.n1 * d.n2 * nch;
@@ -316,7 +316,7 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
     for (int c = 0; c < 3; c++) { h->x0[c] = p->xmin[c]; h->dx[c] = (p->xmax[c] - p->xmin[c]) / n[c]; }
   }
   {  // opt in to the dynamic shared memory of the bulk-copy update kernel (51.7 KB per block)
-    const int smem = UPD_NROW * UPD_ROW * (int)sizeof(double);
+    const int smem = UPD_SMEM;
     const cudaError_t e1 = cudaFuncSetAttribute(update_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     const cudaError_t e2 = cudaFuncSetAttribute(update_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     h->upd_tma = (e1 == cudaSuccess && e2 == cudaSuccess);

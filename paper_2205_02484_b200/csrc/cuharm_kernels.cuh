@@ -170,7 +170,8 @@ struct UpdArgs {
 // ex = E1 at (0, +j, +k, +j+k), E2 at (0, +i, +k, +i+k), E3 at (0, +i, +j, +i+j).
 template <bool SAME>
 __device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8], const double pf[8], const double fx[30],
-                                            const double ex[12], long long idx, int q2, bool live, int cnt[5]) {
+                                            const double ex[12], const Geom& G, const double* cn, double rfl, double ufl,
+                                            long long idx, int q2, bool live, int cnt[5]) {
   const Dims& d = a.d;
   double dU[8];  // -div F (eq. 25)
 #pragma unroll
@@ -195,18 +196,17 @@ __device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8]
     dU[6] = -divB2;
     dU[7] = -divB3;
   }
-  // per-(i,j) tables (broadcast loads, L1/L2 resident), U^n, source, update
-  const Geom G = load_geom(a.C, q2);
+  // U^n, source, update
   State S;
   fluid_state(pb, G, S);
   double U[8];
   flux_vector<0>(pb, S, G, a.gam, U);
   double src[4];
   if (SAME) {
-    source_term(pb, S, G, a.conn + (size_t)q2 * 40, a.gam, src);
+    source_term(pb, S, G, cn, a.gam, src);
   } else {
     fluid_state(pf, G, S);
-    source_term(pf, S, G, a.conn + (size_t)q2 * 40, a.gam, src);
+    source_term(pf, S, G, cn, a.gam, src);
   }
   U[0] = fma(a.dtau, dU[0], U[0]);
 #pragma unroll
@@ -220,7 +220,7 @@ __device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8]
   const int flag = invert_2d(U, G, a.gam, pn, a.nc, its);
   int m = 0;
   if (flag == 0) {
-    m = apply_floors(pn, G, a.C + q2, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), a.fc, a.gam, a.nc);
+    m = apply_floors(pn, G, a.C + q2, rfl, ufl, a.fc, a.gam, a.nc);
   } else if (live) {
     const unsigned long long pos = atomicAdd(a.nfail, 1ull);
     a.list[pos] = (int)idx;
@@ -278,8 +278,11 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_MINB) update_kernel(UpdArgs a)
     ex[4] = __ldg(E2); ex[5] = __ldg(E2 + d.s1); ex[6] = __ldg(E2 + 1); ex[7] = __ldg(E2 + d.s1 + 1);
     ex[8] = __ldg(E3); ex[9] = __ldg(E3 + d.s1); ex[10] = __ldg(E3 + d.s2); ex[11] = __ldg(E3 + d.s1 + d.s2);
   }
+  const Geom G = load_geom(a.C, q2);
+  double cn[40];
+  load_conn(a.conn + (size_t)q2 * 40, cn);
   int cnt[5] = {0, 0, 0, 0, 0};
-  update_zone<SAME>(a, pb, pf, fx, ex, idx, q2, live, cnt);
+  update_zone<SAME>(a, pb, pf, fx, ex, G, cn, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), idx, q2, live, cnt);
   update_stats(a, cnt);
 }
 
@@ -296,6 +299,8 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_MINB) update_kernel(UpdArgs a)
 // and div B stays at round-off exactly as with the stored EMFs.
 constexpr int UPD_ROW = 132;   // doubles per staged row: 1 + 128 + 1 (k+1) + 2 pad -> 1056 B, a multiple of 16
 constexpr int UPD_NROW = 63;   // 8 P^n, 8 P-flux, 10 F1, 10 F2, 5 F3 (hydro), 22 induction-flux rows
+constexpr int UPD_TAB = 62;    // doubles of per-(i,j) records staged behind the rows: Geom 20, connection 40, floors 2
+constexpr int UPD_SMEM = (UPD_NROW * UPD_ROW + 2 * 64) * 8;  // dynamic shared memory per block, bytes
 
 // row r of the stage: which array, which component, which (di, dj) offset of the zone row
 struct UpdRowSrc { signed char arr, comp, di, dj; };  // arr: 0 Pbase, 1 Pflux, 2 F1, 3 F2, 4 F3
@@ -358,21 +363,32 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(Up
   auto tile_bytes = [&](const TileIdx& x) {  // staged zones per row (even count) x 8
     return (unsigned)min(UPD_ROW - 2, d.n3g - (d.ng + x.c * 128 - 1)) * 8u;
   };
-  // thread r < UPD_NROW owns row r: its source pointer for the tile at offset 0, then tile by tile + base
-  const bool issuer = t < UPD_NROW && !(SAME && t >= 8 && t < 16);
+  // Row r is owned by thread 2r (a warp issues its bulk copies one after the other, so the rows are spread over
+  // all four warps): its source pointer for the tile at offset 0, then tile by tile + base.  Thread 127 owns the
+  // three per-(i,j) records (geometry, connection, floors), which ride along as rows 63..65.
+  const int row = t >> 1;
+  const bool issuer = !(t & 1) && row < UPD_NROW && !(SAME && row >= 8 && row < 16);
   const double* src0 = nullptr;
   if (issuer) {
-    const UpdRowSrc q = upd_row_src(t);
+    const UpdRowSrc q = upd_row_src(row);
     const double* arr = q.arr == 0 ? a.Pbase : q.arr == 1 ? a.Pflux : q.arr == 2 ? a.F1 : q.arr == 3 ? a.F2 : a.F3;
     src0 = arr + q.comp * d.nz + q.di * d.s1 + q.dj * d.s2;
   }
-  const unsigned dst = smem_u32(rows + t * UPD_ROW);
-  auto issue = [&](const TileIdx& x) {
+  const unsigned dst = smem_u32(rows + row * UPD_ROW);
+  double* const tab = rows + UPD_NROW * UPD_ROW;  // two slots of [20] geometry record, [40] connection, [2] floors
+  auto issue = [&](const TileIdx& x, int slot) {
     const unsigned bytes = tile_bytes(x);
-    if (t == 0) mbar_expect_tx(bar0, bytes * (SAME ? UPD_NROW - 8 : UPD_NROW));
+    if (t == 0) mbar_expect_tx(bar0, bytes * (SAME ? UPD_NROW - 8 : UPD_NROW) + UPD_TAB * 8u);
     if (issuer) bulk_g2s(dst, src0 + tile_base(x), bytes, bar0);
+    if (t == 127) {
+      const size_t q = (size_t)(d.ng + x.i) * d.n2g + (d.ng + x.j);
+      double* const tb = tab + slot * 64;
+      bulk_g2s(smem_u32(tb), a.C + q, 160u, bar0);
+      bulk_g2s(smem_u32(tb + 20), a.conn + q * 40, 320u, bar0);
+      bulk_g2s(smem_u32(tb + 60), a.floors + q * 2, 16u, bar0);
+    }
   };
-  if (t < 64 && tile < ntiles) issue(cur);
+  if (tile < ntiles) issue(cur, 0);
   int cnt_acc[5] = {0, 0, 0, 0, 0};
   for (int n = 0; tile < ntiles; tile += G, n++, cur = nxt) {
     nxt = advance(cur);
@@ -414,9 +430,12 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(Up
     ex[11] = 0.25 * (ROWZ(56, 0) + ROWZ(55, 0) - ROWZ(62, 0) - ROWZ(61, 0));  // E3(i+1, j+1)
 #undef ROWZ
     __syncthreads();  // every thread holds its operands: the stage can be refilled
-    if (t < 64 && tile + G < ntiles) issue(nxt);
+    if (tile + G < ntiles) issue(nxt, (n + 1) & 1);
     int cnt[5] = {0, 0, 0, 0, 0};
-    update_zone<SAME>(a, pb, pf, fx, ex, idx, q2, live, cnt);
+    // the per-(i,j) records of this tile stay valid in their own (double-buffered) slot for the whole tile
+    const double* tb = tab + (n & 1) * 64;
+    const Geom Gc = load_geom_shared(tb);
+    update_zone<SAME>(a, pb, pf, fx, ex, Gc, tb + 20, tb[60], tb[61], idx, q2, live, cnt);
 #pragma unroll
     for (int q = 0; q < 5; q++) cnt_acc[q] += cnt[q];
   }

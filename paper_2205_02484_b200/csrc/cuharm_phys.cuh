@@ -40,6 +40,24 @@ __device__ __forceinline__ Geom load_geom(const Geom* __restrict__ tab, int q) {
   return G;
 }
 
+// the same record from shared memory (or any generic pointer): plain loads
+__device__ __forceinline__ Geom load_geom_shared(const double* t) {
+  const double2* s = reinterpret_cast<const double2*>(t);
+  Geom G;
+  double2 v;
+  v = s[0]; G.g00 = v.x; G.g01 = v.y;
+  v = s[1]; G.g03 = v.x; G.g11 = v.y;
+  v = s[2]; G.g13 = v.x; G.g22 = v.y;
+  v = s[3]; G.g33 = v.x; G.c00 = v.y;
+  v = s[4]; G.c01 = v.x; G.c03 = v.y;
+  v = s[5]; G.c11 = v.x; G.c13 = v.y;
+  v = s[6]; G.c22 = v.x; G.c33 = v.y;
+  v = s[7]; G.sg = v.x; G.alpha = v.y;
+  v = s[8]; G.ialpha = v.x; G.ac01 = v.y;
+  v = s[9]; G.isg = v.x; G.pad = 0.0;
+  return G;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // Reciprocal and reciprocal square root for the hot path: the hardware seed (MUFU.RCP64H / MUFU.RSQ64H, about 20
 // good bits) plus ONE third-order Newton step, no special-case path.  Result within 2 ulp for normal, finite
@@ -311,7 +329,13 @@ __device__ __forceinline__ constexpr int pair_index(int n, int k) {
   return lo * 4 - (lo * (lo - 1)) / 2 + (hi - lo);
 }
 
-__device__ __forceinline__ void source_term(const double q[8], const State& S, const Geom& G, const double* __restrict__ conn,
+__device__ __forceinline__ void load_conn(const double* __restrict__ conn, double cn[40]) {
+  const double2* c2 = reinterpret_cast<const double2*>(conn);
+#pragma unroll
+  for (int s = 0; s < 20; s++) { const double2 v = __ldg(c2 + s); cn[2 * s] = v.x; cn[2 * s + 1] = v.y; }
+}
+
+__device__ __forceinline__ void source_term(const double q[8], const State& S, const Geom& G, const double* cn,
                                             double gam, double src[4]) {
   const double pg = (gam - 1.0) * q[1];
   const double w = q[0] + q[1] + pg;
@@ -319,10 +343,6 @@ __device__ __forceinline__ void source_term(const double q[8], const State& S, c
   const double ptot = fma(0.5, S.bsq, pg);
   const double uc[4] = {S.u0, S.u1, S.u2, S.u3}, ul[4] = {S.l0, S.l1, S.l2, S.l3};
   const double bc[4] = {S.b0, S.b1, S.b2, S.b3}, bl[4] = {S.m0, S.m1, S.m2, S.m3};
-  double cn[40];
-  const double2* c2 = reinterpret_cast<const double2*>(conn);
-#pragma unroll
-  for (int s = 0; s < 20; s++) { const double2 v = __ldg(c2 + s); cn[2 * s] = v.x; cn[2 * s + 1] = v.y; }
   double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
 #pragma unroll
   for (int k = 0; k < 4; k++) {
