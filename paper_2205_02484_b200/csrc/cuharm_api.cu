@@ -61,6 +61,7 @@ struct cuharm_ctx {
   // graph
   bool upd_tma = false;  // update_tma_kernel usable (shared-memory opt-in succeeded)
   int upd_blocks = 0;    // its persistent grid size
+  int sms = 148;         // multiprocessors of the device
   int fluxk_blocks = 0;  // persistent grid size of flux_k_tma_kernel (0: not usable)
   bool use_graph = false;
   cudaGraphExec_t gexec = nullptr;
@@ -143,15 +144,23 @@ int launch_bc(cuharm_ctx* h, double* P, const unsigned long long* gate) {
   return CUHARM_OK;
 }
 
-// number of marching segments per column: enough warps for several waves over the 148 SMs, segments not shorter
-// than 16 faces (the prologue of a segment reconstructs one extra cell)
-int march_seg(long long columns, int nfaces) {
-  const long long warps = (columns + 31) / 32;
-  int nseg = (int)((148LL * 16 * 6 + warps - 1) / warps);
-  const int maxseg = (nfaces + 15) / 16;
-  if (nseg > maxseg) nseg = maxseg;
-  if (nseg < 1) nseg = 1;
-  return (nfaces + nseg - 1) / nseg;  // faces per segment
+// Faces per marching segment.  A block costs (faces + ~0.6) face-times (the prologue of a segment reconstructs one
+// extra cell) and the 2 x SMs resident blocks run in waves, so the segment count is chosen to minimise
+// waves x (faces per segment + 0.6) among the counts that keep segments at least 16 faces long.
+int march_seg(long long columns, int nfaces, int sms) {
+  const long long col_blocks = (columns + 127) / 128;
+  const long long slots = 2LL * (sms > 0 ? sms : 148);
+  const int maxseg = nfaces >= 32 ? nfaces / 16 : 1;
+  int best = 1;
+  double best_cost = 1e300;
+  for (int nseg = 1; nseg <= maxseg; nseg++) {
+    const int seg = (nfaces + nseg - 1) / nseg;
+    const long long blocks = col_blocks * ((nfaces + seg - 1) / seg);
+    const double waves = (double)((blocks + slots - 1) / slots);
+    const double cost = waves * (seg + 0.6);
+    if (cost < best_cost * 0.999) { best_cost = cost; best = nseg; }
+  }
+  return (nfaces + best - 1) / best;  // faces per segment
 }
 
 template <int RECON, int RIEMANN, bool STAGE>
@@ -173,7 +182,7 @@ void launch_flux_t(cuharm_ctx* h, FluxArgs& a, int dir) {
   } else {
     const long long cols = (long long)(dir == 1 ? nj : ni) * nk;
     const int nf = dir == 1 ? ni : nj;
-    a.seg = march_seg(cols, nf);
+    a.seg = march_seg(cols, nf, h->sms);
     const dim3 grid((unsigned)((cols + 127) / 128), (unsigned)((nf + a.seg - 1) / a.seg));
     if (dir == 1) flux_march_kernel<1, RECON, RIEMANN, STAGE><<<grid, 128, 0, h->stream>>>(a);
     else flux_march_kernel<2, RECON, RIEMANN, STAGE><<<grid, 128, 0, h->stream>>>(a);
@@ -333,6 +342,7 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
       int dev = 0, sms = 0, per = 0;
       cudaGetDevice(&dev);
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+      if (sms > 0) h->sms = sms;
       if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, flux_k_tma_kernel<1, 0, false>, 128, 0) == cudaSuccess && per > 0)
         h->fluxk_blocks = sms * per;
       else
