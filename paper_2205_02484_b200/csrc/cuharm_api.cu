@@ -70,6 +70,10 @@ struct cuharm_ctx {
   int64_t graph_nodes = 0;
 };
 
+#ifndef CUHARM_UPD_STRIP
+#define CUHARM_UPD_STRIP 8
+#endif
+
 namespace {
 
 struct WsLayout {
@@ -244,8 +248,11 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
       const long long nt = (long long)d.n1 * d.n2 * nch;
       const int ntiles = (int)nt;
       const int nb = (int)std::min<long long>(nt, h->upd_blocks);
-      if (Pflux == Pbase) update_tma_kernel<true><<<nb, 128, smem, h->stream>>>(a, ntiles, nch);
-      else update_tma_kernel<false><<<nb, 128, smem, h->stream>>>(a, ntiles, nch);
+      int wj = 1;  // strip width: the largest divisor of n2 not above CUHARM_UPD_STRIP
+      for (int w = 1; w <= CUHARM_UPD_STRIP && w <= d.n2; w++)
+        if (d.n2 % w == 0) wj = w;
+      if (Pflux == Pbase) update_tma_kernel<true><<<nb, 128, smem, h->stream>>>(a, ntiles, nch, wj);
+      else update_tma_kernel<false><<<nb, 128, smem, h->stream>>>(a, ntiles, nch, wj);
     } else {
       if (Pflux == Pbase) update_kernel<true><<<grid, 128, 0, h->stream>>>(a);
       else update_kernel<false><<<grid, 128, 0, h->stream>>>(a);

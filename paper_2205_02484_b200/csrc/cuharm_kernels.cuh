@@ -320,6 +320,7 @@ __device__ __forceinline__ UpdRowSrc upd_row_src(int r) {
 }
 
 struct TileIdx { int i, j, c; };  // zone-row (i, j) (interior numbering) and 128-zone chunk of a tile
+struct TileCnt { int s, i, jj, c; };  // mixed-radix tile counter: j-strip, i, j within the strip, chunk
 
 // Persistent blocks: block b takes tiles b, b + gridDim.x, ...; tile = (i, j, 128-zone chunk of the row), chunk
 // fastest.  One stage per block: the stage is free again as soon as every thread has moved its operands to
@@ -330,7 +331,7 @@ struct TileIdx { int i, j, c; };  // zone-row (i, j) (interior numbering) and 12
 #define CUHARM_UPD_TMA_MINB 3
 #endif
 template <bool SAME>
-__global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(UpdArgs a, int ntiles, int nch) {
+__global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(UpdArgs a, int ntiles, int nch, int wj) {
   extern __shared__ __align__(128) double rows[];  // [UPD_NROW][UPD_ROW]
   __shared__ __align__(8) unsigned long long mbar;
   const Dims& d = a.d;
@@ -343,20 +344,26 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(Up
   }
   __syncthreads();
   int tile = blockIdx.x;
-  // decomposition of the first tile and of the stride, then carried increments (no division in the loop)
-  TileIdx cur, nxt, dlt;
+  // Tile order: strips of wj rows j; inside a strip i runs slower than j, the chunk fastest.  The blocks resident
+  // at one time then cover a patch of (several i) x (wj j) rows, so the rows a tile shares with its i- and
+  // j-neighbours (F1[i+1], F2[j+1], the induction fluxes around each edge) are re-read while still in L2.
+  // Decomposition of the first tile and of the stride, then carried increments (no division in the loop).
+  TileCnt ccur, cdlt;
   {
-    int r = tile / nch;
-    cur.c = tile % nch; cur.j = r % d.n2; cur.i = r / d.n2;
-    r = G / nch;
-    dlt.c = G % nch; dlt.j = r % d.n2; dlt.i = r / d.n2;
+    int r = tile;
+    ccur.c = r % nch; r /= nch; ccur.jj = r % wj; r /= wj; ccur.i = r % d.n1; ccur.s = r / d.n1;
+    r = G;
+    cdlt.c = r % nch; r /= nch; cdlt.jj = r % wj; r /= wj; cdlt.i = r % d.n1; cdlt.s = r / d.n1;
   }
-  auto advance = [&](const TileIdx& x) {
-    TileIdx y{x.i + dlt.i, x.j + dlt.j, x.c + dlt.c};
-    if (y.c >= nch) { y.c -= nch; y.j++; }
-    if (y.j >= d.n2) { y.j -= d.n2; y.i++; }
+  auto advance_cnt = [&](const TileCnt& x) {
+    TileCnt y{x.s + cdlt.s, x.i + cdlt.i, x.jj + cdlt.jj, x.c + cdlt.c};
+    if (y.c >= nch) { y.c -= nch; y.jj++; }
+    if (y.jj >= wj) { y.jj -= wj; y.i++; }
+    if (y.i >= d.n1) { y.i -= d.n1; y.s++; }
     return y;
   };
+  auto to_idx = [&](const TileCnt& x) { return TileIdx{x.i, x.s * wj + x.jj, x.c}; };
+  TileIdx cur = to_idx(ccur), nxt;
   auto tile_base = [&](const TileIdx& x) {  // element offset of the first staged zone of the tile's row
     return (long long)(d.ng + x.i) * d.s1 + (long long)(d.ng + x.j) * d.s2 + (d.ng + x.c * 128 - 1);
   };
@@ -391,7 +398,8 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(Up
   if (tile < ntiles) issue(cur, 0);
   int cnt_acc[5] = {0, 0, 0, 0, 0};
   for (int n = 0; tile < ntiles; tile += G, n++, cur = nxt) {
-    nxt = advance(cur);
+    ccur = advance_cnt(ccur);
+    nxt = to_idx(ccur);
     const int j = d.ng + cur.j, i = d.ng + cur.i;
     const int k0 = d.ng + cur.c * 128;
     const bool live = k0 + t < d.ng + d.n3;
