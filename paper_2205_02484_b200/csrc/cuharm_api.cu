@@ -62,7 +62,7 @@ struct cuharm_ctx {
   bool upd_tma = false;  // update_tma_kernel usable (shared-memory opt-in succeeded)
   int upd_blocks = 0;    // its persistent grid size
   int sms = 148;         // multiprocessors of the device
-  int fluxk_blocks = 0;  // persistent grid size of flux_k_tma_kernel (0: not usable)
+  bool fluxk_row = true; // prefer the whole-row pipeline (flux_k_row_kernel)
   bool use_graph = false;
   cudaGraphExec_t gexec = nullptr;
   cudaStream_t cap_stream = nullptr;
@@ -174,11 +174,19 @@ void launch_flux_t(cuharm_ctx* h, FluxArgs& a, int dir) {
     const int fpw = FluxK<RECON>::FPW;
     const int wpr = (nk + fpw - 1) / fpw;
     const Dims& d = a.d;
-    const bool tma = h->fluxk_blocks > 0 && (d.n3g % 2 == 0) && ((uintptr_t)a.P % 16 == 0);
-    if (tma) {
-      const long long items = (long long)ni * nj * wpr;
-      const int nb = (int)std::min<long long>((items + 3) / 4, h->fluxk_blocks);
-      flux_k_tma_kernel<RECON, RIEMANN, STAGE><<<nb, 128, 0, h->stream>>>(a, wpr);
+    const bool tma = h->fluxk_row && (d.n3g % 2 == 0) && ((uintptr_t)a.P % 16 == 0);
+    const size_t row_smem = 2 * 8 * (size_t)d.n3g * sizeof(double);
+    bool row_ok = tma && row_smem <= 200 * 1024;
+    if (row_ok && row_smem > 48 * 1024)
+      row_ok = cudaFuncSetAttribute(flux_k_row_kernel<RECON, RIEMANN, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)row_smem) == cudaSuccess;
+    if (row_ok) {
+      // whole-row pipeline: warps per block chosen to divide the chunks of a row evenly
+      const int nw = wpr % 3 == 0 ? 3 : (wpr % 4 == 0 ? 4 : (wpr % 2 == 0 ? 2 : (wpr >= 4 ? 4 : wpr)));
+      int per = 0;
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, flux_k_row_kernel<RECON, RIEMANN, STAGE>, 32 * nw, row_smem) != cudaSuccess || per < 1) per = 1;
+      const int nb = (int)std::min<long long>((long long)ni * nj, (long long)h->sms * per);
+      flux_k_row_kernel<RECON, RIEMANN, STAGE><<<nb, 32 * nw, row_smem, h->stream>>>(a, wpr);
     } else {
       const dim3 grid((unsigned)wpr, (unsigned)((nj + 3) / 4), (unsigned)ni);
       flux_k_kernel<RECON, RIEMANN, STAGE><<<grid, 128, 0, h->stream>>>(a);
@@ -331,7 +339,7 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
     const int n[3] = {p->n1, p->n2, p->n3};
     for (int c = 0; c < 3; c++) { h->x0[c] = p->xmin[c]; h->dx[c] = (p->xmax[c] - p->xmin[c]) / n[c]; }
   }
-  {  // opt in to the dynamic shared memory of the bulk-copy update kernel (51.7 KB per block)
+  {  // opt in to the dynamic shared memory of the bulk-copy update kernel (67.5 KB per block)
     const int smem = UPD_SMEM;
     const cudaError_t e1 = cudaFuncSetAttribute(update_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     const cudaError_t e2 = cudaFuncSetAttribute(update_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -346,18 +354,17 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
     }
     if (!h->upd_tma) cudaGetLastError();
     {
-      int dev = 0, sms = 0, per = 0;
+      int dev = 0, sms = 0;
       cudaGetDevice(&dev);
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
       if (sms > 0) h->sms = sms;
-      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, flux_k_tma_kernel<1, 0, false>, 128, 0) == cudaSuccess && per > 0)
-        h->fluxk_blocks = sms * per;
-      else
-        cudaGetLastError();
     }
+#ifdef CUHARM_NO_ROW
+    h->fluxk_row = false;
+#endif
 #ifdef CUHARM_NO_TMA
     h->upd_tma = false;
-    h->fluxk_blocks = 0;
+    h->fluxk_row = false;
 #endif
   }
   *out = h;

@@ -297,110 +297,98 @@ __global__ void __launch_bounds__(128, CUHARM_FLUXK_MINB) flux_k_kernel(FluxArgs
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Direction 3, bulk-copy version (n3g even, 16-byte aligned P): persistent warps, each with its own one-stage
-// pipeline.  Work item = (i, j, w) as above, w fastest; warp g takes items g, g + W, ...  The 34 cells x 8 variables
-// an item reads arrive as 8 bulk copies of KSEG doubles into the warp's stage; the stage is free again once the
-// lanes have moved their three cells per variable to registers, so the copies of the next item fly during the
-// whole of this item's arithmetic and no lane ever waits on DRAM with a scoreboard.
+// Direction 3, whole-row version (n3g even, 16-byte aligned P): persistent blocks of NW warps.  A work item is one
+// (i, j) row: its 8 variables arrive as 8 bulk copies of the whole row (n3g doubles each) into one of two stages,
+// and warp w of the block takes the chunks w, w + NW, ... of the row (29 / 31 faces each, as above).  Compared with
+// per-thread loads nothing waits on DRAM with a scoreboard (the copies of the next two rows fly during the
+// arithmetic of this one), and whole rows keep the copy count low: a warp issues its bulk copies one after the
+// other at ~8 issue slots each.
 // ---------------------------------------------------------------------------------------------------------
-constexpr int KSEG = 36;  // doubles per staged row segment: 34 cells rounded up to an even start and count
-
-struct ItemIdx { int i, j, w; };
-
-#ifndef CUHARM_FLUXK_TMA_MINB
-#define CUHARM_FLUXK_TMA_MINB 4
-#endif
-
 template <int RECON, int RIEMANN, bool STAGE>
-__global__ void __launch_bounds__(128, CUHARM_FLUXK_TMA_MINB) flux_k_tma_kernel(FluxArgs a, int wpr) {
-  __shared__ __align__(128) double stage_all[4][8][KSEG];
-  __shared__ __align__(8) unsigned long long mbar_all[4];
+__global__ void __launch_bounds__(128, 4) flux_k_row_kernel(FluxArgs a, int wpr) {
+  extern __shared__ __align__(128) double rowbuf[];  // [2][8][n3g]
+  __shared__ __align__(8) unsigned long long mbar2[2];
   const Dims& d = a.d;
   constexpr int HALO = FluxK<RECON>::HALO, FPW = FluxK<RECON>::FPW;
   const unsigned FULL = 0xffffffffu;
-  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  double (*stage)[KSEG] = stage_all[wib];
-  const unsigned bar = smem_u32(&mbar_all[wib]);
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const int rs = d.n3g;
+  const unsigned bar0 = smem_u32(&mbar2[0]);
   const int ni = a.hi1 - a.lo1 + 1, nj = a.hi2 - a.lo2 + 1;
-  const long long nitems = (long long)ni * nj * wpr;
-  const long long W = (long long)gridDim.x * 4;
-  long long item = (long long)blockIdx.x * 4 + wib;
-  // decomposition of the first item and of the stride, then carried increments (no division in the loop)
-  ItemIdx cur, nxt, dlt;
-  {
-    long long r = item / wpr;
-    cur.w = (int)(item % wpr); cur.j = (int)(r % nj); cur.i = (int)(r / nj);
-    r = W / wpr;
-    dlt.w = (int)(W % wpr); dlt.j = (int)(r % nj); dlt.i = (int)(r / nj);
-  }
-  auto advance = [&](const ItemIdx& x) {
-    ItemIdx y{x.i + dlt.i, x.j + dlt.j, x.w + dlt.w};
-    if (y.w >= wpr) { y.w -= wpr; y.j++; }
-    if (y.j >= nj) { y.j -= nj; y.i++; }
-    return y;
-  };
-  // segment start (even, clamped) of an item's chunk
-  auto seg_start = [&](int w) {
-    int cs = a.lo3 + w * FPW - HALO - 1;
-    cs = cs < 0 ? 0 : cs & ~1;
-    return cs;
-  };
-  // lanes 0..7, one variable each: a single thread needs several hundred cycles per bulk copy it issues, eight
-  // lanes issue theirs concurrently
-  auto issue = [&](const ItemIdx& x) {
-    const int cs = seg_start(x.w);
-    const unsigned bytes = (unsigned)min(KSEG, d.n3g - cs) * 8u;
-    const double* src = a.P + (a.lo1 + x.i) * d.s1 + (a.lo2 + x.j) * d.s2 + cs + lane * d.nz;
-    if (lane == 0) mbar_expect_tx(bar, 8u * bytes);
+  const int nrows = ni * nj, G = gridDim.x;
+  int row = blockIdx.x;
+  int ci = row / nj, cj = row % nj;          // carried (i, j) of the current row
+  const int di = G / nj, dj = G % nj;
+  auto issue = [&](int i, int j, int stage) {  // lanes 0..7 of warp 0, one variable each
+    const double* src = a.P + (long long)(a.lo1 + i) * d.s1 + (long long)(a.lo2 + j) * d.s2 + lane * d.nz;
+    const unsigned bar = bar0 + 8 * stage;
+    if (lane == 0) mbar_expect_tx(bar, 8u * rs * 8u);
     __syncwarp(0xffu);
-    bulk_g2s(smem_u32(&stage[lane][0]), src, bytes, bar);
+    bulk_g2s(smem_u32(rowbuf + (stage * 8 + lane) * rs), src, (unsigned)rs * 8u, bar);
   };
-  if (lane == 0) {
-    mbar_init(bar, 1);
+  if (threadIdx.x == 0) {
+    mbar_init(bar0, 1);
+    mbar_init(bar0 + 8, 1);
     mbar_fence_init();
   }
-  __syncwarp();
-  if (lane < 8 && item < nitems) issue(cur);
+  __syncthreads();
+  if (wib == 0 && lane < 8) {
+    if (row < nrows) issue(ci, cj, 0);
+    if (row + G < nrows) {
+      int i2 = ci + di, j2 = cj + dj;
+      if (j2 >= nj) { j2 -= nj; i2++; }
+      issue(i2, j2, 1);
+    }
+  }
   double cwmax = 0.0;
-  for (unsigned n = 0; item < nitems; item += W, n++, cur = nxt) {
-    nxt = advance(cur);
-    const int i = a.lo1 + cur.i, j = a.lo2 + cur.j;
-    const int f0 = a.lo3 + cur.w * FPW;
-    const int c = f0 - HALO + lane;            // this lane's cell = the cell whose lower face is face c
-    const int cc = min(max(c, 1), d.n3g - 2);  // clamped for the reads; clamped lanes never produce output
-    const int o = cc - seg_start(cur.w);
-    mbar_wait(bar, n & 1);
-    double ym1[8], y0[8], y1[8];
+  for (int n = 0; row < nrows; row += G, n++) {
+    const int s = n & 1;
+    const int i = a.lo1 + ci, j = a.lo2 + cj;
+    const double* st = rowbuf + s * 8 * rs;
+    mbar_wait(bar0 + 8 * s, (n >> 1) & 1);
+    for (int w = wib; w < wpr; w += nw) {
+      const int f0 = a.lo3 + w * FPW;
+      const int c = f0 - HALO + lane;            // this lane's cell = the cell whose lower face is face c
+      const int cc = min(max(c, 1), d.n3g - 2);  // clamped for the reads; clamped lanes never produce output
+      double pl[8], pr[8];
 #pragma unroll
-    for (int v = 0; v < 8; v++) { ym1[v] = stage[v][o - 1]; y0[v] = stage[v][o]; y1[v] = stage[v][o + 1]; }
-    __syncwarp();  // all lanes hold their cells: the stage can be refilled
-    if (lane < 8 && item + W < nitems) issue(nxt);
-    double pl[8], pr[8];
-#pragma unroll
-    for (int v = 0; v < 8; v++) {
-      const double s = slope2_mc(y0[v] - ym1[v], y1[v] - y0[v]);
-      double l, r;
-      if (RECON == 0) {
-        plm_faces(y0[v], s, l, r);
-      } else {
-        const double sup = __shfl_down_sync(FULL, s, 1);   // slope of cell c+1 (lane 31: garbage)
-        const double ehi = ppm_edge(y0[v], y1[v], s, sup);
-        const double elo = __shfl_up_sync(FULL, ehi, 1);   // edge value c-1/2 (lane 0: garbage)
-        l = elo;
-        r = ehi;
-        ppm_mono(y0[v], l, r);
+      for (int v = 0; v < 8; v++) {
+        const double ym1 = st[v * rs + cc - 1], y0 = st[v * rs + cc], y1 = st[v * rs + cc + 1];
+        const double sl = slope2_mc(y0 - ym1, y1 - y0);
+        double l, r;
+        if (RECON == 0) {
+          plm_faces(y0, sl, l, r);
+        } else {
+          const double sup = __shfl_down_sync(FULL, sl, 1);   // slope of cell c+1 (lane 31: garbage)
+          const double ehi = ppm_edge(y0, y1, sl, sup);
+          const double elo = __shfl_up_sync(FULL, ehi, 1);    // edge value c-1/2 (lane 0: garbage)
+          l = elo;
+          r = ehi;
+          ppm_mono(y0, l, r);
+        }
+        pl[v] = __shfl_up_sync(FULL, r, 1);  // upper-edge state of cell c-1
+        pr[v] = l;
       }
-      pl[v] = __shfl_up_sync(FULL, r, 1);  // upper-edge state of cell c-1
-      pr[v] = l;
+      const bool ok = lane >= HALO && lane < HALO + FPW && c <= a.hi3;
+      if (ok) {
+        const Geom G3 = load_geom(a.Gf, i * d.n2g + j);
+        double F[8], cwv;
+        face_flux<3, RIEMANN>(pl, pr, G3, a.gam, F, cwv);
+        store_flux<3, STAGE>(a, i * d.s1 + j * d.s2 + c, F, cwv);
+        cwmax = fmax(cwmax, cwv);
+      }
     }
-    const bool ok = lane >= HALO && lane < HALO + FPW && c <= a.hi3;
-    if (ok) {
-      const Geom G = load_geom(a.Gf, i * d.n2g + j);
-      double F[8], cwv;
-      face_flux<3, RIEMANN>(pl, pr, G, a.gam, F, cwv);
-      store_flux<3, STAGE>(a, i * d.s1 + j * d.s2 + c, F, cwv);
-      cwmax = fmax(cwmax, cwv);
+    // advance the carried row index by 2G for the refill, by G for the next iteration
+    int i1 = ci + di, j1 = cj + dj;
+    if (j1 >= nj) { j1 -= nj; i1++; }
+    __syncthreads();  // every warp is done with stage s
+    if (wib == 0 && lane < 8 && row + 2 * G < nrows) {
+      int i2 = i1 + di, j2 = j1 + dj;
+      if (j2 >= nj) { j2 -= nj; i2++; }
+      issue(i2, j2, s);
     }
+    ci = i1;
+    cj = j1;
   }
   atomic_max_nonneg(a.cwmax, cwmax);
 }
