@@ -89,6 +89,19 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def aggregate(ms_local, zones, steps, world, dist=None, device="cpu"):
+    """Whole-job throughput of `world` independent replicas (the path does not shard in this build):
+    max over ranks of the device-timed region, value = world x zones x steps / that time.  No data-path collective;
+    this all-reduce of one scalar is the only exchange."""
+    ms = float(ms_local)
+    if dist is not None and world > 1:
+        import torch
+        t = torch.tensor([ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return ms, world * zones * steps / (ms * 1e-3)
+
+
 def make_workload(name, **kw):
     from workloads import config
     from workloads.params import TORUS
@@ -210,11 +223,7 @@ def run_ours(args):
         timing = s.get_timing()
         s.set_timing(False)
         s.use_graph(True)
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * zones * args.steps / (ms * 1e-3)
+    ms, value = aggregate(ms, zones, args.steps, world, dist, "cuda")
     divb = s.divb()[1]
     stats = s.stats()
 
@@ -231,11 +240,7 @@ def run_ours(args):
     e1.record()
     barrier()
     ms_e2e = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
-    e2e_val = world * zones * e2e_steps / (ms_e2e * 1e-3)
+    ms_e2e, e2e_val = aggregate(ms_e2e, zones, e2e_steps, world, dist, "cuda")
     nbytes = prim_pinned.numel() * 8
 
     if rank == 0:
