@@ -60,7 +60,7 @@ struct cuharm_ctx {
   int64_t t_n[CUHARM_NCLASS] = {0};
   // graph
   bool upd_tma = false;  // update_tma_kernel usable (shared-memory opt-in succeeded)
-  int upd_blocks = 0;    // its persistent grid size
+  int upd_blocks = 0, upd_blocks64 = 0;  // its persistent grid sizes (128- and 64-zone tiles)
   int sms = 148;         // multiprocessors of the device
   bool fluxk_row = true; // prefer the whole-row pipeline (flux_k_row_kernel)
   bool use_graph = false;
@@ -250,17 +250,24 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
               nfail, h->cnt + CNT_STATS, dtau, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], h->p.gam,
               newton_cfg(h->p), floor_cfg(h->p)};
     dim3 grid((d.n3 + 127) / 128, d.n2, d.n1);
-    const size_t smem = UPD_SMEM;
     if (tma) {
-      const int nch = (d.n3 + 127) / 128;
+      const int tb = d.n3 <= 64 ? 64 : 128;
+      const size_t smem = upd_smem(tb);
+      const int nch = (d.n3 + tb - 1) / tb;
       const long long nt = (long long)d.n1 * d.n2 * nch;
       const int ntiles = (int)nt;
-      const int nb = (int)std::min<long long>(nt, h->upd_blocks);
+      const int nb = (int)std::min<long long>(nt, tb == 64 ? h->upd_blocks64 : h->upd_blocks);
       int wj = 1;  // strip width: the largest divisor of n2 not above CUHARM_UPD_STRIP
       for (int w = 1; w <= CUHARM_UPD_STRIP && w <= d.n2; w++)
         if (d.n2 % w == 0) wj = w;
-      if (Pflux == Pbase) update_tma_kernel<true><<<nb, 128, smem, h->stream>>>(a, ntiles, nch, wj);
-      else update_tma_kernel<false><<<nb, 128, smem, h->stream>>>(a, ntiles, nch, wj);
+      const bool same = Pflux == Pbase;
+      if (tb == 64) {
+        if (same) update_tma_kernel<true, 64><<<nb, 64, smem, h->stream>>>(a, ntiles, nch, wj);
+        else update_tma_kernel<false, 64><<<nb, 64, smem, h->stream>>>(a, ntiles, nch, wj);
+      } else {
+        if (same) update_tma_kernel<true, 128><<<nb, 128, smem, h->stream>>>(a, ntiles, nch, wj);
+        else update_tma_kernel<false, 128><<<nb, 128, smem, h->stream>>>(a, ntiles, nch, wj);
+      }
     } else {
       if (Pflux == Pbase) update_kernel<true><<<grid, 128, 0, h->stream>>>(a);
       else update_kernel<false><<<grid, 128, 0, h->stream>>>(a);
@@ -340,18 +347,19 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
     for (int c = 0; c < 3; c++) { h->x0[c] = p->xmin[c]; h->dx[c] = (p->xmax[c] - p->xmin[c]) / n[c]; }
   }
   {  // opt in to the dynamic shared memory of the bulk-copy update kernel (67.5 KB per block)
-    const int smem = UPD_SMEM;
-    const cudaError_t e1 = cudaFuncSetAttribute(update_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    const cudaError_t e2 = cudaFuncSetAttribute(update_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    h->upd_tma = (e1 == cudaSuccess && e2 == cudaSuccess);
-    if (h->upd_tma) {  // persistent grid: every SM filled with as many blocks as fit
+    auto setup = [&](auto kern_t, auto kern_f, int tb, int& blocks) {
+      const int smem = upd_smem(tb);
       int dev = 0, sms = 0, per = 0;
+      if (cudaFuncSetAttribute(kern_t, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return false;
+      if (cudaFuncSetAttribute(kern_f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return false;
       cudaGetDevice(&dev);
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, update_tma_kernel<false>, 128, smem) != cudaSuccess || per < 1)
-        h->upd_tma = false;
-      h->upd_blocks = sms * per;
-    }
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern_f, tb, smem) != cudaSuccess || per < 1) return false;
+      blocks = sms * per;  // persistent grid: every SM filled with as many blocks as fit
+      return true;
+    };
+    h->upd_tma = setup(update_tma_kernel<true, 128>, update_tma_kernel<false, 128>, 128, h->upd_blocks) &&
+                 setup(update_tma_kernel<true, 64>, update_tma_kernel<false, 64>, 64, h->upd_blocks64);
     if (!h->upd_tma) cudaGetLastError();
     {
       int dev = 0, sms = 0;

@@ -287,20 +287,20 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_MINB) update_kernel(UpdArgs a)
 }
 
 // TMA kernel (n3g even, 16-byte aligned arrays).  The streamed operands of the 128 zones of a block are 63 row
-// segments (55 in the predictor) of UPD_ROW doubles each, contiguous along k: the lanes of warps 0 and 1 issue one
+// segments (55 in the predictor) of TB + 4 doubles each, contiguous along k: the lanes of warps 0 and 1 issue one
 // 1D bulk copy (cp.async.bulk, global -> shared, completion on an mbarrier) per row, so the whole DRAM footprint of
 // the block is in flight at once and holds no registers while it flies.  Every thread then reads its zone (and the
-// k-1, k+1 neighbours) from shared memory.  Segment = zones k0-1 .. k0+UPD_ROW-3 of the row (k0 = first zone of
+// k-1, k+1 neighbours) from shared memory.  Segment = zones k0-1 .. k0+TB+1 of the row (k0 = first zone of
 // the block; the -1 makes the start even, i.e. 16-byte aligned, because ng is odd).
 //
 // Flux-CT is fused in: instead of the three edge-EMF arrays of emf_kernel the block stages the 22 rows of
 // transverse induction fluxes its 12 EMFs per zone are made of and evaluates eq. 21 in place, with the same
 // expression (same operand order) wherever an EMF is needed, so every zone that shares an edge gets the same bits
 // and div B stays at round-off exactly as with the stored EMFs.
-constexpr int UPD_ROW = 132;   // doubles per staged row: 1 + 128 + 1 (k+1) + 2 pad -> 1056 B, a multiple of 16
+__host__ __device__ constexpr int upd_row(int tb) { return tb + 4; }  // doubles per staged row: 1 + TB + 1 (k+1) + 2 pad, a multiple of 16 B
 constexpr int UPD_NROW = 63;   // 8 P^n, 8 P-flux, 10 F1, 10 F2, 5 F3 (hydro), 22 induction-flux rows
 constexpr int UPD_TAB = 62;    // doubles of per-(i,j) records staged behind the rows: Geom 20, connection 40, floors 2
-constexpr int UPD_SMEM = (UPD_NROW * UPD_ROW + 2 * 64) * 8;  // dynamic shared memory per block, bytes
+__host__ __device__ constexpr int upd_smem(int tb) { return (UPD_NROW * upd_row(tb) + 2 * 64) * 8; }  // dynamic shared memory per block
 
 // row r of the stage: which array, which component, which (di, dj) offset of the zone row
 struct UpdRowSrc { signed char arr, comp, di, dj; };  // arr: 0 Pbase, 1 Pflux, 2 F1, 3 F2, 4 F3
@@ -330,8 +330,10 @@ struct TileCnt { int s, i, jj, c; };  // mixed-radix tile counter: j-strip, i, j
 #ifndef CUHARM_UPD_TMA_MINB
 #define CUHARM_UPD_TMA_MINB 3
 #endif
-template <bool SAME>
-__global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(UpdArgs a, int ntiles, int nch, int wj) {
+// TB = zones (threads) per tile: 128, or 64 for short rows (n3 <= 64), which would leave half a 128-zone tile idle.
+template <bool SAME, int TB>
+__global__ void __launch_bounds__(TB, (CUHARM_UPD_TMA_MINB * 128) / TB) update_tma_kernel(UpdArgs a, int ntiles, int nch, int wj) {
+  constexpr int UPD_ROW = upd_row(TB);
   extern __shared__ __align__(128) double rows[];  // [UPD_NROW][UPD_ROW]
   __shared__ __align__(8) unsigned long long mbar;
   const Dims& d = a.d;
@@ -365,16 +367,16 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(Up
   auto to_idx = [&](const TileCnt& x) { return TileIdx{x.i, x.s * wj + x.jj, x.c}; };
   TileIdx cur = to_idx(ccur), nxt;
   auto tile_base = [&](const TileIdx& x) {  // element offset of the first staged zone of the tile's row
-    return (long long)(d.ng + x.i) * d.s1 + (long long)(d.ng + x.j) * d.s2 + (d.ng + x.c * 128 - 1);
+    return (long long)(d.ng + x.i) * d.s1 + (long long)(d.ng + x.j) * d.s2 + (d.ng + x.c * TB - 1);
   };
   auto tile_bytes = [&](const TileIdx& x) {  // staged zones per row (even count) x 8
-    return (unsigned)min(UPD_ROW - 2, d.n3g - (d.ng + x.c * 128 - 1)) * 8u;
+    return (unsigned)min(UPD_ROW - 2, d.n3g - (d.ng + x.c * TB - 1)) * 8u;
   };
-  // Row r is owned by thread 2r (a warp issues its bulk copies one after the other, so the rows are spread over
-  // all four warps): its source pointer for the tile at offset 0, then tile by tile + base.  Thread 127 owns the
+  // Row r is owned by thread 2r (r for 64-thread blocks; a warp issues its bulk copies one after the other, so the rows are spread over
+  // all four warps): its source pointer for the tile at offset 0, then tile by tile + base.  The last thread owns the
   // three per-(i,j) records (geometry, connection, floors), which ride along as rows 63..65.
-  const int row = t >> 1;
-  const bool issuer = !(t & 1) && row < UPD_NROW && !(SAME && row >= 8 && row < 16);
+  const int row = TB == 128 ? t >> 1 : t;
+  const bool issuer = (TB == 128 ? !(t & 1) : true) && row < UPD_NROW && !(SAME && row >= 8 && row < 16);
   const double* src0 = nullptr;
   if (issuer) {
     const UpdRowSrc q = upd_row_src(row);
@@ -387,7 +389,7 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(Up
     const unsigned bytes = tile_bytes(x);
     if (t == 0) mbar_expect_tx(bar0, bytes * (SAME ? UPD_NROW - 8 : UPD_NROW) + UPD_TAB * 8u);
     if (issuer) bulk_g2s(dst, src0 + tile_base(x), bytes, bar0);
-    if (t == 127) {
+    if (t == TB - 1) {
       const size_t q = (size_t)(d.ng + x.i) * d.n2g + (d.ng + x.j);
       double* const tb = tab + slot * 64;
       bulk_g2s(smem_u32(tb), a.C + q, 160u, bar0);
@@ -401,7 +403,7 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_TMA_MINB) update_tma_kernel(Up
     ccur = advance_cnt(ccur);
     nxt = to_idx(ccur);
     const int j = d.ng + cur.j, i = d.ng + cur.i;
-    const int k0 = d.ng + cur.c * 128;
+    const int k0 = d.ng + cur.c * TB;
     const bool live = k0 + t < d.ng + d.n3;
     const int tc = live ? t : d.ng + d.n3 - 1 - k0;  // clamped lane position
     const long long idx = i * d.s1 + j * d.s2 + k0 + tc;
