@@ -3,6 +3,7 @@
 // reductions.  fp64, SoA prim[8][n1g][n2g][n3g] with k (phi) fastest: a warp runs along k at fixed (i,j), so
 // every geometry read is a broadcast (the metric is phi-independent).
 #pragma once
+#include <type_traits>
 #include "cuharm_flux.cuh"
 
 namespace cuharm {
@@ -372,24 +373,38 @@ __global__ void __launch_bounds__(TB, (CUHARM_UPD_TMA_MINB * 128) / TB) update_t
   auto tile_bytes = [&](const TileIdx& x) {  // staged zones per row (even count) x 8
     return (unsigned)min(UPD_ROW - 2, d.n3g - (d.ng + x.c * TB - 1)) * 8u;
   };
-  // Row r is owned by thread 2r (r for 64-thread blocks; a warp issues its bulk copies one after the other, so the rows are spread over
-  // all four warps): its source pointer for the tile at offset 0, then tile by tile + base.  The last thread owns the
-  // three per-(i,j) records (geometry, connection, floors), which ride along as rows 63..65.
-  const int row = TB == 128 ? t >> 1 : t;
-  const bool issuer = (TB == 128 ? !(t & 1) : true) && row < UPD_NROW && !(SAME && row >= 8 && row < 16);
-  const double* src0 = nullptr;
-  if (issuer) {
-    const UpdRowSrc q = upd_row_src(row);
-    const double* arr = q.arr == 0 ? a.Pbase : q.arr == 1 ? a.Pflux : q.arr == 2 ? a.F1 : q.arr == 3 ? a.F2 : a.F3;
-    src0 = arr + q.comp * d.nz + q.di * d.s1 + q.dj * d.s2;
-  }
-  const unsigned dst = smem_u32(rows + row * UPD_ROW);
+  // Every warp issues its share of the tile's copies (rows r = w, w + NWARP, ...) with warp-uniform operands: the
+  // row index is unrolled per warp, the addresses come from kernel parameters and the tile indices, so each bulk
+  // copy is a handful of uniform-datapath instructions; per-lane operands would make the compiler serialise the
+  // lanes in an elect loop that waits on the previous copy.
+  constexpr int NWARP = TB / 32;
   double* const tab = rows + UPD_NROW * UPD_ROW;  // two slots of [20] geometry record, [40] connection, [2] floors
-  auto issue = [&](const TileIdx& x, int slot) {
+  auto issue_rows = [&](auto wtag, unsigned bytes, long long base) {
+    constexpr int W = decltype(wtag)::value;
+#pragma unroll
+    for (int r = W; r < UPD_NROW; r += NWARP) {
+      if (SAME && r >= 8 && r < 16) continue;
+      const UpdRowSrc q = upd_row_src(r);
+      const double* arr = q.arr == 0 ? a.Pbase : q.arr == 1 ? a.Pflux : q.arr == 2 ? a.F1 : q.arr == 3 ? a.F2 : a.F3;
+      bulk_g2s(smem_u32(rows + r * UPD_ROW), arr + q.comp * d.nz + q.di * d.s1 + q.dj * d.s2 + base, bytes, bar0);
+    }
+  };
+  auto issue = [&](const TileIdx& x, int slot) {  // all warps; lane 0 of each issues
+    if ((t & 31) != 0) return;
     const unsigned bytes = tile_bytes(x);
-    if (t == 0) mbar_expect_tx(bar0, bytes * (SAME ? UPD_NROW - 8 : UPD_NROW) + UPD_TAB * 8u);
-    if (issuer) bulk_g2s(dst, src0 + tile_base(x), bytes, bar0);
-    if (t == TB - 1) {
+    const long long base = tile_base(x);
+    const int w = t >> 5;
+    if (w == 0) {
+      mbar_expect_tx(bar0, bytes * (SAME ? UPD_NROW - 8 : UPD_NROW) + UPD_TAB * 8u);
+      issue_rows(std::integral_constant<int, 0>{}, bytes, base);
+    } else if (w == 1) {
+      issue_rows(std::integral_constant<int, 1>{}, bytes, base);
+    } else if (NWARP > 2 && w == 2) {
+      issue_rows(std::integral_constant<int, 2 % NWARP>{}, bytes, base);
+    } else if (NWARP > 2) {
+      issue_rows(std::integral_constant<int, 3 % NWARP>{}, bytes, base);
+    }
+    if (w == NWARP - 1) {
       const size_t q = (size_t)(d.ng + x.i) * d.n2g + (d.ng + x.j);
       double* const tb = tab + slot * 64;
       bulk_g2s(smem_u32(tb), a.C + q, 160u, bar0);

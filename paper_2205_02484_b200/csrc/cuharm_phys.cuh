@@ -542,7 +542,15 @@ __device__ __forceinline__ int apply_floors(double q[8], const Geom& G, const Ge
     double drho = 0.0, du = 0.0;
     if (fc.sigma_max > 0.0) drho = fmax(0.0, fma(bsq, fc.isigma, -q[0]));
     if (fc.b2_over_u_max > 0.0) du = fmax(0.0, fma(bsq, fc.ib2u, -q[1]));
-    if (drho > 0.0 || du > 0.0) mask |= apply_ceilings_cold(q, Gp, drho, du, fc, gam, nc);
+    if (drho > 0.0 || du > 0.0) {
+      // the out-of-line rare path works on a copy, so that only the copy's address escapes and q stays in registers
+      double t[8];
+#pragma unroll
+      for (int v = 0; v < 8; v++) t[v] = q[v];
+      mask |= apply_ceilings_cold(t, Gp, drho, du, fc, gam, nc);
+#pragma unroll
+      for (int v = 0; v < 8; v++) q[v] = t[v];
+    }
   }
   if (fc.gamma_max > 0.0) {
     const double q2 = (mask & 4) ? gamma_sq_minus_one(q, G) : qsq;
