@@ -183,7 +183,9 @@ __device__ __forceinline__ void flux_vector(const double q[8], const State& S, c
 // A = (u^t)^2 (1 - c_ms^2) - c_ms^2 g^tt > 0 because g^tt < 0 everywhere in Kerr-Schild coordinates, so the
 // "+" root is the larger one.  A29: a negative discriminant is clamped to zero.
 // ---------------------------------------------------------------------------------------------------------
-template <int DIR>
+// ONLY_MAX: return in cp the larger of (cp, -cm, 0) = (|B/2| + sqrt(disc)) / A, which is all eq. 17 needs (the same
+// floating-point value as taking the maximum of the two roots' magnitudes); cm is then not set.
+template <int DIR, bool ONLY_MAX = false>
 __device__ __forceinline__ void wave_speeds(const double q[8], const State& S, const Geom& G, double gam, double& cp,
                                             double& cm) {
   // c_ms^2 = N / D with N = b^2 + gam p, D = b^2 + w (eqs. 18-19).  The quadratic is homogeneous in its
@@ -202,8 +204,12 @@ __device__ __forceinline__ void wave_speeds(const double q[8], const State& S, c
   disc = disc > 1e-300 ? disc : 1e-300;
   const double sq = disc * frsqrt(disc);
   const double iA = frcp(A);
-  cp = (hB + sq) * iA;
-  cm = (hB - sq) * iA;
+  if (ONLY_MAX) {
+    cp = (fabs(hB) + sq) * iA;
+  } else {
+    cp = (hB + sq) * iA;
+    cm = (hB - sq) * iA;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -292,14 +298,19 @@ template <int DIR, int RIEMANN>
 __device__ __forceinline__ void face_flux(const double pl[8], const double pr[8], const Geom& G, double gam, double F[8],
                                           double& cw) {
   State Sl, Sr;
-  double Hl[8], Hr[8], cpl, cml, cpr, cmr;
+  double Hl[8], Hr[8], cpl, cml = 0.0, cpr, cmr = 0.0;
   fluid_state(pl, G, Sl);
   fluid_state(pr, G, Sr);
-  wave_speeds<DIR>(pl, Sl, G, gam, cpl, cml);
-  wave_speeds<DIR>(pr, Sr, G, gam, cpr, cmr);
-  const double cmax = fmax(0.0, fmax(cpr, cpl));
-  const double cmin = fmax(0.0, fmax(-cmr, -cml));
-  cw = fmax(cmax, cmin);
+  wave_speeds<DIR, RIEMANN == 0>(pl, Sl, G, gam, cpl, cml);
+  wave_speeds<DIR, RIEMANN == 0>(pr, Sr, G, gam, cpr, cmr);
+  double cmax = 0.0, cmin = 0.0;
+  if (RIEMANN == 0) {
+    cw = fmax(cpl, cpr);  // = max(c_max, c_min) of P:L154: each side's bound is already max(c_1, -c_2) >= 0
+  } else {
+    cmax = fmax(0.0, fmax(cpr, cpl));
+    cmin = fmax(0.0, fmax(-cmr, -cml));
+    cw = fmax(cmax, cmin);
+  }
   if (RIEMANN == 0) {
     // eq. 17: (F^l + F^r - c_w (U^r - U^l))/2 = ((F^l + c_w U^l) + (F^r - c_w U^r))/2
     side_flux<DIR>(pl, Sl, gam, cw, Hl);
@@ -335,6 +346,7 @@ __device__ __forceinline__ void load_conn(const double* __restrict__ conn, doubl
   for (int s = 0; s < 20; s++) { const double2 v = __ldg(c2 + s); cn[2 * s] = v.x; cn[2 * s + 1] = v.y; }
 }
 
+template <bool KILLING = true>
 __device__ __forceinline__ void source_term(const double q[8], const State& S, const Geom& G, const double* cn,
                                             double gam, double src[4]) {
   const double pg = (gam - 1.0) * q[1];
@@ -343,6 +355,9 @@ __device__ __forceinline__ void source_term(const double q[8], const State& S, c
   const double ptot = fma(0.5, S.bsq, pg);
   const double uc[4] = {S.u0, S.u1, S.u2, S.u3}, ul[4] = {S.l0, S.l1, S.l2, S.l3};
   const double bc[4] = {S.b0, S.b1, S.b2, S.b3}, bl[4] = {S.m0, S.m1, S.m2, S.m3};
+  // nu = t and nu = phi: T^k_l Gamma^l_{nu k} = (1/2) T^{kl} d_nu g_kl vanishes identically because the metric
+  // depends on neither t nor phi (energy and angular-momentum conservation); the contraction would return its own
+  // round-off, so the two sums are not formed (KILLING = true).  Minkowski: Gamma = 0 altogether.
   double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
 #pragma unroll
   for (int k = 0; k < 4; k++) {
@@ -350,10 +365,10 @@ __device__ __forceinline__ void source_term(const double q[8], const State& S, c
 #pragma unroll
     for (int l = 0; l < 4; l++) {
       const double T = fma(eu, ul[l], -bc[k] * bl[l]) + (k == l ? ptot : 0.0);  // T^k_l
-      s0 = fma(T, cn[l * 10 + pair_index(0, k)], s0);
+      if (!KILLING) s0 = fma(T, cn[l * 10 + pair_index(0, k)], s0);
       s1 = fma(T, cn[l * 10 + pair_index(1, k)], s1);
       s2 = fma(T, cn[l * 10 + pair_index(2, k)], s2);
-      s3 = fma(T, cn[l * 10 + pair_index(3, k)], s3);
+      if (!KILLING) s3 = fma(T, cn[l * 10 + pair_index(3, k)], s3);
     }
   }
   src[0] = G.sg * s0; src[1] = G.sg * s1; src[2] = G.sg * s2; src[3] = G.sg * s3;
