@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(Flux
           const double y2 = pre[v];
           const double d2 = y2 - yn[v];
           const double s1 = slope2_mc(dn[v], d2);            // cell f+1
-          const double ehi = ppm_edge(yc[v], yn[v], sc[v], s1);  // edge f+1/2
+          const double ehi = ppm_edge_d(yc[v], dn[v], sc[v], s1);  // edge f+1/2
           double l = elo[v], r = ehi;
           ppm_mono(yc[v], l, r);
           pl[v] = rprev[v];
@@ -270,13 +270,14 @@ __global__ void __launch_bounds__(128, CUHARM_FLUXK_MINB) flux_k_kernel(FluxArgs
   for (int v = 0; v < 8; v++) {
     const double* yv = y + v * nz;
     const double ym1 = yv[-1], y0 = yv[0], y1 = yv[1];
-    const double s = slope2_mc(y0 - ym1, y1 - y0);
+    const double dp = y1 - y0;
+    const double s = slope2_mc(y0 - ym1, dp);
     double l, r;
     if (RECON == 0) {
       plm_faces(y0, s, l, r);
     } else {
       const double sup = __shfl_down_sync(FULL, s, 1);   // slope of cell c+1 (lane 31: garbage)
-      const double ehi = ppm_edge(y0, y1, s, sup);
+      const double ehi = ppm_edge_d(y0, dp, s, sup);
       const double elo = __shfl_up_sync(FULL, ehi, 1);   // edge value c-1/2 (lane 0: garbage)
       l = elo;
       r = ehi;
@@ -354,13 +355,14 @@ __global__ void __launch_bounds__(128, 4) flux_k_row_kernel(FluxArgs a, int wpr)
 #pragma unroll
       for (int v = 0; v < 8; v++) {
         const double ym1 = st[v * rs + cc - 1], y0 = st[v * rs + cc], y1 = st[v * rs + cc + 1];
-        const double sl = slope2_mc(y0 - ym1, y1 - y0);
+        const double dp = y1 - y0;
+        const double sl = slope2_mc(y0 - ym1, dp);
         double l, r;
         if (RECON == 0) {
           plm_faces(y0, sl, l, r);
         } else {
           const double sup = __shfl_down_sync(FULL, sl, 1);   // slope of cell c+1 (lane 31: garbage)
-          const double ehi = ppm_edge(y0, y1, sl, sup);
+          const double ehi = ppm_edge_d(y0, dp, sl, sup);
           const double elo = __shfl_up_sync(FULL, ehi, 1);    // edge value c-1/2 (lane 0: garbage)
           l = elo;
           r = ehi;
