@@ -102,8 +102,16 @@ __device__ __forceinline__ void store_flux(const FluxArgs& a, long long idx, con
 // the doubled MC slope sc of cell f, the unlimited edge value elo at f-1/2, the limited upper-edge state rprev of
 // cell f-1, and `pre` = y_{f+2}, loaded one iteration ahead so that its DRAM latency hides behind a whole face.
 // ---------------------------------------------------------------------------------------------------------
+// software prefetch distance (faces beyond the register look-ahead) per marching direction; measured on B200 at
+// 256^3: along X1 (plane stride) 2 faces is best, along X2 (row stride) 1 face
+#ifndef CUHARM_MARCH_PF1
+#define CUHARM_MARCH_PF1 2
+#endif
+#ifndef CUHARM_MARCH_PF2
+#define CUHARM_MARCH_PF2 1
+#endif
 #ifndef CUHARM_MARCH_PF
-#define CUHARM_MARCH_PF 1   // software prefetch distance (faces beyond the register look-ahead); 0 = off
+#define CUHARM_MARCH_PF 1   // 0 = no software prefetch at all
 #endif
 #ifndef CUHARM_PF_LEVEL
 #define CUHARM_PF_LEVEL 1
@@ -182,7 +190,8 @@ __global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(Flux
       const long long ahead = (f + 3 < nd ? 3 : 2) * sd;
 #if CUHARM_MARCH_PF
       {
-        const long long far = (f + 3 + CUHARM_MARCH_PF < nd ? 3 + CUHARM_MARCH_PF : 2) * sd;
+        constexpr int PFD = DIR == 1 ? CUHARM_MARCH_PF1 : CUHARM_MARCH_PF2;
+        const long long far = (f + 3 + PFD < nd ? 3 + PFD : 2) * sd;
 #pragma unroll
         for (int v = 0; v < 8; v++) prefetch_l1(y + v * nz + far);
         prefetch_l1(reinterpret_cast<const char*>(a.Gf + gq + gstep));
