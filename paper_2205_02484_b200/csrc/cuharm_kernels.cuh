@@ -169,12 +169,8 @@ struct UpdArgs {
 // Per-zone work once the streamed operands are in registers.  pb = P^n, pf = the state the fluxes were built from
 // (pf is pb in the predictor), fx[6v..6v+5] = F1[i+1], F1[i], F2[j+1], F2[j], F3[k+1], F3[k] of hydro component v,
 // ex = E1 at (0, +j, +k, +j+k), E2 at (0, +i, +k, +i+k), E3 at (0, +i, +j, +i+j).
-template <bool SAME>
-__device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8], const double pf[8], const double fx[30],
-                                            const double ex[12], const Geom& G, const double* cn, double rfl, double ufl,
-                                            long long idx, int q2, bool live, int cnt[5]) {
-  const Dims& d = a.d;
-  double dU[8];  // -div F (eq. 25)
+// -div F of one zone (eq. 25) from its face fluxes and edge EMFs (eq. 22; A3)
+__device__ __forceinline__ void zone_divergence(const UpdArgs& a, const double fx[30], const double ex[12], double dU[8]) {
 #pragma unroll
   for (int v = 0; v < 5; v++)
     dU[v] = -fma(fx[6 * v] - fx[6 * v + 1], a.idx1,
@@ -197,6 +193,13 @@ __device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8]
     dU[6] = -divB2;
     dU[7] = -divB3;
   }
+}
+
+template <bool SAME>
+__device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8], const double pf[8], const double dU[8],
+                                            const Geom& G, const double* cn, double rfl, double ufl,
+                                            long long idx, int q2, bool live, int cnt[5]) {
+  const Dims& d = a.d;
   // U^n, source, update
   State S;
   fluid_state(pb, G, S);
@@ -283,7 +286,9 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_MINB) update_kernel(UpdArgs a)
   double cn[40];
   load_conn(a.conn + (size_t)q2 * 40, cn);
   int cnt[5] = {0, 0, 0, 0, 0};
-  update_zone<SAME>(a, pb, pf, fx, ex, G, cn, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), idx, q2, live, cnt);
+  double dU[8];
+  zone_divergence(a, fx, ex, dU);
+  update_zone<SAME>(a, pb, pf, dU, G, cn, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), idx, q2, live, cnt);
   update_stats(a, cnt);
 }
 
@@ -336,13 +341,14 @@ template <bool SAME, int TB>
 __global__ void __launch_bounds__(TB, (CUHARM_UPD_TMA_MINB * 128) / TB) update_tma_kernel(UpdArgs a, int ntiles, int nch, int wj) {
   constexpr int UPD_ROW = upd_row(TB);
   extern __shared__ __align__(128) double rows[];  // [UPD_NROW][UPD_ROW]
-  __shared__ __align__(8) unsigned long long mbar;
+  __shared__ __align__(8) unsigned long long mbar[2];  // [0] copies landed (tx count), [1] stage released (TB arrivals)
   const Dims& d = a.d;
   const int t = threadIdx.x;
   const int G = gridDim.x;
-  const unsigned bar0 = smem_u32(&mbar);
+  const unsigned bar0 = smem_u32(&mbar[0]);
   if (t == 0) {
     mbar_init(bar0, 1);
+    mbar_init(bar0 + 8, TB);
     mbar_fence_init();
   }
   __syncthreads();
@@ -454,13 +460,18 @@ __global__ void __launch_bounds__(TB, (CUHARM_UPD_TMA_MINB * 128) / TB) update_t
     ex[10] = 0.25 * (ROWZ(53, 0) + ROWZ(52, 0) - ROWZ(61, 0) - ROWZ(60, 0));  // E3(i, j+1)
     ex[11] = 0.25 * (ROWZ(56, 0) + ROWZ(55, 0) - ROWZ(62, 0) - ROWZ(61, 0));  // E3(i+1, j+1)
 #undef ROWZ
-    __syncthreads();  // every thread holds its operands: the stage can be refilled
+    // Every thread now holds its operands: once all have arrived the stage can be refilled.  The barrier is split
+    // (arrive here, wait after the divergence arithmetic), so nobody idles while the last warp finishes its reads.
+    mbar_arrive(bar0 + 8);
+    double dU[8];
+    zone_divergence(a, fx, ex, dU);
+    mbar_wait(bar0 + 8, n & 1);
     if (tile + G < ntiles) issue(nxt, (n + 1) & 1);
     int cnt[5] = {0, 0, 0, 0, 0};
     // the per-(i,j) records of this tile stay valid in their own (double-buffered) slot for the whole tile
     const double* tb = tab + (n & 1) * 64;
     const Geom Gc = load_geom_shared(tb);
-    update_zone<SAME>(a, pb, pf, fx, ex, Gc, tb + 20, tb[60], tb[61], idx, q2, live, cnt);
+    update_zone<SAME>(a, pb, pf, dU, Gc, tb + 20, tb[60], tb[61], idx, q2, live, cnt);
 #pragma unroll
     for (int q = 0; q < 5; q++) cnt_acc[q] += cnt[q];
   }
