@@ -196,8 +196,21 @@ void launch_flux_t(cuharm_ctx* h, FluxArgs& a, int dir) {
     const int nf = dir == 1 ? ni : nj;
     a.seg = march_seg(cols, nf, h->sms);
     const dim3 grid((unsigned)((cols + 127) / 128), (unsigned)((nf + a.seg - 1) / a.seg));
-    if (dir == 1) flux_march_kernel<1, RECON, RIEMANN, STAGE><<<grid, 128, 0, h->stream>>>(a);
-    else flux_march_kernel<2, RECON, RIEMANN, STAGE><<<grid, 128, 0, h->stream>>>(a);
+    // face geometry staged per block: (rows a block's 128 columns can touch) x (faces per segment) records
+    const int nt = dir == 1 ? nj : ni;
+    a.geo_rows = std::min(nt, 127 / nk + 2);
+    size_t gsm = (size_t)a.geo_rows * a.seg * sizeof(Geom);
+#ifdef CUHARM_NO_GEO_STAGE
+    gsm = 1 << 30;
+#endif
+    if (gsm > 40 * 1024) { a.geo_rows = 0; gsm = 0; }
+    if (a.geo_rows > 0) {
+      if (dir == 1) flux_march_kernel<1, RECON, RIEMANN, STAGE, true><<<grid, 128, gsm, h->stream>>>(a);
+      else flux_march_kernel<2, RECON, RIEMANN, STAGE, true><<<grid, 128, gsm, h->stream>>>(a);
+    } else {
+      if (dir == 1) flux_march_kernel<1, RECON, RIEMANN, STAGE, false><<<grid, 128, 0, h->stream>>>(a);
+      else flux_march_kernel<2, RECON, RIEMANN, STAGE, false><<<grid, 128, 0, h->stream>>>(a);
+    }
   }
 }
 
@@ -213,7 +226,7 @@ int launch_flux(cuharm_ctx* h, const double* P, int dir, double* F, double* cw, 
   }
   Timed t_(h, CUHARM_K_FLUX1 + dir - 1);
   FluxArgs a{d, P, dir == 1 ? h->gF1 : (dir == 2 ? h->gF2 : h->gC), F, cw, cwmax, h->p.gam,
-             lo[0], lo[1], lo[2], hi[0], hi[1], hi[2], 0};
+             lo[0], lo[1], lo[2], hi[0], hi[1], hi[2], 0, 0};
   const int rc = h->p.recon, rm = h->p.riemann;
   if (rc == 0 && rm == 0) launch_flux_t<0, 0, STAGE>(h, a, dir);
   else if (rc == 0 && rm == 1) launch_flux_t<0, 1, STAGE>(h, a, dir);

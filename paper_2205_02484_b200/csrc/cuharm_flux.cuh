@@ -82,6 +82,8 @@ struct FluxArgs {
   double gam;
   int lo1, lo2, lo3, hi1, hi2, hi3;  // inclusive face ranges in i, j, k
   int seg;                           // marching kernels: faces per segment (blockIdx.y = segment)
+  int geo_rows;                      // marching kernels: transverse rows whose face geometry a block stages in
+                                     // shared memory (0: read it from global memory face by face)
 };
 
 template <int DIR, bool STAGE>
@@ -134,7 +136,7 @@ __device__ __forceinline__ void prefetch_l1(const void* p) {
 #define CUHARM_MARCH_MINB 2
 #endif
 
-template <int DIR, int RECON, int RIEMANN, bool STAGE>
+template <int DIR, int RECON, int RIEMANN, bool STAGE, bool GEO>
 __global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(FluxArgs a) {
   static_assert(DIR == 1 || DIR == 2, "marching kernel: directions 1 and 2");
   const Dims& d = a.d;
@@ -142,6 +144,23 @@ __global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(Flux
   const int nt = DIR == 1 ? (a.hi2 - a.lo2 + 1) : (a.hi1 - a.lo1 + 1);
   const int q = blockIdx.x * 128 + threadIdx.x;
   double cwv = 0.0;
+  // The face geometry the block will need -- the records of (faces of its segment) x (the transverse rows its 128
+  // columns touch) -- is staged in shared memory once, so the march reads it with shared-memory latency.
+  extern __shared__ __align__(16) double2 geo[];  // [face in segment][row][10]
+  const int t_first = (DIR == 1 ? a.lo2 : a.lo1) + (blockIdx.x * 128) / nk;
+  if (GEO) {
+    const int f0 = (DIR == 1 ? a.lo1 : a.lo2) + blockIdx.y * a.seg;
+    const int f1 = min(f0 + a.seg, (DIR == 1 ? a.hi1 : a.hi2) + 1);
+    const int t_max = DIR == 1 ? a.hi2 : a.hi1;
+    const int nrec = (f1 - f0) * a.geo_rows;
+    for (int e = threadIdx.x; e < nrec * 10; e += 128) {
+      const int rec = e / 10, w = e - rec * 10;
+      const int f = f0 + rec / a.geo_rows, tt = min(t_first + rec % a.geo_rows, t_max);
+      const int g = DIR == 1 ? f * d.n2g + tt : tt * d.n2g + f;
+      geo[e] = __ldg(reinterpret_cast<const double2*>(a.Gf + g) + w);
+    }
+    __syncthreads();
+  }
   if (q < nt * nk) {
     const int t = (DIR == 1 ? a.lo2 : a.lo1) + q / nk;
     const int k = a.lo3 + q % nk;
@@ -197,8 +216,10 @@ __global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(Flux
         const long long far = (f + 3 + PFD < nd ? 3 + PFD : 2) * sd;
 #pragma unroll
         for (int v = 0; v < 8; v++) prefetch_l1(y + v * nz + far);
-        prefetch_l1(reinterpret_cast<const char*>(a.Gf + gq + gstep));
-        prefetch_l1(reinterpret_cast<const char*>(a.Gf + gq + gstep) + 128);
+        if (!GEO) {
+          prefetch_l1(reinterpret_cast<const char*>(a.Gf + gq + gstep));
+          prefetch_l1(reinterpret_cast<const char*>(a.Gf + gq + gstep) + 128);
+        }
       }
 #endif
 #pragma unroll
@@ -233,7 +254,8 @@ __global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(Flux
         }
         pre[v] = nxt;
       }
-      const Geom G = load_geom(a.Gf, gq);
+      const Geom G = GEO ? load_geom_shared(reinterpret_cast<const double*>(geo + ((f - fa) * a.geo_rows + (t - t_first)) * 10))
+                         : load_geom(a.Gf, gq);
       double F[8], c;
       face_flux<DIR, RIEMANN>(pl, pr, G, a.gam, F, c);
       cwv = fmax(cwv, c);
