@@ -66,6 +66,8 @@ struct cuharm_ctx {
   bool use_graph = false;
   cudaGraphExec_t gexec = nullptr;
   cudaStream_t cap_stream = nullptr;
+  cudaStream_t side[2] = {nullptr, nullptr};  // branches of the recorded graph (flux kernels of directions 2, 3)
+  cudaEvent_t fj[3] = {nullptr, nullptr, nullptr};  // fork / join events of those branches
   double graph_dt = 0.0;
   int64_t graph_nodes = 0;
 };
@@ -241,9 +243,38 @@ int launch_flux(cuharm_ctx* h, const double* P, int dir, double* F, double* cw, 
 int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pout, double dtau, int which) {
   const Dims& d = h->d;
   unsigned long long* cwmax = h->cnt + (which == 0 ? CNT_CWPRED : CNT_CWSCR);
-  for (int dir = 1; dir <= 3; dir++) {
-    int rc = launch_flux<false>(h, Pflux, dir, h->F[dir - 1], nullptr, cwmax + (dir - 1));
+  // The three flux kernels are independent of one another.  While a graph is being recorded they go on three
+  // branches (fork / join through events), so that the drain of one overlaps the ramp-up of the next; launched
+  // directly they stay in stream order (that is also the mode in which per-kernel events time them).
+  bool fork = false;
+#ifndef CUHARM_NO_FORK
+  if (h->capturing) {
+    fork = true;
+    for (int s = 0; s < 2 && fork; s++)
+      if (!h->side[s] && cudaStreamCreateWithFlags(&h->side[s], cudaStreamNonBlocking) != cudaSuccess) fork = false;
+    for (int e = 0; e < 3 && fork; e++)
+      if (!h->fj[e] && cudaEventCreateWithFlags(&h->fj[e], cudaEventDisableTiming) != cudaSuccess) fork = false;
+    if (!fork) cudaGetLastError();
+  }
+#endif
+  if (fork) {
+    cudaStream_t main_s = h->stream;
+    CK(cudaEventRecord(h->fj[0], main_s));
+    int rc = launch_flux<false>(h, Pflux, 1, h->F[0], nullptr, cwmax + 0);
+    for (int s = 0; s < 2 && !rc; s++) {
+      CK(cudaStreamWaitEvent(h->side[s], h->fj[0], 0));
+      h->stream = h->side[s];
+      rc = launch_flux<false>(h, Pflux, 2 + s, h->F[1 + s], nullptr, cwmax + 1 + s);
+      h->stream = main_s;
+      CK(cudaEventRecord(h->fj[1 + s], h->side[s]));
+      CK(cudaStreamWaitEvent(main_s, h->fj[1 + s], 0));
+    }
     if (rc) return rc;
+  } else {
+    for (int dir = 1; dir <= 3; dir++) {
+      int rc = launch_flux<false>(h, Pflux, dir, h->F[dir - 1], nullptr, cwmax + (dir - 1));
+      if (rc) return rc;
+    }
   }
   // bulk-copy (TMA) staging of the update kernel needs 16-byte aligned row segments: even n3g, aligned arrays.
   // That kernel evaluates the edge EMFs itself (flux-CT fused); otherwise they go through emf_kernel and h->E.
@@ -629,6 +660,8 @@ int cuharm_destroy(cuharm_handle h) {
   if (!h) return CUHARM_EINVAL;
   if (h->gexec) cudaGraphExecDestroy(h->gexec);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  for (int k = 0; k < 2; k++) if (h->side[k]) cudaStreamDestroy(h->side[k]);
+  for (int k = 0; k < 3; k++) if (h->fj[k]) cudaEventDestroy(h->fj[k]);
   for (auto& e : h->ev) cudaEventDestroy(e);
   delete h;
   return CUHARM_OK;
