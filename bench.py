@@ -29,13 +29,13 @@ B_ALG = 1218.0          # algorithmic bytes per zone-cycle (DESIGN.
 # emf: read 6 B-fluxes 48, write 3 EMFs 24; update: P^n 64 + hydro fluxes 120 + EMFs 24 (+ P-half 64 in the
 # corrector, averaged: +32) in, 64 + 4 (flag) out
 KERNEL_BYTES = {"flux1": 120.0, "flux2": 120.0, "flux3": 120.0, "emf": 72.0, "update": 332.0}
-# From the ncu --set full capture of this command at C4 (profiles/r1c_ncu_summary.md), per launch and averaged over
+# From the ncu --set full capture of this command at C4 (profiles/r1d_ncu_summary.md), per launch and averaged over
 # the predictor and corrector launches: DRAM bytes read + written, and fp64 (DFMA/DMUL/DADD/DSETP) warp
 # instructions executed.  Only quoted for the workload they were captured on.
-NCU_C4 = {"update": {"traffic": 6.68e9, "fp64_warp_inst": 3.63e8},
-          "flux1": {"traffic": 2.19e9, "fp64_warp_inst": 1.84e8},
-          "flux2": {"traffic": 2.19e9, "fp64_warp_inst": 1.84e8},
-          "flux3": {"traffic": 2.08e9, "fp64_warp_inst": 2.07e8}}
+NCU_C4 = {"update": {"traffic": 6.18e9, "fp64_warp_inst": 3.50e8},
+          "flux1": {"traffic": 2.20e9, "fp64_warp_inst": 1.75e8},
+          "flux2": {"traffic": 2.19e9, "fp64_warp_inst": 1.75e8},
+          "flux3": {"traffic": 2.08e9, "fp64_warp_inst": 1.97e8}}
 # fp64 pipe: 16 lanes per SM sub-partition = one warp instruction per 2 cycles per sub-partition
 FP64_WARP_INST_PER_S = 148 * 4 * 1.965e9 / 2.0
 
@@ -261,7 +261,7 @@ def run_ours(args):
                 roof_alu = {"bound": "alu", "kernel": dom, "achieved": a_alu, "peak": FP64_WARP_INST_PER_S,
                             "unit": "fp64 warp-instructions/s", "frac": a_alu / FP64_WARP_INST_PER_S,
                             "peak_source": "148 SMs x 4 sub-partitions x 1.965 GHz / 2 cycles per fp64 warp instruction",
-                            "count_source": "ncu, profiles/r1c_ncu_summary.md"}
+                            "count_source": "ncu, profiles/r1d_ncu_summary.md"}
             roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                     "frac": achieved / peak, "traffic": ncu["traffic"] if ncu else None, "peak_source": peak_src,
                     "kernel_ms_per_launch": per_launch_ms, "kernel_time_shares": shares,
