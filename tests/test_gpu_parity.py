@@ -282,6 +282,39 @@ def test_failed_zones_are_repaired_like_the_oracle():
     assert (prim_errors(p, got, ref, tol=1e-10) < 1e-10).all(), prim_errors(p, got, ref)
 
 
+# ------------------------------------------------------------------ full size, in the launch configuration bench.py times
+def test_full_size_c4_k_invariant_torus_matches_the_2d_oracle():
+    """BASELINE.json's headline size (C4: 256^3, PPM + LLF) through the same path bench.py times (graph replay, bulk-
+    copy kernels with two 128-zone chunks per row, strip-ordered tiles).  The oracle cannot do 1.7e7 zones in
+    seconds, but a property that holds at any size lets it check EVERY zone: phi-independent input stays phi-
+    independent and equals the run at N3 = 1 (SURVEY 8(c) pin 13 / A31, pinned for the oracle itself in
+    test_oracle_scheme_pins.py).  So the GPU steps the 2D perturbed, magnetised torus replicated along phi at
+    256^3; the oracle steps the 256 x 256 x 1 original; tolerances as for one RK2 step."""
+    p2 = config("C4", n3=1)
+    prim2, _ = fm_torus(p2)                       # seeded +-2 % perturbation of u, one draw per (i, j)
+    ref = prim2.copy()
+    g = oracle.Grid(p2)
+    g.bind(ref)
+    dt = g.cfl_dt(0.45)
+    g.step(dt)
+    p3 = config("C4")
+    ng = p3["ng"]
+    assert (p3["n1"], p3["n2"], p3["n3"]) == (256, 256, 256)
+    prim3 = np.ascontiguousarray(np.broadcast_to(prim2[:, :, :, ng:ng + 1], prim2.shape[:3] + (p3["n3"] + 2 * ng,)))
+    s = cu.Solver(p3, prim3)
+    s.use_graph(True)
+    s.step(dt)
+    got = s.prim.cpu().numpy()
+    gi = interior(p3, got)
+    assert (gi == gi[..., :1]).all(), "phi-invariant input must stay bitwise phi-invariant"
+    err = prim_errors(p2, np.ascontiguousarray(got[..., :2 * ng + 1]), ref)   # the k = 0 plane, shaped like the 2D array
+    assert (err < 1e-11).all(), err
+    assert s.divb()[1] < 1e-12
+    st = s.stats()
+    assert st[0] == 0          # no inversion failures
+    s.close()
+
+
 # ------------------------------------------------------------------ launch modes, errors, edge shapes
 def test_graph_replay_is_bitwise_identical_to_plain_launches():
     p = config("C4", n1=24, n2=16, n3=12)
