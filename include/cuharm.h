@@ -109,6 +109,15 @@ int cuharm_last_cfl_dt(cuharm_handle h, double xi, double* dt_out);
  * the corners where that sum exceeds 1e-290 (below it the terms are in the subnormal range).  Synchronises. */
 int cuharm_divb(cuharm_handle h, double* max_abs, double* max_norm);
 
+/* Fluxes through the coordinate shell of zone centres of radial index i (0 <= i < n1), the paper's horizon
+ * diagnostics when i is the shell nearest r_h (eqs. 43-46): out[0] = Mdot = sum sqrt(-g) rho u^1,
+ * out[1] = phi_B = 1/2 sum sqrt(-g) |B^1| (*F^{rt} = B^r), out[2] = Ldot = sum sqrt(-g) T^1_phi,
+ * out[3] = Edot = -sum sqrt(-g) T^1_t, each summed over the interior (j, k) with weight dX2 dX3 (the integrand
+ * sqrt(-g) J^1 dX2 dX3 is coordinate invariant).  Mdot is negative for inflow, as eq. 43 is printed.  Sums are
+ * deterministic (fixed-order trees).  out: HOST pointer to 4 doubles.  Needs geometry and bound primitives with
+ * valid interior; synchronises.  CUHARM_EINVAL for i out of range. */
+int cuharm_shell_fluxes(cuharm_handle h, int32_t i, double out[4]);
+
 /* Copy a geometry table to a caller array d_out[comp][n1g][n2g]: loc 0 centre, 1 = 1-face (I-1/2,J), 2 = 2-face
  * (I,J-1/2): 22 comps = g_cov (00 01 02 03 11 12 13 22 23 33), g_con (same order), sqrt(-g), lapse; loc 3: the 40
  * connection coefficients Gamma^l_{nk}, l-major, (n,k) in the same 10-pair order.  Test helper.  Asynchronous. */

@@ -1213,6 +1213,41 @@ int oracle_divb(oracle_handle h, double* max_abs, double* max_norm) {
   return 0;
 }
 
+// fluxes through the coordinate shell of zone centres X1 = X1_i (eqs. 43-46),
+// "at the horizon" when i is the shell nearest r_h.  In the code's coordinates the integrand of each surface
+// integral is sqrt(-g) x (the X1 component of the current) dX2 dX3, which is coordinate invariant:
+//   out[0] = Mdot  = sum sqrt(-g) rho u^1            dX2 dX3   (eq. 43; negative for inflow, as printed)
+//   out[1] = phi_B = 1/2 sum sqrt(-g) |B^1|          dX2 dX3   (eq. 44; *F^{rt} = B^r)
+//   out[2] = Ldot  = sum sqrt(-g) T^1_phi            dX2 dX3   (eq. 45)
+//   out[3] = Edot  = sum -sqrt(-g) T^1_t             dX2 dX3   (eq. 46)
+// i: interior numbering 0..n1-1.  Plain sums in (j, k) order.
+int oracle_shell_fluxes(oracle_handle h, int32_t i, double out[4]) {
+  Ctx& c = h->c;
+  if (!c.prim) return -2;
+  if (i < 0 || i >= c.p.n1) return -1;
+  const int ng = c.ng, n2 = c.p.n2, n3 = c.p.n3;
+  const int ii = ng + i;
+  const double dA = c.dx[1] * c.dx[2];
+  double mdot = 0.0, phib = 0.0, ldot = 0.0, edot = 0.0;
+  for (int j = ng; j < ng + n2; j++) {
+    const Geom& G = c.gc[(size_t)ii * c.n2g + j];
+    for (int k = ng; k < ng + n3; k++) {
+      double q[8];
+      for (int v = 0; v < 8; v++) q[v] = c.prim[c.vidx(v, ii, j, k)];
+      State S;
+      fluid_state(q, G, S);
+      double F[8];
+      flux_vector(q, S, G, c.p.gam, 1, F);   // sqrt(-g) x (rho u^1, T^1_t, T^1_1, T^1_2, T^1_3, ...)
+      mdot += F[0] * dA;
+      phib += 0.5 * G.sqrtg * std::fabs(q[5]) * dA;
+      ldot += F[4] * dA;
+      edot += -F[1] * dA;
+    }
+  }
+  out[0] = mdot; out[1] = phib; out[2] = ldot; out[3] = edot;
+  return 0;
+}
+
 // 0 failed inversions, 1 zones repaired, 2 rho-floor hits, 3 u-floor hits, 4 ceilings, 5 Lorentz caps,
 // 6 Newton iterations, 7 zones repaired by the last-resort rule
 int oracle_get_stats(oracle_handle h, int64_t out[8]) {

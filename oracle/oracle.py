@@ -257,6 +257,13 @@ class Grid:
         assert rc == 0
         return a.value, n.value
 
+    def shell_fluxes(self, i):
+        """(Mdot, phi_B, Ldot, Edot) through the shell of zone centres of radial index i (eqs. 43-46)."""
+        out = np.zeros(4)
+        rc = lib().oracle_shell_fluxes(self._h, C.c_int32(i), out.ctypes.data_as(C.POINTER(C.c_double)))
+        assert rc == 0, rc
+        return out
+
     def get_stats(self):
         out = np.zeros(8, dtype=np.int64)
         lib().oracle_get_stats(self._h, out.ctypes.data_as(C.POINTER(C.c_int64)))

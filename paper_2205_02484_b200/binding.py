@@ -70,6 +70,7 @@ def lib():
         L.cuharm_cfl_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
         L.cuharm_last_cfl_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
         L.cuharm_divb.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.cuharm_shell_fluxes.argtypes = [vp, C.c_int32, C.POINTER(C.c_double)]
         L.cuharm_get_geom.argtypes = [vp, C.c_int32, dp]
         L.cuharm_apply_bc.argtypes = [vp, dp]
         L.cuharm_flux_dir.argtypes = [vp, dp, C.c_int32, dp, dp]
@@ -147,6 +148,13 @@ def cuharm_last_cfl_dt(h, xi: float) -> float:
     dt = C.c_double()
     _check(lib().cuharm_last_cfl_dt(h, float(xi), C.byref(dt)), "cuharm_last_cfl_dt")
     return dt.value
+
+
+def cuharm_shell_fluxes(h, i):
+    """(Mdot, phi_B, Ldot, Edot) through the shell of zone centres of radial index i (eqs. 43-46)."""
+    out = (C.c_double * 4)()
+    _check(lib().cuharm_shell_fluxes(h, C.c_int32(i), out), "cuharm_shell_fluxes")
+    return tuple(out)
 
 
 def cuharm_divb(h):
@@ -235,6 +243,7 @@ class Solver:
     def cfl_dt(self, xi): return cuharm_cfl_dt(self.h, xi)
     def last_cfl_dt(self, xi): return cuharm_last_cfl_dt(self.h, xi)
     def divb(self): return cuharm_divb(self.h)
+    def shell_fluxes(self, i): return cuharm_shell_fluxes(self.h, i)
     def stats(self): return cuharm_get_stats(self.h)
     def use_graph(self, on=True): cuharm_use_graph(self.h, on)
     def launch_count(self): return cuharm_launch_count(self.h)

@@ -601,6 +601,24 @@ int cuharm_last_cfl_dt(cuharm_handle h, double xi, double* dt_out) {
   return dt_from_cw(h, h->cnt + CNT_CWPRED, xi, dt_out);
 }
 
+int cuharm_shell_fluxes(cuharm_handle h, int32_t i, double out[4]) {
+  if (!h || !out) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  const Dims& d = h->d;
+  if (i < 0 || i >= d.n1) return CUHARM_EINVAL;
+  // scratch: the head of the EMF array (idle between steps): n2 x 4 partial sums + 4 results
+  double* partial = h->E;
+  double* res = h->E + (size_t)d.n2 * 4;
+  ShellArgs a{d, h->prim, h->gC, d.ng + i, h->p.gam, h->dx[1] * h->dx[2], partial, res};
+  shell_flux_kernel<<<d.n2, 128, 0, h->stream>>>(a);
+  shell_sum_kernel<<<1, 128, 0, h->stream>>>(a);
+  h->launches += 2;
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(out, res, 4 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return CUHARM_OK;
+}
+
 int cuharm_divb(cuharm_handle h, double* max_abs, double* max_norm) {
   if (!h || !max_abs || !max_norm) return CUHARM_EINVAL;
   if (!h->bound || !h->have_geom) return CUHARM_ESTATE;

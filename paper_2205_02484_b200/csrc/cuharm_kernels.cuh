@@ -617,6 +617,71 @@ __global__ void __launch_bounds__(128) divb_kernel(DivbArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Fluxes through the shell of zone centres of radial index i (eqs. 43-46):
+// Mdot = sum sqrt(-g) rho u^1, phi_B = 1/2 sum sqrt(-g) |B^1|, Ldot = sum sqrt(-g) T^1_phi, Edot = -sum sqrt(-g) T^1_t,
+// each times dX2 dX3.  Deterministic two-level sum: block j reduces its row along k in a fixed tree order into
+// partial[j][4]; shell_sum_kernel (one block) reduces over j the same way.  No floating-point atomics.
+// ---------------------------------------------------------------------------------------------------------
+struct ShellArgs {
+  Dims d;
+  const double* P;
+  const Geom* C;
+  int i;        // zone index including ghosts
+  double gam, dA;
+  double* partial;  // [n2][4]
+  double* out;      // [4]
+};
+
+__device__ __forceinline__ void block_sum4(double v[4], double (*sh)[4]) {
+  // fixed-order tree over the 128 threads of the block; result in sh[0]
+  const int t = threadIdx.x;
+#pragma unroll
+  for (int c = 0; c < 4; c++) sh[t][c] = v[c];
+  __syncthreads();
+  for (int s = 64; s > 0; s >>= 1) {
+    if (t < s) {
+#pragma unroll
+      for (int c = 0; c < 4; c++) sh[t][c] += sh[t + s][c];
+    }
+    __syncthreads();
+  }
+}
+
+__global__ void __launch_bounds__(128) shell_flux_kernel(ShellArgs a) {
+  __shared__ double sh[128][4];
+  const Dims& d = a.d;
+  const int j = d.ng + blockIdx.x;
+  const Geom G = load_geom(a.C, a.i * d.n2g + j);
+  double acc[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int k = d.ng + threadIdx.x; k < d.ng + d.n3; k += 128) {
+    const long long idx = a.i * d.s1 + j * d.s2 + k;
+    double q[8], F[8];
+#pragma unroll
+    for (int v = 0; v < 8; v++) q[v] = a.P[v * d.nz + idx];
+    State S;
+    fluid_state(q, G, S);
+    flux_vector<1>(q, S, G, a.gam, F);  // sqrt(-g) x (rho u^1, T^1_t, T^1_1, T^1_2, T^1_3, ...)
+    acc[0] += F[0] * a.dA;
+    acc[1] += 0.5 * G.sg * fabs(q[5]) * a.dA;
+    acc[2] += F[4] * a.dA;
+    acc[3] += -F[1] * a.dA;
+  }
+  block_sum4(acc, sh);
+  if (threadIdx.x < 4) a.partial[blockIdx.x * 4 + threadIdx.x] = sh[0][threadIdx.x];
+}
+
+__global__ void __launch_bounds__(128) shell_sum_kernel(ShellArgs a) {
+  __shared__ double sh[128][4];
+  double acc[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int j = threadIdx.x; j < a.d.n2; j += 128) {
+#pragma unroll
+    for (int c = 0; c < 4; c++) acc[c] += a.partial[j * 4 + c];
+  }
+  block_sum4(acc, sh);
+  if (threadIdx.x < 4) a.out[threadIdx.x] = sh[0][threadIdx.x];
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // Full-grid primitive <-> conserved (eqs. 27-31), centre geometry, ghosts included.
 // ---------------------------------------------------------------------------------------------------------
 struct ConvArgs {
