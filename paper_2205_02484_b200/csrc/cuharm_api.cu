@@ -260,11 +260,18 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
   if (fork) {
     cudaStream_t main_s = h->stream;
     CK(cudaEventRecord(h->fj[0], main_s));
-    int rc = launch_flux<false>(h, Pflux, 1, h->F[0], nullptr, cwmax + 0);
+#ifndef CUHARM_FORK_ORDER
+#define CUHARM_FORK_ORDER 1
+#endif
+    // launch order of the three directions (main branch first); measured best on B200: the persistent X3 kernel
+    // first, the many-block marching kernels fill in behind it
+    static const int order[3][3] = {{1, 2, 3}, {3, 1, 2}, {1, 3, 2}};
+    const int* od = order[CUHARM_FORK_ORDER];
+    int rc = launch_flux<false>(h, Pflux, od[0], h->F[od[0] - 1], nullptr, cwmax + od[0] - 1);
     for (int s = 0; s < 2 && !rc; s++) {
       CK(cudaStreamWaitEvent(h->side[s], h->fj[0], 0));
       h->stream = h->side[s];
-      rc = launch_flux<false>(h, Pflux, 2 + s, h->F[1 + s], nullptr, cwmax + 1 + s);
+      rc = launch_flux<false>(h, Pflux, od[1 + s], h->F[od[1 + s] - 1], nullptr, cwmax + od[1 + s] - 1);
       h->stream = main_s;
       CK(cudaEventRecord(h->fj[1 + s], h->side[s]));
       CK(cudaStreamWaitEvent(main_s, h->fj[1 + s], 0));
