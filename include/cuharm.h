@@ -43,7 +43,7 @@ typedef struct {
   int32_t n1, n2, n3, ng; /* interior zones per direction (n3 == 1 allowed); ghost layers, ng >= 3          */
   int32_t coords;         /* 0 = MKS (eq. 39; A14); 1 = Minkowski-Cartesian (tests; A39)        */
   double a, gam;          /* black-hole spin (eq. 38); adiabatic index of p = (gam-1) u     */
-  double r_in, r_out, R0, hslope; /* MKS: X1 in [ln(r_in-R0), ln(r_out-R0)], X2 in [-1,1], X3 in [0,2pi)    */
+  double r_in, r_out, R0, hslope; /* MKS: X1 in [ln(r_in-R0), X1(r_out)], X2 in [-1,1], X3 in [0,2pi)         */
   double xmin[3], xmax[3];        /* Minkowski box                                                          */
   int32_t recon;   /* 0 = PLM + MC limiter (eqs. 15-16; A2); 1 = PPM (A20)              */
   int32_t riemann; /* 0 = local Lax-Friedrichs (eq. 17); 1 = HLL (eq. 20)                   */
@@ -56,7 +56,9 @@ typedef struct {
   double newton_tol;                          /* |dW/W| criterion of the 2D Newton-Raphson (A8)     */
   int32_t newton_maxit, newton_extra;         /* iteration cap; extra iterations after the criterion is met */
   int32_t fixup_max_passes;                   /* Jacobi passes of the eq. 34 repair (A13)                   */
-  int32_t reserved;
+  int32_t n_x;     /* hyper-exponential radial branch of eq. 39: r = R0 + exp(X + (X - x_b)^n_x) for */
+  double r_break;  /* X >= x_b = ln(r_break - R0) (the paper: n_x = 4, r_break = 400 M, r_out = 5e3 M); the grid    */
+                   /* stays uniform in X1 from ln(r_in - R0) to the X1 of r_out.  Off unless n_x >= 2, r_break > R0 */
 } cuharm_params;
 
 /* Create a context for the grid and scheme described by *p (the statement of the problem: spin a, adiabatic

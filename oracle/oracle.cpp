@@ -47,7 +47,8 @@ struct oracle_params {
   double newton_tol;
   int32_t newton_maxit, newton_extra;
   int32_t fixup_max_passes;
-  int32_t reserved;
+  int32_t n_x;      // hyper-exponential radial branch of eq. 39: exponent n_X; < 2 = plain exponential
+  double r_break;   // radius of the transition X = x_b (the paper: 400 M); used when n_x >= 2 and r_break > R0
 };
 
 }  // extern "C"
@@ -60,17 +61,51 @@ const double PI = 3.14159265358979323846;
 // C-1  Coordinates (eq. 39; A14: the sine argument is pi(1+Y), not pi(1+Y)/2).
 // ------------------------------------------------------------------------------------------
 struct Coord {
-  double r, th, drdX, dthdY, d2thdY2;
+  double r, th, drdX, dthdY, d2thdY2, d2rdX2;
 };
+
+// eq. 39, radial part: r = R0 + exp(X) for X < x_b, R0 + exp(X + (X - x_b)^{n_X}) for X >= x_b, x_b = ln(r_break - R0).
+bool hyper_on(const oracle_params& p) { return p.coords == 0 && p.n_x >= 2 && p.r_break > p.R0; }
+
+void radial_map(const oracle_params& p, double X, double& r, double& d1, double& d2) {
+  double E = X, E1 = 1.0, E2 = 0.0;  // exponent and its first two derivatives
+  if (hyper_on(p)) {
+    double xb = std::log(p.r_break - p.R0);
+    if (X >= xb) {
+      double y = X - xb;
+      E = X + std::pow(y, p.n_x);
+      E1 = 1.0 + p.n_x * std::pow(y, p.n_x - 1);
+      E2 = p.n_x * (p.n_x - 1) * std::pow(y, p.n_x - 2);
+    }
+  }
+  double e = std::exp(E);
+  r = p.R0 + e;
+  d1 = e * E1;                 // dr/dX
+  d2 = e * (E1 * E1 + E2);     // d2r/dX2
+}
+
+// X at which the map reaches the radius r (inverse of radial_map; bisection on the monotone exponent)
+double radial_inverse(const oracle_params& p, double r) {
+  double target = std::log(r - p.R0);
+  if (!hyper_on(p)) return target;
+  double xb = std::log(p.r_break - p.R0);
+  if (target <= xb) return target;
+  double lo = xb, hi = target;   // X + (X-xb)^n >= X, so the solution lies in [xb, target]
+  for (int it = 0; it < 200; it++) {
+    double mid = 0.5 * (lo + hi);
+    double E = mid + std::pow(mid - xb, p.n_x);
+    if (E < target) lo = mid; else hi = mid;
+  }
+  return 0.5 * (lo + hi);
+}
 
 Coord coord_map(const oracle_params& p, double X1, double X2) {
   Coord c;
   if (p.coords == 1) {  // Minkowski: unused
-    c.r = 1.0; c.th = 0.5 * PI; c.drdX = 1.0; c.dthdY = 1.0; c.d2thdY2 = 0.0;
+    c.r = 1.0; c.th = 0.5 * PI; c.drdX = 1.0; c.dthdY = 1.0; c.d2thdY2 = 0.0; c.d2rdX2 = 0.0;
     return c;
   }
-  c.r = p.R0 + std::exp(X1);
-  c.drdX = c.r - p.R0;
+  radial_map(p, X1, c.r, c.drdX, c.d2rdX2);
   double arg = PI * (1.0 + X2);
   c.th = 0.5 * PI * (1.0 + X2) + 0.5 * (1.0 - p.hslope) * std::sin(arg);
   c.dthdY = 0.5 * PI * (1.0 + (1.0 - p.hslope) * std::cos(arg));
@@ -169,9 +204,9 @@ void conn_at(const oracle_params& p, double X1, double X2, double conn[4][4][4])
   // g_phiphi = s2 * (Sig + a^2 s2 (1+f))
   dgr[3][3] = s2 * (dSig_r + a * a * s2 * df_r);
   dgt[3][3] = ds2_t * (Sig + a * a * s2 * (1.0 + f)) + s2 * (dSig_t + a * a * (ds2_t * (1.0 + f) + s2 * df_t));
-  // MKS: gM_{mn} = J_m J_n g_{mn};  dJ_1/dX = r' (since r' = r - R0),  dJ_2/dY = th''
+  // MKS: gM_{mn} = J_m J_n g_{mn};  dJ_1/dX = r'',  dJ_2/dY = th''
   double J[4] = {1.0, c.drdX, c.dthdY, 1.0};
-  double dJ1[4] = {0.0, c.drdX, 0.0, 0.0};     // d J_m / dX
+  double dJ1[4] = {0.0, c.d2rdX2, 0.0, 0.0};   // d J_m / dX  (= r' on the plain exponential branch)
   double dJ2[4] = {0.0, 0.0, c.d2thdY2, 0.0};  // d J_m / dY
   double dg[4][4][4];                          // dg[s][k][n] = d_n gM_{s k}
   for (int m = 0; m < 4; m++) for (int n = 0; n < 4; n++) {
@@ -910,6 +945,11 @@ int oracle_get_threads(void) {
 }
 
 // ---- point-level entry points (for the pins) ----
+void oracle_radial_map(const oracle_params* p, double X1, double out[4]) {   // r, r', r'', and X of r_out
+  radial_map(*p, X1, out[0], out[1], out[2]);
+  out[3] = radial_inverse(*p, p->r_out);
+}
+
 void oracle_coord_map(const oracle_params* p, double X1, double X2, double out[5]) {
   Coord c = coord_map(*p, X1, X2);
   out[0] = c.r; out[1] = c.th; out[2] = c.drdX; out[3] = c.dthdY; out[4] = c.d2thdY2;
@@ -1000,7 +1040,7 @@ int oracle_grid_init(oracle_handle* out, const oracle_params* p) {
   c.nz = (size_t)c.n1g * c.n2g * c.n3g;
   if (p->coords == 0) {
     c.x0[0] = std::log(p->r_in - p->R0);
-    c.dx[0] = (std::log(p->r_out - p->R0) - std::log(p->r_in - p->R0)) / p->n1;
+    c.dx[0] = (radial_inverse(*p, p->r_out) - c.x0[0]) / p->n1;   // uniform in X up to the X of r_out
     c.x0[1] = -1.0; c.dx[1] = 2.0 / p->n2;
     c.x0[2] = 0.0;  c.dx[2] = 2.0 * PI / p->n3;
   } else {

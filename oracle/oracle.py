@@ -28,7 +28,8 @@ class OracleParams(C.Structure):
         ("sigma_max", C.c_double), ("b2_over_u_max", C.c_double), ("gamma_max", C.c_double),
         ("newton_tol", C.c_double),
         ("newton_maxit", C.c_int32), ("newton_extra", C.c_int32),
-        ("fixup_max_passes", C.c_int32), ("reserved", C.c_int32),
+        ("fixup_max_passes", C.c_int32), ("n_x", C.c_int32),
+        ("r_break", C.c_double),
     ]
 
 
@@ -75,6 +76,13 @@ def coord_map(params: dict, X1, X2):
     out = np.zeros(5)
     lib().oracle_coord_map(C.byref(make_params(params)), C.c_double(X1), C.c_double(X2), _d(out))
     return dict(r=out[0], th=out[1], drdX=out[2], dthdY=out[3], d2thdY2=out[4])
+
+
+def radial_map(params: dict, X1):
+    """r, dr/dX, d2r/dX2 of eq. 39's radial map at X1, and X_out = the X of r_out."""
+    out = np.zeros(4)
+    lib().oracle_radial_map(C.byref(make_params(params)), C.c_double(X1), _d(out))
+    return dict(r=out[0], d1=out[1], d2=out[2], X_out=out[3])
 
 
 def metric_at(params: dict, X1, X2, polar_face=0):

@@ -30,7 +30,8 @@ class CuharmParams(C.Structure):
         ("sigma_max", C.c_double), ("b2_over_u_max", C.c_double), ("gamma_max", C.c_double),
         ("newton_tol", C.c_double),
         ("newton_maxit", C.c_int32), ("newton_extra", C.c_int32),
-        ("fixup_max_passes", C.c_int32), ("reserved", C.c_int32),
+        ("fixup_max_passes", C.c_int32), ("n_x", C.c_int32),
+        ("r_break", C.c_double),
     ]
 
 

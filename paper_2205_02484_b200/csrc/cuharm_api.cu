@@ -62,6 +62,8 @@ struct cuharm_ctx {
   bool upd_tma = false;  // update_tma_kernel usable (shared-memory opt-in succeeded)
   int upd_blocks = 0, upd_blocks64 = 0;  // its persistent grid sizes (128- and 64-zone tiles)
   int sms = 148;         // multiprocessors of the device
+  double xb = 0.0;       // eq. 39: X1 of the exponential -> hyper-exponential transition
+  int nx = 0;            // its exponent (0: plain exponential)
   bool fluxk_row = true; // prefer the whole-row pipeline (flux_k_row_kernel)
   bool use_graph = false;
   cudaGraphExec_t gexec = nullptr;
@@ -360,6 +362,7 @@ int check_params(const cuharm_params* p) {
     return CUHARM_EINVAL;
   if (p->coords == 0) {
     if (!(p->r_in - p->R0 > 0.0) || !(p->r_out > p->r_in) || !(std::fabs(p->a) <= 1.0)) return CUHARM_EINVAL;
+    if (p->n_x < 0 || p->n_x > 16 || !std::isfinite(p->r_break)) return CUHARM_EINVAL;
   } else {
     for (int c = 0; c < 3; c++)
       if (!(p->xmax[c] > p->xmin[c])) return CUHARM_EINVAL;
@@ -390,7 +393,29 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
   if (p->coords == 0) {  // eq. 39: uniform in X1 = ln(r - R0), X2 in [-1,1], X3 in [0, 2 pi)
     const double PI = 3.14159265358979323846;
     h->x0[0] = std::log(p->r_in - p->R0);
-    h->dx[0] = (std::log(p->r_out - p->R0) - std::log(p->r_in - p->R0)) / p->n1;
+    // outer edge: the X1 at which eq. 39's radial map reaches r_out.  On the hyper-exponential branch that is the
+    // root of X + (X - x_b)^n = ln(r_out - R0), found by Newton from above (the function is convex and increasing)
+    double x_out = std::log(p->r_out - p->R0);
+    h->xb = 0.0;
+    h->nx = 0;
+    if (p->n_x >= 2 && p->r_break > p->R0) {
+      h->nx = p->n_x;
+      h->xb = std::log(p->r_break - p->R0);
+      const double target = x_out;
+      if (target > h->xb) {
+        double x = target;
+        for (int it = 0; it < 100; it++) {
+          const double y = x - h->xb;
+          const double f = x + std::pow(y, h->nx) - target;
+          const double fp = 1.0 + h->nx * std::pow(y, h->nx - 1);
+          const double xn = x - f / fp;
+          if (std::fabs(xn - x) <= 1e-16 * std::fabs(x)) { x = xn; break; }
+          x = xn;
+        }
+        x_out = x;
+      }
+    }
+    h->dx[0] = (x_out - h->x0[0]) / p->n1;
     h->x0[1] = -1.0; h->dx[1] = 2.0 / p->n2;
     h->x0[2] = 0.0;  h->dx[2] = 2.0 * PI / p->n3;
   } else {
@@ -467,7 +492,7 @@ int cuharm_metric_precompute(cuharm_handle h) {
   const cuharm_params& p = h->p;
   const Dims& d = h->d;
   GeomArgs a{d.n1g, d.n2g, d.ng, d.n2, p.coords, (p.coords == 0 && p.bc_x2 == 2) ? 1 : 0, p.a, p.R0, p.hslope,
-             h->x0[0], h->x0[1], h->dx[0], h->dx[1], p.rho_fl_coef, p.rho_fl_pow, p.rho_fl_abs, p.u_fl_coef,
+             h->xb, h->nx, h->x0[0], h->x0[1], h->dx[0], h->dx[1], p.rho_fl_coef, p.rho_fl_pow, p.rho_fl_abs, p.u_fl_coef,
              p.u_fl_pow, p.u_fl_abs, h->gC, h->gF1, h->gF2, h->conn, h->floors};
   const int n = d.n1g * d.n2g;
   geom_kernel<<<(n + 63) / 64, 64, 0, h->stream>>>(a);

@@ -11,6 +11,8 @@ struct GeomArgs {
   int n1g, n2g, ng, n2;
   int coords, polar_bc;  // polar_bc: X2 boundary is the polar reflection -> the 2-faces J = 0, n2 lie on the axis (A32)
   double a, R0, hslope;
+  double xb;       // X1 of the exponential -> hyper-exponential transition (eq. 39); used when nx >= 2
+  int nx;          // exponent n_X of the hyper-exponential branch; < 2: plain exponential everywhere
   double x0_1, x0_2, dx1, dx2;
   double rho_fl_coef, rho_fl_pow, rho_fl_abs, u_fl_coef, u_fl_pow, u_fl_abs;
   Geom *C, *F1, *F2;
@@ -20,13 +22,31 @@ struct GeomArgs {
 
 struct MksPoint {
   double r, th, rp, thp, thpp;  // r, theta, dr/dX1, dtheta/dX2, d2theta/dX2^2
+  double rpp;                   // d2r/dX1^2
 };
+
+__device__ inline double ipow(double y, int n) {  // y^n for small n >= 0 by repeated multiplication
+  double v = 1.0;
+  for (int q = 0; q < n; q++) v *= y;
+  return v;
+}
 
 __device__ inline MksPoint mks_point(const GeomArgs& A, double X1, double X2) {
   const double PI = 3.14159265358979323846;
   MksPoint p;
-  p.r = A.R0 + exp(X1);
-  p.rp = p.r - A.R0;
+  // eq. 39: r = R0 + exp(E), E = X for X < x_b, E = X + (X - x_b)^n_X beyond; r' = (r - R0) E', r'' = (r - R0)(E'^2 + E'')
+  double E = X1, E1 = 1.0, E2 = 0.0;
+  if (A.nx >= 2 && X1 >= A.xb) {
+    const double y = X1 - A.xb;
+    const double ym2 = ipow(y, A.nx - 2);
+    E = X1 + ym2 * y * y;
+    E1 = 1.0 + A.nx * ym2 * y;
+    E2 = A.nx * (A.nx - 1) * ym2;
+  }
+  const double e = exp(E);
+  p.r = A.R0 + e;
+  p.rp = e * E1;
+  p.rpp = e * (E1 * E1 + E2);
   const double arg = PI * (1.0 + X2);
   const double s = sin(arg), c = cos(arg);
   p.th = 0.5 * PI * (1.0 + X2) + 0.5 * (1.0 - A.hslope) * s;
@@ -101,7 +121,7 @@ __device__ inline void mks_conn(const GeomArgs& A, double X1, double X2, const G
   for (int m = 0; m < 4; m++)
     for (int n = 0; n < m; n++) { k[m][n] = k[n][m]; kr[m][n] = kr[n][m]; kt[m][n] = kt[n][m]; }
   const double J[4] = {1.0, p.rp, p.thp, 1.0};
-  const double J1[4] = {0.0, p.rp, 0.0, 0.0};    // dJ/dX1 (r' = r - R0 so r'' = r')
+  const double J1[4] = {0.0, p.rpp, 0.0, 0.0};   // dJ/dX1 = r'' (= r' on the plain exponential branch)
   const double J2[4] = {0.0, 0.0, p.thpp, 0.0};  // dJ/dX2
   double dg[4][4][4];                            // dg[m][n][c] = d_c g_{mn}
   for (int m = 0; m < 4; m++)

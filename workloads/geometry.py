@@ -6,13 +6,29 @@ sqrt(-g) to turn a physical set-up into the primitive array both implementations
 import numpy as np
 
 
+def _hyper(p: dict):
+    return p["coords"] == 0 and p.get("n_x", 0) >= 2 and p.get("r_break", 0.0) > p["R0"]
+
+
+def radial_x_of_r(p: dict, r):
+    """X1 at which eq. 39's radial map (with its hyper-exponential branch, if switched on) reaches the radius r."""
+    target = np.log(r - p["R0"])
+    if not _hyper(p):
+        return target
+    xb = np.log(p["r_break"] - p["R0"])
+    if target <= xb:
+        return target
+    from scipy.optimize import brentq
+    return brentq(lambda x: x + (x - xb) ** p["n_x"] - target, xb, target, xtol=1e-15, rtol=1e-15)
+
+
 def grid_coords(p: dict, centred=True):
     """X1, X2, X3 of zone centres over the extended grid (ghosts included)."""
     ng = p["ng"]
     n = (p["n1"], p["n2"], p["n3"])
     if p["coords"] == 0:
         x0 = (np.log(p["r_in"] - p["R0"]), -1.0, 0.0)
-        x1 = (np.log(p["r_out"] - p["R0"]), 1.0, 2.0 * np.pi)
+        x1 = (radial_x_of_r(p, p["r_out"]), 1.0, 2.0 * np.pi)
     else:
         x0, x1 = p["xmin"], p["xmax"]
     out = []
@@ -26,10 +42,17 @@ def grid_coords(p: dict, centred=True):
 
 
 def mks_to_ks(p: dict, X1, X2):
-    r = p["R0"] + np.exp(X1)
+    X1 = np.asarray(X1, dtype=float)
+    E, E1 = X1, np.ones_like(X1)
+    if _hyper(p):                                   # eq. 39, X >= x_b: r = R0 + exp(X + (X - x_b)^n_X)
+        xb = np.log(p["r_break"] - p["R0"])
+        y = np.maximum(X1 - xb, 0.0)
+        E = X1 + y ** p["n_x"]
+        E1 = 1.0 + p["n_x"] * y ** (p["n_x"] - 1)
+    r = p["R0"] + np.exp(E)
     arg = np.pi * (1.0 + X2)
     th = 0.5 * np.pi * (1.0 + X2) + 0.5 * (1.0 - p["hslope"]) * np.sin(arg)
-    drdX = r - p["R0"]
+    drdX = (r - p["R0"]) * E1
     dthdY = 0.5 * np.pi * (1.0 + (1.0 - p["hslope"]) * np.cos(arg))
     return r, th, drdX, dthdY
 

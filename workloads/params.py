@@ -27,6 +27,7 @@ def default_params(**kw) -> dict:
         sigma_max=50.0, b2_over_u_max=2.5e3, gamma_max=50.0,           # eqs. 36-37
         newton_tol=1e-10, newton_maxit=30, newton_extra=2,             # P:L233 (A8)
         fixup_max_passes=4,
+        n_x=0, r_break=0.0,            # hyper-exponential radial branch of eq. 39: off; the paper: 4, 400
     )
     d.update(kw)
     if "a" in kw and "r_in" not in kw:
