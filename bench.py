@@ -136,6 +136,8 @@ def run_reference(args):
     per_step = []
     p = None
     import oracle
+    if args.threads:
+        oracle.set_threads(args.threads)
     p, prim = make_workload(args.config, n3=args.ref_n3)
     g = oracle.Grid(p)
     g.bind(prim)
@@ -203,6 +205,8 @@ def run_ours(args):
     e0.record()
     for _ in range(args.steps):
         s.step(dt)
+        if args.cfl_each_step:           # second protocol, eq. 26 evaluated (and synchronised) every step;
+            s.last_cfl_dt(0.45)          # the step size itself stays fixed so that the work per step is the same
     e1.record()
     barrier()
     ms = e0.elapsed_time(e1)
@@ -301,6 +305,7 @@ def run_ours(args):
                                       f"riemann={'HLL' if p['riemann'] else 'LLF'}, fixed dt from cfl_dt(0.45)",
                           "l2": "inputs larger than L2 (prim 1.15 GB, fluxes 3 GB per substep vs 126 MB L2)",
                           "parallelism": "replicas only" if world > 1 else "single GPU", "graph": bool(args.graph),
+                          "cfl_each_step": bool(args.cfl_each_step),
                           "dt": dt},
                "clocks": clocks, "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": nbytes,
                                          "d2h_bytes_per_step": nbytes, "steps": e2e_steps,
@@ -325,6 +330,8 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=3)
     ap.add_argument("--ref-n3", type=int, default=32)
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cfl-each-step", action="store_true", help="call cuharm_last_cfl_dt (eq. 26) after every step")
+    ap.add_argument("--threads", type=int, default=0, help="reference arm: OpenMP threads of the oracle (0 = all)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
