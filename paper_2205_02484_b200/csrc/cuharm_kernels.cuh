@@ -3,7 +3,6 @@
 // reductions.  fp64, SoA prim[8][n1g][n2g][n3g] with k (phi) fastest: a warp runs along k at fixed (i,j), so
 // every geometry read is a broadcast (the metric is phi-independent).
 #pragma once
-#include <type_traits>
 #include "cuharm_flux.cuh"
 
 namespace cuharm {
@@ -308,23 +307,10 @@ constexpr int UPD_NROW = 63;   // 8 P^n, 8 P-flux, 10 F1, 10 F2, 5 F3 (hydro), 2
 constexpr int UPD_TAB = 62;    // doubles of per-(i,j) records staged behind the rows: Geom 20, connection 40, floors 2
 __host__ __device__ constexpr int upd_smem(int tb) { return (UPD_NROW * upd_row(tb) + 2 * 64) * 8; }  // dynamic shared memory per block
 
-// row r of the stage: which array, which component, which (di, dj) offset of the zone row
-struct UpdRowSrc { signed char arr, comp, di, dj; };  // arr: 0 Pbase, 1 Pflux, 2 F1, 3 F2, 4 F3
-__device__ __forceinline__ UpdRowSrc upd_row_src(int r) {
-  if (r < 8) return {0, (signed char)r, 0, 0};
-  if (r < 16) return {1, (signed char)(r - 8), 0, 0};
-  if (r < 26) return {2, (signed char)((r - 16) >> 1), (signed char)(((r - 16) & 1) ? 0 : 1), 0};   // F1[i+1], F1[i]
-  if (r < 36) return {3, (signed char)((r - 26) >> 1), 0, (signed char)(((r - 26) & 1) ? 0 : 1)};   // F2[j+1], F2[j]
-  if (r < 41) return {4, (signed char)(r - 36), 0, 0};
-  // induction fluxes; component slots F1: [5] = B2, [6] = B3;  F2: [5] = B3, [6] = B1;  F3: [5] = B1, [6] = B2
-  if (r < 43) return {3, 5, 0, (signed char)(r - 41)};                 // 41, 42: F2(B3) at j, j+1
-  if (r < 46) return {4, 6, 0, (signed char)(r - 44)};                 // 43..45: F3(B2) at j-1, j, j+1
-  if (r < 49) return {4, 5, (signed char)(r - 47), 0};                 // 46..48: F3(B1) at i-1, i, i+1
-  if (r < 51) return {2, 6, (signed char)(r - 49), 0};                 // 49, 50: F1(B3) at i, i+1
-  if (r < 57) return {2, 5, (signed char)((r - 51) / 3), (signed char)((r - 51) % 3 - 1)};  // F1(B2) (i..i+1) x (j-1..j+1)
-  return {3, 6, (signed char)((r - 57) % 3 - 1), (signed char)((r - 57) / 3)};              // F2(B1) (i-1..i+1) x (j..j+1)
-}
-
+// Stage rows: 0..7 P^n; 8..15 P-flux; 16..25 F1 hydro, (i+1, i) per component; 26..35 F2 hydro, (j+1, j) per component;
+// 36..40 F3 hydro; induction fluxes (component slots F1: [5] = B2, [6] = B3;  F2: [5] = B3, [6] = B1;  F3: [5] = B1,
+// [6] = B2): 41, 42 F2(B3) at j, j+1; 43..45 F3(B2) at j-1, j, j+1; 46..48 F3(B1) at i-1, i, i+1; 49, 50 F1(B3) at
+// i, i+1; 51..56 F1(B2) on (i, i+1) x (j-1, j, j+1); 57..62 F2(B1) on (j, j+1) x (i-1, i, i+1).
 struct TileIdx { int i, j, c; };  // zone-row (i, j) (interior numbering) and 128-zone chunk of a tile
 struct TileCnt { int s, i, jj, c; };  // mixed-radix tile counter: j-strip, i, j within the strip, chunk
 
@@ -379,36 +365,68 @@ __global__ void __launch_bounds__(TB, (CUHARM_UPD_TMA_MINB * 128) / TB) update_t
   auto tile_bytes = [&](const TileIdx& x) {  // staged zones per row (even count) x 8
     return (unsigned)min(UPD_ROW - 2, d.n3g - (d.ng + x.c * TB - 1)) * 8u;
   };
-  // Every warp issues its share of the tile's copies (rows r = w, w + NWARP, ...) with warp-uniform operands: the
-  // row index is unrolled per warp, the addresses come from kernel parameters and the tile indices, so each bulk
-  // copy is a handful of uniform-datapath instructions; per-lane operands would make the compiler serialise the
-  // lanes in an elect loop that waits on the previous copy.
+  // Every warp issues its share of the tile's copies with warp-uniform operands (addresses from kernel parameters
+  // and the tile indices), so each bulk copy is a handful of uniform-datapath instructions; per-lane operands would
+  // make the compiler serialise the lanes in an elect loop that waits on the previous copy.
   constexpr int NWARP = TB / 32;
   double* const tab = rows + UPD_NROW * UPD_ROW;  // two slots of [20] geometry record, [40] connection, [2] floors
-  auto issue_rows = [&](auto wtag, unsigned bytes, long long base) {
-    constexpr int W = decltype(wtag)::value;
+  // Rows are dealt to the warps in four groups of contiguous stage rows (two groups for 64-thread blocks), and
+  // inside a group the source addresses are walked with running byte pointers (one 64-bit add per row or less),
+  // following the row table above.
+  const long long nz8 = d.nz * 8, s18 = d.s1 * 8, s28 = d.s2 * 8;
+  const unsigned rowb = UPD_ROW * 8u;
+  const unsigned stage0 = smem_u32(rows);
+  auto put = [&](int r, const char* src, unsigned bytes) { bulk_g2s(stage0 + r * rowb, src, bytes, bar0); };
+  auto issue_group = [&](int grp, unsigned bytes, long long base8) {
+    if (grp == 0) {  // rows 0..15: P^n, P-flux
+      const char* pb = reinterpret_cast<const char*>(a.Pbase) + base8;
 #pragma unroll
-    for (int r = W; r < UPD_NROW; r += NWARP) {
-      if (SAME && r >= 8 && r < 16) continue;
-      const UpdRowSrc q = upd_row_src(r);
-      const double* arr = q.arr == 0 ? a.Pbase : q.arr == 1 ? a.Pflux : q.arr == 2 ? a.F1 : q.arr == 3 ? a.F2 : a.F3;
-      bulk_g2s(smem_u32(rows + r * UPD_ROW), arr + q.comp * d.nz + q.di * d.s1 + q.dj * d.s2 + base, bytes, bar0);
+      for (int v = 0; v < 8; v++) { put(v, pb, bytes); pb += nz8; }
+      if (!SAME) {
+        const char* pf = reinterpret_cast<const char*>(a.Pflux) + base8;
+#pragma unroll
+        for (int v = 0; v < 8; v++) { put(8 + v, pf, bytes); pf += nz8; }
+      }
+    } else if (grp == 1) {  // rows 16..35: hydro fluxes of directions 1 and 2, (upper face, lower face) per component
+      const char* f1 = reinterpret_cast<const char*>(a.F1) + base8;
+      const char* f2 = reinterpret_cast<const char*>(a.F2) + base8;
+#pragma unroll
+      for (int v = 0; v < 5; v++) {
+        put(16 + 2 * v, f1 + s18, bytes); put(17 + 2 * v, f1, bytes); f1 += nz8;
+        put(26 + 2 * v, f2 + s28, bytes); put(27 + 2 * v, f2, bytes); f2 += nz8;
+      }
+    } else if (grp == 2) {  // rows 36..50: hydro fluxes of direction 3; induction fluxes F2(B3), F3(B2), F3(B1), F1(B3)
+      const char* f3 = reinterpret_cast<const char*>(a.F3) + base8;
+#pragma unroll
+      for (int v = 0; v < 5; v++) { put(36 + v, f3, bytes); f3 += nz8; }
+      // f3 now points at component 5 = F3(B1); component 6 = F3(B2) is one array further
+      put(46, f3 - s18, bytes); put(47, f3, bytes); put(48, f3 + s18, bytes);
+      f3 += nz8;
+      put(43, f3 - s28, bytes); put(44, f3, bytes); put(45, f3 + s28, bytes);
+      const char* f2b3 = reinterpret_cast<const char*>(a.F2) + base8 + 5 * nz8;
+      put(41, f2b3, bytes); put(42, f2b3 + s28, bytes);
+      const char* f1b3 = reinterpret_cast<const char*>(a.F1) + base8 + 6 * nz8;
+      put(49, f1b3, bytes); put(50, f1b3 + s18, bytes);
+    } else {  // rows 51..62: F1(B2) on (i..i+1) x (j-1..j+1), F2(B1) on (i-1..i+1) x (j..j+1)
+      const char* f1b2 = reinterpret_cast<const char*>(a.F1) + base8 + 5 * nz8 - s28;
+#pragma unroll
+      for (int q = 0; q < 3; q++) { put(51 + q, f1b2, bytes); put(54 + q, f1b2 + s18, bytes); f1b2 += s28; }
+      const char* f2b1 = reinterpret_cast<const char*>(a.F2) + base8 + 6 * nz8 - s18;
+#pragma unroll
+      for (int q = 0; q < 3; q++) { put(57 + q, f2b1, bytes); put(60 + q, f2b1 + s28, bytes); f2b1 += s18; }
     }
   };
   auto issue = [&](const TileIdx& x, int slot) {  // all warps; lane 0 of each issues
     if ((t & 31) != 0) return;
     const unsigned bytes = tile_bytes(x);
-    const long long base = tile_base(x);
+    const long long base8 = tile_base(x) * 8;
     const int w = t >> 5;
-    if (w == 0) {
-      mbar_expect_tx(bar0, bytes * (SAME ? UPD_NROW - 8 : UPD_NROW) + UPD_TAB * 8u);
-      issue_rows(std::integral_constant<int, 0>{}, bytes, base);
-    } else if (w == 1) {
-      issue_rows(std::integral_constant<int, 1>{}, bytes, base);
-    } else if (NWARP > 2 && w == 2) {
-      issue_rows(std::integral_constant<int, 2 % NWARP>{}, bytes, base);
-    } else if (NWARP > 2) {
-      issue_rows(std::integral_constant<int, 3 % NWARP>{}, bytes, base);
+    if (w == 0) mbar_expect_tx(bar0, bytes * (SAME ? UPD_NROW - 8 : UPD_NROW) + UPD_TAB * 8u);
+    if (NWARP == 4) {
+      issue_group(w, bytes, base8);
+    } else {  // two warps: groups (0, 2) and (1, 3)
+      issue_group(w, bytes, base8);
+      issue_group(w + 2, bytes, base8);
     }
     if (w == NWARP - 1) {
       const size_t q = (size_t)(d.ng + x.i) * d.n2g + (d.ng + x.j);
