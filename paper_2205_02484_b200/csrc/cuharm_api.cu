@@ -130,6 +130,20 @@ struct Timed {
 int launch_bc(cuharm_ctx* h, double* P, const unsigned long long* gate) {
   Timed t_(h, CUHARM_K_BC);
   const Dims& d = h->d;
+#ifndef CUHARM_BC_SEPARATE
+  {  // one launch for the whole ghost fill (bit-identical to the three-kernel sequence below)
+    if (h->p.bc_x1 == 3 && h->p.bc_x2 == 3 && h->p.bc_x3 == 3) return CUHARM_OK;
+    const int nrows_a = d.n1g * d.n2g - d.n1 * d.n2;
+    const int kchunks = (d.n3g + 127) / 128;
+    const int per = 128 / (2 * d.ng);
+    const long long nb = (long long)nrows_a * kchunks + ((long long)d.n1 * d.n2 + per - 1) / per;
+    BcAllArgs b{d, P, h->gC, h->p.bc_x1, h->p.bc_x2, h->p.bc_x3, h->p.coords, h->p.gamma_max, gate, nrows_a};
+    bc_all_kernel<<<(unsigned)nb, 128, 0, h->stream>>>(b);
+    h->launches++;
+    CK(cudaGetLastError());
+    return CUHARM_OK;
+  }
+#endif
   BcArgs a{d, P, h->gC, 0, h->p.coords, h->p.gamma_max, gate};
   const int T = 128;
   if (h->p.bc_x1 != 3) {

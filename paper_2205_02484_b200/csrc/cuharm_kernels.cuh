@@ -115,6 +115,105 @@ __global__ void bc_x3_kernel(BcArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// S1 in one launch.  The three fills above run X1, X2, X3 one after the other, each over the full extended range of
+// the other two directions, so the final content of a ghost zone (i, j, k) is a composition: X3 copies from
+// (i, j, ks) what X2 left there, which X2 took (with its sign flips / rescaling) from (i, js, ks) as X1 left it,
+// which X1 made from the interior zone (is, js, ks).  Every source of that chain is a zone no fill writes
+// (interior, or a ghost of a `fixed` direction), so all ghost zones can be produced at once, in place, from the
+// same inputs and by the same arithmetic in the same order as the three-kernel sequence: bit-identical results.
+// Block rows: first the (i, j) rows that are ghosts in X1 or X2 (whole k range), then the rows interior in (i, j)
+// (their 2 ng ghost zones in k only), 21 of those rows per block.
+// ---------------------------------------------------------------------------------------------------------
+struct BcAllArgs {
+  Dims d;
+  double* P;
+  const Geom* C;
+  int kind1, kind2, kind3, coords;
+  double gamma_max;
+  const unsigned long long* gate;
+  int nrows_a;  // (i, j) rows with a ghost index in X1 or X2
+};
+
+__device__ __forceinline__ int bc_source(int x, int n, int ng, int kind, bool reflect_ok) {
+  // source index of ghost index x (extended numbering) in a direction with n interior zones
+  if (x >= ng && x < ng + n) return x;
+  if (kind == 1) {
+    const int I = x - ng;
+    return ng + ((I % n) + n) % n;
+  }
+  if (kind == 2 && reflect_ok) return x < ng ? 2 * ng - 1 - x : 2 * (ng + n) - 1 - x;
+  return x < ng ? ng : ng + n - 1;
+}
+
+__device__ __forceinline__ void bc_zone(const BcAllArgs& a, int i, int j, int k) {
+  const Dims& d = a.d;
+  const bool gi = (i < d.ng || i >= d.ng + d.n1) && a.kind1 != 3;
+  const bool gj = (j < d.ng || j >= d.ng + d.n2) && a.kind2 != 3;
+  const bool gk = (k < d.ng || k >= d.ng + d.n3) && a.kind3 != 3;
+  if (!(gi || gj || gk)) return;
+  const int is = gi ? bc_source(i, d.n1, d.ng, a.kind1, false) : i;
+  const int js = gj ? bc_source(j, d.n2, d.ng, a.kind2, true) : j;
+  const int ks = gk ? bc_source(k, d.n3, d.ng, a.kind3, false) : k;
+  double q[8];
+  const long long src = is * d.s1 + js * d.s2 + ks;
+#pragma unroll
+  for (int v = 0; v < 8; v++) q[v] = a.P[v * d.nz + src];
+  if (gi && a.kind1 == 0) {  // X1 outflow: what bc_x1_kernel does in row js
+    const Geom Gg = load_geom(a.C, i * d.n2g + js);
+    const double ratio = __ldg(&a.C[is * d.n2g + js].sg) / Gg.sg;  // sqrt(-g) B^i constant across the copy
+    q[5] *= ratio; q[6] *= ratio; q[7] *= ratio;
+    if (a.coords == 0) inflow_check(q, Gg, i < d.ng, a.gamma_max);
+  }
+  if (gj) {  // X2: what bc_x2_kernel does in column i
+    if (a.kind2 == 2) { q[3] = -q[3]; q[6] = -q[6]; }  // utilde^2, B^2 change sign
+    if (a.kind2 == 0) {
+      const double ratio = __ldg(&a.C[i * d.n2g + js].sg) / __ldg(&a.C[i * d.n2g + j].sg);
+      q[5] *= ratio; q[6] *= ratio; q[7] *= ratio;
+    }
+  }
+  const long long dst = i * d.s1 + j * d.s2 + k;
+#pragma unroll
+  for (int v = 0; v < 8; v++) a.P[v * d.nz + dst] = q[v];
+}
+
+__global__ void __launch_bounds__(128) bc_all_kernel(BcAllArgs a) {
+  if (a.gate && *a.gate == 0ull) return;
+  const Dims& d = a.d;
+  const int b = blockIdx.x;
+  const int kchunks = (d.n3g + 127) / 128;
+  if (b < a.nrows_a * kchunks) {
+    // family A: rows with a ghost index in X1 or X2, enumerated as the extended (i, j) plane minus its interior
+    const int row = b / kchunks, k = (b - row * kchunks) * 128 + threadIdx.x;
+    if (k >= d.n3g) return;
+    int i, j;
+    const int top = d.ng * d.n2g;                 // rows with i < ng
+    const int mid = d.n1 * 2 * d.ng;              // interior i, ghost j
+    if (row < top) { i = row / d.n2g; j = row - i * d.n2g; }
+    else if (row < top + mid) {
+      const int r = row - top;
+      i = d.ng + r / (2 * d.ng);
+      const int jj = r - (i - d.ng) * 2 * d.ng;
+      j = jj < d.ng ? jj : d.n2 + jj;
+    } else {
+      const int r = row - top - mid;
+      i = d.ng + d.n1 + r / d.n2g;
+      j = r - (i - d.ng - d.n1) * d.n2g;
+    }
+    bc_zone(a, i, j, k);
+  } else {
+    // family B: interior (i, j) rows, their 2 ng ghost zones in k; 21 rows x 6 zones per block (ng = 3)
+    const int per = 128 / (2 * d.ng);
+    const int slot = threadIdx.x / (2 * d.ng), g = threadIdx.x - slot * 2 * d.ng;
+    if (slot >= per) return;
+    const long long row = (long long)(b - a.nrows_a * kchunks) * per + slot;
+    if (row >= (long long)d.n1 * d.n2) return;
+    const int i = d.ng + (int)(row / d.n2), j = d.ng + (int)(row % d.n2);
+    const int k = g < d.ng ? g : d.n3 + g;
+    bc_zone(a, i, j, k);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // S4  Flux-CT edge EMFs (eq. 21).  E^1 on (I, J-1/2, K-1/2), E^2 on (I-1/2, J, K-1/2),
 // E^3 on (I-1/2, J-1/2, K), each stored at zone (I,J,K).  Range ng..ng+N inclusive in every direction.
 // ---------------------------------------------------------------------------------------------------------
