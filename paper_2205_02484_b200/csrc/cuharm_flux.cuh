@@ -339,8 +339,14 @@ __global__ void __launch_bounds__(128, CUHARM_FLUXK_MINB) flux_k_kernel(FluxArgs
 // arithmetic of this one), and whole rows keep the copy count low: a warp issues its bulk copies one after the
 // other at ~8 issue slots each.
 // ---------------------------------------------------------------------------------------------------------
+#ifndef CUHARM_KROW_T
+#define CUHARM_KROW_T 128
+#endif
+#ifndef CUHARM_KROW_B
+#define CUHARM_KROW_B 4
+#endif
 template <int RECON, int RIEMANN, bool STAGE>
-__global__ void __launch_bounds__(128, 4) flux_k_row_kernel(FluxArgs a, int wpr) {
+__global__ void __launch_bounds__(CUHARM_KROW_T, CUHARM_KROW_B) flux_k_row_kernel(FluxArgs a, int wpr) {
   extern __shared__ __align__(128) double rowbuf[];  // [2][8][n3g]
   __shared__ __align__(8) unsigned long long mbar2[2];
   const Dims& d = a.d;
