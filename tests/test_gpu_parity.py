@@ -360,7 +360,9 @@ def test_graph_replay_is_bitwise_identical_to_plain_launches():
 
 
 def test_tiny_and_ragged_grids():
-    for n in ((1, 1, 1), (3, 2, 1), (5, 7, 129), (2, 3, 130)):
+    # n3 odd -> generic kernels; even -> bulk-copy kernels: 64-zone tiles (n3 <= 64), one ragged 128-zone chunk, two and
+    # three chunks with a ragged tail; n2 prime / composite -> strip widths 1 and 6 of the tile order
+    for n in ((1, 1, 1), (3, 2, 1), (5, 7, 129), (2, 3, 130), (6, 17, 50), (3, 5, 64), (3, 5, 66), (5, 18, 100), (4, 7, 258)):
         p = minkowski_params(*n)
         r = rng(n[2])
         shape = (8, n[0] + 6, n[1] + 6, n[2] + 6)
