@@ -25,7 +25,7 @@ def default_params(**kw) -> dict:
         rho_fl_coef=1e-5, rho_fl_pow=-1.5, rho_fl_abs=1e-20,           # eq. 35 (A9)
         u_fl_coef=1e-5 / 3.0, u_fl_pow=-2.5, u_fl_abs=1e-20,
         sigma_max=50.0, b2_over_u_max=2.5e3, gamma_max=50.0,           # eqs. 36-37
-        newton_tol=1e-10, newton_maxit=30, newton_extra=2,             # P:L233 (A8)
+        newton_tol=1e-10, newton_maxit=30, newton_extra=0,             # P:L233 (A8: the paper's literal stopping rule)
         fixup_max_passes=4,
         n_x=0, r_break=0.0,            # hyper-exponential radial branch of eq. 39: off; the paper: 4, 400
     )
