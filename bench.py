@@ -32,7 +32,7 @@ KERNEL_BYTES = {"flux1": 120.0, "flux2": 120.0, "flux3": 120.0, "emf": 72.0, "up
 # From the ncu --set full capture of this command at C4 (profiles/r1d_ncu_summary.md), per launch and averaged over
 # the predictor and corrector launches: DRAM bytes read + written, and fp64 (DFMA/DMUL/DADD/DSETP) warp
 # instructions executed.  Only quoted for the workload they were captured on.
-NCU_C4 = {"update": {"traffic": 6.18e9, "fp64_warp_inst": 3.50e8},
+NCU_C4 = {"update": {"traffic": 6.21e9, "fp64_warp_inst": 3.00e8},
           "flux1": {"traffic": 2.20e9, "fp64_warp_inst": 1.75e8},
           "flux2": {"traffic": 2.19e9, "fp64_warp_inst": 1.75e8},
           "flux3": {"traffic": 2.08e9, "fp64_warp_inst": 1.97e8}}
