@@ -29,13 +29,20 @@ B_ALG = 1218.0          # algorithmic bytes per zone-cycle (DESIGN.
 # emf: read 6 B-fluxes 48, write 3 EMFs 24; update: P^n 64 + hydro fluxes 120 + EMFs 24 (+ P-half 64 in the
 # corrector, averaged: +32) in, 64 + 4 (flag) out
 KERNEL_BYTES = {"flux1": 120.0, "flux2": 120.0, "flux3": 120.0, "emf": 72.0, "update": 332.0}
-# From the ncu --set full capture of this command at C4 (profiles/r1d_ncu_summary.md), per launch and averaged over
-# the predictor and corrector launches: DRAM bytes read + written, and fp64 (DFMA/DMUL/DADD/DSETP) warp
-# instructions executed.  Only quoted for the workload they were captured on.
-NCU_C4 = {"update": {"traffic": 6.21e9, "fp64_warp_inst": 3.00e8},
-          "flux1": {"traffic": 2.20e9, "fp64_warp_inst": 1.75e8},
-          "flux2": {"traffic": 2.19e9, "fp64_warp_inst": 1.75e8},
-          "flux3": {"traffic": 2.08e9, "fp64_warp_inst": 1.97e8}}
+# ncu --set full counters of this command at C4, per launch and averaged over the predictor and corrector launches
+# (DRAM bytes read + written; fp64 DFMA/DMUL/DADD/DSETP warp instructions executed), are READ from the committed
+# summary of the capture, never typed in here.  Only quoted for the workload they were captured on.
+NCU_FILE = os.path.join(ROOT, "profiles", "ncu_c4_counters.json")
+
+
+def ncu_counters():
+    try:
+        d = json.load(open(NCU_FILE))
+        return d["kernels"], d.get("source", os.path.relpath(NCU_FILE, ROOT))
+    except Exception:
+        return {}, None
+
+
 # fp64 pipe: 16 lanes per SM sub-partition = one warp instruction per 2 cycles per sub-partition
 FP64_WARP_INST_PER_S = 148 * 4 * 1.965e9 / 2.0
 
@@ -49,9 +56,12 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / power / throttle reasons sampled every 20 ms while the timed region runs."""
+    """nvidia-smi clocks / power / throttle reasons sampled every 20 ms from before the warm-up until after the last
+    timed region; every row carries its arrival time, so each timed region is summarised over its own window (a
+    0.1 s region still sees the rows that arrived while it ran, plus the nearest one on either side)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
     def __init__(self, index=0):
         self.rows, self.proc, self.index = [], None, index
@@ -67,19 +77,28 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(",")])
+            self.rows.append((time.perf_counter(), [x.strip() for x in line.split(",")]))
 
     def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            self.t.join(timeout=2)
+
+    def window(self, t0, t1):
+        """Summary of the rows that arrived in [t0, t1] (wall clock of this process), widened to the nearest row on
+        either side when fewer than 3 fall inside."""
         if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
-        self.t.join(timeout=2)
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"], "samples": 0}
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1]
+        if len(rows) < 3:
+            before = [r for (t, r) in self.rows if t < t0][-1:]
+            after = [r for (t, r) in self.rows if t > t1][:1]
+            rows = before + rows + after
         sm, mx, pw, reasons = [], [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+        for r in rows:
             try:
                 sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
-                for n, v in zip(names, r[3:7]):
+                for n, v in zip(self.NAMES, r[3:7]):
                     if v.lower().startswith("active"):
                         reasons.add(n)
             except Exception:
@@ -87,7 +106,7 @@ class ClockSampler:
         sm.sort()
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "sm_min_mhz": sm[0] if sm else None, "power_w_max": max(pw) if pw else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm), "window_s": round(t1 - t0, 3)}
 
 
 def aggregate(ms_local, zones, steps, world, dist=None, device="cpu"):
@@ -112,13 +131,14 @@ def make_workload(name, **kw):
     return p, prim
 
 
-def oracle_sample(name, steps, n3_sample=8, threads=None):
-    """The oracle as it stands on a phi-slab of the same torus (same (r,theta) grid and scheme, n3 = n3_sample):
-    returns (zone-cycles/s, cores, description, seconds)."""
+def oracle_sample(name, steps, n3_sample=None, threads=None, prebuilt=None):
+    """The oracle as it stands on the `name` torus (n3_sample: a phi-slab of n3_sample zones of the same (r, theta)
+    grid and scheme; None: the full grid; prebuilt = (params, host array) of that workload, stepped in place):
+    (zone-cycles/s, threads used, description, seconds)."""
     import oracle
-    p, prim = make_workload(name, n3=n3_sample)
-    if threads:
-        oracle.set_threads(threads)
+    kw = {} if n3_sample is None else {"n3": n3_sample}
+    p, prim = prebuilt if prebuilt is not None else make_workload(name, **kw)
+    oracle.set_threads(threads if threads else (os.cpu_count() or 1))
     g = oracle.Grid(p)
     g.bind(prim)
     dt = g.cfl_dt(0.45)
@@ -127,7 +147,10 @@ def oracle_sample(name, steps, n3_sample=8, threads=None):
         g.step(dt)
     sec = time.perf_counter() - t0
     zones = p["n1"] * p["n2"] * p["n3"]
-    return zones * steps / sec, oracle.get_threads(), f"{name} torus, {p['n1']}x{p['n2']}x{p['n3']} phi-slab of the {name} grid, {steps} RK2 steps", sec
+    what = "full grid" if n3_sample is None else f"phi-slab of the {name} grid"
+    used = oracle.get_threads()
+    g.close()
+    return zones * steps / sec, used, f"{name} torus, {p['n1']}x{p['n2']}x{p['n3']} ({what}), {steps} RK2 steps", sec
 
 
 def run_reference(args):
@@ -190,29 +213,32 @@ def run_ours(args):
     dt = s.cfl_dt(0.45)                                   # fixed dt chosen beforehand (eq. 26, xi = 0.45)
     if args.graph:
         s.use_graph(True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()                  # before the warm-up, so that rows exist when a 0.1 s region starts
     for _ in range(args.warmup):
         s.step(dt)
     barrier()
 
     # ---- timed region: K steps, device-resident inputs, CUDA events on the library's stream -----------------
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
     if not args.graph:
         s.set_timing(True)
     l0 = s.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    w0 = time.perf_counter()
     e0.record()
     for _ in range(args.steps):
-        s.step(dt)
-        if args.cfl_each_step:           # second protocol, eq. 26 evaluated (and synchronised) every step;
-            s.last_cfl_dt(0.45)          # the step size itself stays fixed so that the work per step is the same
+        if args.cfl_each_step:           # second protocol -- a new dt every step from eq. 26, taken on the
+            s.step_cfl(0.45)             # device from the previous predictor's face speeds (same graph, no host sync)
+        else:
+            s.step(dt)
     e1.record()
     barrier()
+    w1 = time.perf_counter()
     ms = e0.elapsed_time(e1)
     launches = s.launch_count() - l0
-    clocks = sampler.stop() if rank == 0 else None
+    clocks = sampler.window(w0, w1) if rank == 0 else None
     timing = s.get_timing() if not args.graph else {}
     s.set_timing(False)
     if args.graph:
@@ -231,6 +257,30 @@ def run_ours(args):
     ms, value = aggregate(ms, zones, args.steps, world, dist, "cuda")
     divb = s.divb()[1]
     stats = s.stats()
+
+    # ---- sustained: the metric's own workload is hundreds of steps (BASELINE.json: 500 at C4), long enough for the
+    # board to reach its power cap.  After >= sustain_warm_s seconds of the same load, time >= 300 steps (and >=
+    # sustain_s seconds) the same way; clocks, power and throttle reasons over that window ride along.
+    sustained = None
+    if args.sustain_s > 0:
+        est = ms / args.steps
+        n_warm = max(1, int(args.sustain_warm_s * 1e3 / est))
+        n_sus = max(300, int(args.sustain_s * 1e3 / est))
+        barrier()
+        for _ in range(n_warm):
+            s.step(dt)
+        barrier()
+        ws0 = time.perf_counter()
+        e0.record()
+        for _ in range(n_sus):
+            s.step(dt)
+        e1.record()
+        barrier()
+        ws1 = time.perf_counter()
+        ms_s, val_s = aggregate(e0.elapsed_time(e1), zones, n_sus, world, dist, "cuda")
+        sustained = {"steps": n_sus, "warm_steps": n_warm, "ms_per_step": ms_s / n_sus, "value": val_s, "unit": UNIT,
+                     "seconds": ms_s * 1e-3, "clocks": sampler.window(ws0, ws1) if rank == 0 else None,
+                     "divb_norm": s.divb()[1], "failed_inversions": int(s.stats()[0])}
 
     # ---- e2e: the same step through the public API with HOST buffers: H2D of the primitives from pinned memory,
     # one step, D2H of the result into pinned memory, every step inside the timed region.  Two solver objects on two
@@ -264,9 +314,12 @@ def run_ours(args):
     s2.close()
     ms_e2e, e2e_val = aggregate(ms_e2e, zones, e2e_steps, world, dist, "cuda")
     nbytes = prim_pinned.numel() * 8
+    if rank == 0:
+        sampler.stop()
 
     if rank == 0:
         peak, peak_src, pk = peaks()
+        ncu_all, ncu_src = ncu_counters()
         # dominant kernel class by measured device time
         roof = None
         roof_alu = None
@@ -277,15 +330,16 @@ def run_ours(args):
             dom = max((k for k in KERNEL_BYTES if timing[k][1]), key=lambda k: timing[k][0])
             per_launch_ms = timing[dom][0] / timing[dom][1]
             achieved = KERNEL_BYTES[dom] * zones / (per_launch_ms * 1e-3) / 1e9
-            ncu = NCU_C4.get(dom) if (args.config == "C4" and world == 1) else None
+            ncu = ncu_all.get(dom) if (args.config == "C4" and world == 1) else None
             if ncu:
                 a_alu = ncu["fp64_warp_inst"] / (per_launch_ms * 1e-3)
                 roof_alu = {"bound": "alu", "kernel": dom, "achieved": a_alu, "peak": FP64_WARP_INST_PER_S,
                             "unit": "fp64 warp-instructions/s", "frac": a_alu / FP64_WARP_INST_PER_S,
                             "peak_source": "148 SMs x 4 sub-partitions x 1.965 GHz / 2 cycles per fp64 warp instruction",
-                            "count_source": "ncu, profiles/r1d_ncu_summary.md"}
+                            "count_source": f"ncu, {ncu_src}"}
             roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                    "frac": achieved / peak, "traffic": ncu["traffic"] if ncu else None, "peak_source": peak_src,
+                    "frac": achieved / peak, "traffic": ncu["traffic"] if ncu else None,
+                    "traffic_source": f"ncu --set full, {ncu_src}" if ncu else None, "peak_source": peak_src,
                     "kernel_ms_per_launch": per_launch_ms, "kernel_time_shares": shares,
                     "step_frac_of_hbm_roofline": value / world * B_ALG / (peak * 1e9),
                     "note": "achieved = algorithmic bytes of the dominant kernel class per launch / its mean "
@@ -294,16 +348,26 @@ def run_ours(args):
             roof = {"bound": "hbm", "kernel": "whole step", "achieved": value / world * B_ALG / 1e9,
                     "peak": peak, "unit": "GB/s", "frac": value / world * B_ALG / (peak * 1e9), "traffic": None,
                     "peak_source": peak_src}
+        if sustained is not None:
+            sustained["step_frac_of_hbm_roofline"] = sustained["value"] / world * B_ALG / (peak * 1e9)
         cpu = None
         if not args.no_cpu:
-            v, cores, sample, sec = oracle_sample(args.config, args.cpu_steps, args.ref_n3)
+            # SURVEY 8(d) "CPU baseline": (i) all host cores, full steps of this config; (ii) one core at C3
+            full = None if args.cpu_n3 <= 0 else args.cpu_n3
+            v, cores, sample, sec = oracle_sample(args.config, args.cpu_steps, full,
+                                                  prebuilt=(p, prim_host) if full is None else None)
             cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": sec}
+            v1, c1, sample1, sec1 = oracle_sample("C3", 1, None, threads=1)
+            cpu["single_core"] = {"value": v1, "unit": UNIT, "cores": c1, "kind": "oracle", "sample": sample1, "seconds": sec1}
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                "dtype": "f64", "data": "synthetic",
                "config": {"workload": f"{args.config}: {p['n1']}x{p['n2']}x{p['n3']} MKS Fishbone-Moncrief torus, "
                                       f"a={p['a']}, gam={p['gam']:.4f}, recon={'PPM' if p['recon'] else 'PLM-MC'}, "
-                                      f"riemann={'HLL' if p['riemann'] else 'LLF'}, fixed dt from cfl_dt(0.45)",
+                                      f"riemann={'HLL' if p['riemann'] else 'LLF'}, "
+                                      + ("dt from eq. 26 every step (cuharm_step_cfl, xi = 0.45)" if args.cfl_each_step
+                                         else "fixed dt from cfl_dt(0.45)"),
+                          "newton_tol": p["newton_tol"], "newton_extra": p["newton_extra"], "newton_maxit": p["newton_maxit"],
                           "l2": "inputs larger than L2 (prim 1.15 GB, fluxes 3 GB per substep vs 126 MB L2)",
                           "parallelism": "replicas only" if world > 1 else "single GPU", "graph": bool(args.graph),
                           "cfl_each_step": bool(args.cfl_each_step),
@@ -311,7 +375,8 @@ def run_ours(args):
                "clocks": clocks, "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": nbytes,
                                          "d2h_bytes_per_step": nbytes, "steps": e2e_steps,
                                          "pipeline": "2 solver objects on 2 streams, alternate steps"},
-               "gpu_launches": int(launches), "roofline": roof, "roofline_alu": roof_alu, "cpu_baseline": cpu,
+               "gpu_launches": int(launches), "roofline": roof, "roofline_alu": roof_alu, "sustained": sustained,
+               "cpu_baseline": cpu,
                "checks": {"divb_norm": divb, "stats": stats}}
         print(json.dumps(out), flush=True)
     s.close()
@@ -328,10 +393,13 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--graph", type=int, default=1)
     ap.add_argument("--e2e-steps", type=int, default=6)
-    ap.add_argument("--cpu-steps", type=int, default=3)
-    ap.add_argument("--ref-n3", type=int, default=32)
+    ap.add_argument("--cpu-steps", type=int, default=2, help="cpu_baseline: RK2 steps of the oracle on all host cores")
+    ap.add_argument("--cpu-n3", type=int, default=0, help="cpu_baseline: phi zones of the sample (0 = the full grid)")
+    ap.add_argument("--ref-n3", type=int, default=32, help="--impl reference: phi zones of the per-step sample")
+    ap.add_argument("--sustain-s", type=float, default=3.0, help="sustained leg: at least this many seconds (0 = skip)")
+    ap.add_argument("--sustain-warm-s", type=float, default=2.0, help="sustained leg: load before its timed region")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--cfl-each-step", action="store_true", help="call cuharm_last_cfl_dt (eq. 26) after every step")
+    ap.add_argument("--cfl-each-step", action="store_true", help="a new dt every step from eq. 26 (cuharm_step_cfl)")
     ap.add_argument("--threads", type=int, default=0, help="reference arm: OpenMP threads of the oracle (0 = all)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -13,6 +13,13 @@
  *   - All work is enqueued on the CUDA stream given to cuharm_grid_init.  Only the calls that return host
  *     scalars (cuharm_cfl_dt, cuharm_last_cfl_dt, cuharm_divb, cuharm_get_stats) synchronise that stream.
  *   - There is no CPU fallback: without a CUDA device every compute call returns CUHARM_ECUDA.
+ *   - The context belongs to the CUDA device that is current when cuharm_grid_init is called; every later call
+ *     makes that device current for its own duration and restores the caller's.
+ *   - Geometry: Kerr-Schild in the (diagonal-Jacobian) MKS coordinates of eq. 39, or Minkowski.  The kernels
+ *     store and contract only the metric entries that do not vanish identically there (00 01 03 11 13 22 33 of
+ *     g_{mu nu} and g^{mu nu}; g^{t phi} = 0), use u_i = g_ij utilde^j and beta^2 = beta^3 = 0, and drop the nu = t,
+ *     phi source terms (the metric depends on neither).  `coords` in {0, 1} is the only geometry the library
+ *     accepts; a metric with another zero pattern needs other kernels.
  *
  * Array layout (device, fp64, C order, the last index fastest):
  *   prim[8][n1+2ng][n2+2ng][n3+2ng], variables (rho, u, utilde^1, utilde^2, utilde^3, B^1, B^2, B^3)
@@ -40,7 +47,7 @@ typedef struct cuharm_ctx* cuharm_handle; /* opaque, host side; owns no device m
 /* Plain-old-data parameter block; struct_bytes = sizeof(cuharm_params) guards against layout drift. */
 typedef struct {
   int32_t struct_bytes;
-  int32_t n1, n2, n3, ng; /* interior zones per direction (n3 == 1 allowed); ghost layers, ng >= 3          */
+  int32_t n1, n2, n3, ng; /* interior zones per direction (n3 == 1 allowed); ghost layers, 3 <= ng <= 8     */
   int32_t coords;         /* 0 = MKS (eq. 39; A14); 1 = Minkowski-Cartesian (tests; A39)        */
   double a, gam;          /* black-hole spin (eq. 38); adiabatic index of p = (gam-1) u     */
   double r_in, r_out, R0, hslope; /* MKS: X1 in [ln(r_in-R0), X1(r_out)], X2 in [-1,1], X3 in [0,2pi)         */
@@ -82,12 +89,25 @@ int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_by
  * zones of the bound d_prim.  Errors: ESTATE (not bound). */
 int cuharm_metric_precompute(cuharm_handle h);
 
-/* One full RK2 (midpoint predictor / corrector) step of size dt, in place (eq. 25; A5): each substep
+/* The step size is kept in a device scalar that the kernels read, so one recorded CUDA graph (cuharm_use_graph)
+ * serves every dt.
+ *
+ * One full RK2 (midpoint predictor / corrector) step of size dt, in place (eq. 25; A5): each substep
  * = reconstruction (eqs. 15-16 / PPM) -> LLF/HLL face fluxes (eqs. 17-20) -> flux-CT (eqs. 21-22; A3) -> source
  * (eq. 14) -> update -> Noble 2D inversion (eqs. 27-31; A6-A8) -> floors (eqs. 35-37) -> ghost fill -> repair of
  * failed zones (eq. 34; A13) -> ghost fill.  d_prim has valid ghosts on entry and on exit.  Asynchronous.
  * Errors: ESTATE (not bound / no geometry), EINVAL (dt not finite or <= 0). */
 int cuharm_step(cuharm_handle h, double dt);
+
+/* The same step with dt taken ON THE DEVICE from eq. 26 (A17) applied to the face speeds the predictor
+ * of the previous step saw ("the next time step"): dt = min(dt_max, 1 / sum_l max c_w^l / (xi dx^l))
+ * (dt_max <= 0: no cap) -- the value cuharm_last_cfl_dt would return, bit for bit, without the read-back and the
+ * synchronisation.  Asynchronous.  Errors: ESTATE (no previous step since bind), EINVAL (xi not finite or <= 0). */
+int cuharm_step_cfl(cuharm_handle h, double xi, double dt_max);
+
+/* Integrated time since cuharm_bind (*t, the sum of the step sizes) and the size of the last step (*dt_last);
+ * either pointer may be NULL.  HOST pointers.  Synchronises. */
+int cuharm_get_time(cuharm_handle h, double* t, double* dt_last);
 
 /* Pure inversion (eqs. 27-31) on full-grid arrays of the prim layout: d_U holds the 8 conserved variables
  * sqrt(-g)(rho u^t, T^t_t, T^t_i, B^i) (A18); d_prim_inout carries the Newton guess in and the answer out;
@@ -99,7 +119,8 @@ int cuharm_cons_to_prim(cuharm_handle h, const double* d_U, double* d_prim_inout
 int cuharm_prim_to_cons(cuharm_handle h, const double* d_prim, double* d_U);
 
 /* Time step of eq. 26 (A17) from the bound primitives: dt^l = xi dx^l / max_faces c_w^l,
- * 1/dt = sum_l 1/dt^l.  Overwrites the flux workspace.  Synchronises. */
+ * 1/dt = sum_l 1/dt^l.  Overwrites the flux workspace.  Synchronises.  *dt_out = 0 if a wave speed anywhere is
+ * not finite (physics trouble is not an error code; cuharm_step rejects dt = 0). */
 int cuharm_cfl_dt(cuharm_handle h, double xi, double* dt_out);
 
 /* Same formula from the face speeds the predictor of the last cuharm_step saw ("the next time step",
@@ -127,6 +148,12 @@ int cuharm_get_geom(cuharm_handle h, int32_t loc, double* d_out);
 
 /* Fill the ghost zones of an arbitrary primitive array of the bound shape.  Asynchronous. */
 int cuharm_apply_bc(cuharm_handle h, double* d_prim);
+
+/* Floors, ceilings and Lorentz cap (eqs. 35-37; A9-A12) as a stage of their own on the interior zones
+ * of an arbitrary primitive array of the bound shape, in place; d_mask[zone] (int32, [n1g][n2g][n3g], may be NULL)
+ * = bit mask: 1 rho floor, 2 u floor, 4 ceiling applied, 8 Lorentz cap, 16 ceiling re-inversion failed.  Test
+ * helper.  Asynchronous. */
+int cuharm_apply_floors(cuharm_handle h, double* d_prim, int32_t* d_mask);
 
 /* Stage-level test helpers (asynchronous; arrays have the prim layout unless stated):
  * face fluxes of direction dir (1..3) BEFORE flux-CT, d_F[8][zones] stored at the zone whose LOWER dir-face it

@@ -1300,6 +1300,24 @@ int oracle_get_flags(oracle_handle h, int32_t* out) {
   return 0;
 }
 
+// stage-level: floors / ceilings / Lorentz cap (C-12) on every interior zone of a caller-provided primitive array,
+// in place; mask[zone] = apply_floors' bit mask (may be null)
+int oracle_apply_floors_grid(oracle_handle h, double* prim, int32_t* mask) {
+  Ctx& c = h->c;
+  const int ng = c.ng;
+  for (int i = ng; i < ng + c.p.n1; i++)
+    for (int j = ng; j < ng + c.p.n2; j++)
+      for (int k = ng; k < ng + c.p.n3; k++) {
+        size_t g2 = (size_t)i * c.n2g + j;
+        double q[8];
+        get_prim(c, prim, i, j, k, q);
+        int m = apply_floors(c.p, c.rc[g2], c.gc[g2], q);
+        for (int v = 0; v < 8; v++) prim[c.vidx(v, i, j, k)] = q[v];
+        if (mask) mask[c.idx(i, j, k)] = m;
+      }
+  return 0;
+}
+
 // stage-level: fix-up on a caller-provided primitive array with caller-provided flags
 int oracle_fixup(oracle_handle h, double* prim, const int32_t* flag) {
   Ctx& c = h->c;

@@ -282,6 +282,13 @@ class Grid:
         lib().oracle_get_flags(self._h, out.ctypes.data_as(_ip))
         return out
 
+    def apply_floors(self, prim):
+        """C-12 on every interior zone of prim, in place; returns the per-zone bit mask."""
+        assert prim.dtype == np.float64 and prim.flags.c_contiguous and prim.shape == (8,) + self.shape
+        mask = np.zeros(self.shape, dtype=np.int32)
+        lib().oracle_apply_floors_grid(self._h, _d(prim), mask.ctypes.data_as(_ip))
+        return mask
+
     def fixup(self, prim, flag):
         assert prim.dtype == np.float64 and prim.flags.c_contiguous
         flag = np.ascontiguousarray(flag, dtype=np.int32)

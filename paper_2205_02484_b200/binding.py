@@ -66,6 +66,9 @@ def lib():
         L.cuharm_bind.argtypes = [vp, dp, vp, C.c_size_t]
         L.cuharm_metric_precompute.argtypes = [vp]
         L.cuharm_step.argtypes = [vp, C.c_double]
+        L.cuharm_step_cfl.argtypes = [vp, C.c_double, C.c_double]
+        L.cuharm_get_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.cuharm_apply_floors.argtypes = [vp, dp, ip]
         L.cuharm_cons_to_prim.argtypes = [vp, dp, dp, ip]
         L.cuharm_prim_to_cons.argtypes = [vp, dp, dp]
         L.cuharm_cfl_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
@@ -129,6 +132,21 @@ def cuharm_metric_precompute(h):
 
 def cuharm_step(h, dt: float):
     _check(lib().cuharm_step(h, float(dt)), "cuharm_step")
+
+
+def cuharm_step_cfl(h, xi: float, dt_max: float = 0.0):
+    _check(lib().cuharm_step_cfl(h, float(xi), float(dt_max)), "cuharm_step_cfl")
+
+
+def cuharm_get_time(h):
+    """(integrated time since bind, size of the last step)."""
+    t, dt = C.c_double(), C.c_double()
+    _check(lib().cuharm_get_time(h, C.byref(t), C.byref(dt)), "cuharm_get_time")
+    return t.value, dt.value
+
+
+def cuharm_apply_floors(h, prim, mask=None):
+    _check(lib().cuharm_apply_floors(h, _dptr(prim), _dptr(mask)), "cuharm_apply_floors")
 
 
 def cuharm_cons_to_prim(h, U, prim_inout, flag=None):
@@ -241,6 +259,8 @@ class Solver:
         cuharm_bind(self.h, self.prim, self.workspace)
 
     def step(self, dt): cuharm_step(self.h, dt)
+    def step_cfl(self, xi, dt_max=0.0): cuharm_step_cfl(self.h, xi, dt_max)
+    def time(self): return cuharm_get_time(self.h)
     def cfl_dt(self, xi): return cuharm_cfl_dt(self.h, xi)
     def last_cfl_dt(self, xi): return cuharm_last_cfl_dt(self.h, xi)
     def divb(self): return cuharm_divb(self.h)
@@ -279,6 +299,12 @@ class Solver:
         return F, cw
 
     def apply_bc(self, prim): cuharm_apply_bc(self.h, prim)
+
+    def apply_floors(self, prim):
+        import torch
+        mask = torch.zeros(self.shape[1:], dtype=torch.int32, device=self.device)
+        cuharm_apply_floors(self.h, prim, mask)
+        return mask
 
     def close(self):
         if getattr(self, "h", None):

@@ -33,7 +33,8 @@ int cuda_fail(cudaError_t e, const char* what) {
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 // counters block (unsigned long long slots)
-enum { CNT_STATS = 0, CNT_NFAIL = 8, CNT_CWPRED = 10, CNT_CWSCR = 13, CNT_DIVB = 16, CNT_TOTAL = 32 };
+enum { CNT_STATS = 0, CNT_NFAIL = 8, CNT_CWPRED = 10, CNT_CWSCR = 13, CNT_DIVB = 16, CNT_CLOCK = 18, CNT_TOTAL = 32 };
+// CNT_CLOCK: two doubles, the step size of the current step and the integrated time (set_dt_kernel, dt_from_cw_kernel)
 
 }  // namespace
 
@@ -41,6 +42,7 @@ struct cuharm_ctx {
   cuharm_params p;
   Dims d;
   cudaStream_t stream;
+  int dev = 0;  // CUDA device the context was created on; every entry point runs with it current
   double dx[3], x0[3];
   // borrowed device memory
   double* prim = nullptr;
@@ -70,13 +72,23 @@ struct cuharm_ctx {
   cudaStream_t cap_stream = nullptr;
   cudaStream_t side[2] = {nullptr, nullptr};  // branches of the recorded graph (flux kernels of directions 2, 3)
   cudaEvent_t fj[3] = {nullptr, nullptr, nullptr};  // fork / join events of those branches
-  double graph_dt = 0.0;
   int64_t graph_nodes = 0;
 };
 
-#ifndef CUHARM_UPD_STRIP
-#define CUHARM_UPD_STRIP 8
-#endif
+// update_tma_kernel: tiles are ordered in strips of this many rows j (shared rows are then re-read from L2)
+constexpr int UPD_STRIP = 8;
+
+// Makes the context's device current for the duration of an entry point and restores the caller's.
+struct DevGuard {
+  int prev = -1;
+  bool changed = false;
+  explicit DevGuard(const cuharm_ctx* h) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != h->dev) changed = cudaSetDevice(h->dev) == cudaSuccess;
+  }
+  ~DevGuard() {
+    if (changed) cudaSetDevice(prev);
+  }
+};
 
 namespace {
 
@@ -130,38 +142,15 @@ struct Timed {
 int launch_bc(cuharm_ctx* h, double* P, const unsigned long long* gate) {
   Timed t_(h, CUHARM_K_BC);
   const Dims& d = h->d;
-#ifndef CUHARM_BC_SEPARATE
-  {  // one launch for the whole ghost fill (bit-identical to the three-kernel sequence below)
-    if (h->p.bc_x1 == 3 && h->p.bc_x2 == 3 && h->p.bc_x3 == 3) return CUHARM_OK;
-    const int nrows_a = d.n1g * d.n2g - d.n1 * d.n2;
-    const int kchunks = (d.n3g + 127) / 128;
-    const int per = 128 / (2 * d.ng);
-    const long long nb = (long long)nrows_a * kchunks + ((long long)d.n1 * d.n2 + per - 1) / per;
-    BcAllArgs b{d, P, h->gC, h->p.bc_x1, h->p.bc_x2, h->p.bc_x3, h->p.coords, h->p.gamma_max, gate, nrows_a};
-    bc_all_kernel<<<(unsigned)nb, 128, 0, h->stream>>>(b);
-    h->launches++;
-    CK(cudaGetLastError());
-    return CUHARM_OK;
-  }
-#endif
-  BcArgs a{d, P, h->gC, 0, h->p.coords, h->p.gamma_max, gate};
-  const int T = 128;
-  if (h->p.bc_x1 != 3) {
-    a.kind = h->p.bc_x1;
-    bc_x1_kernel<<<dim3((d.n3g + T - 1) / T, d.n2g, 2 * d.ng), T, 0, h->stream>>>(a);
-    h->launches++;
-  }
-  if (h->p.bc_x2 != 3) {
-    a.kind = h->p.bc_x2;
-    bc_x2_kernel<<<dim3((d.n3g + T - 1) / T, d.n1g, 2 * d.ng), T, 0, h->stream>>>(a);
-    h->launches++;
-  }
-  if (h->p.bc_x3 != 3) {
-    a.kind = h->p.bc_x3;
-    const long long n = (long long)d.n1g * d.n2g * 2 * d.ng;
-    bc_x3_kernel<<<(unsigned)((n + T - 1) / T), T, 0, h->stream>>>(a);
-    h->launches++;
-  }
+  // one launch for the whole ghost fill (the composition of the X1 -> X2 -> X3 fills, cuharm_kernels.cuh)
+  if (h->p.bc_x1 == 3 && h->p.bc_x2 == 3 && h->p.bc_x3 == 3) return CUHARM_OK;
+  const int nrows_a = d.n1g * d.n2g - d.n1 * d.n2;
+  const int kchunks = (d.n3g + 127) / 128;
+  const int per = 128 / (2 * d.ng);
+  const long long nb = (long long)nrows_a * kchunks + ((long long)d.n1 * d.n2 + per - 1) / per;
+  BcAllArgs b{d, P, h->gC, h->p.bc_x1, h->p.bc_x2, h->p.bc_x3, h->p.coords, h->p.gamma_max, gate, nrows_a};
+  bc_all_kernel<<<(unsigned)nb, 128, 0, h->stream>>>(b);
+  h->launches++;
   CK(cudaGetLastError());
   return CUHARM_OK;
 }
@@ -218,9 +207,6 @@ void launch_flux_t(cuharm_ctx* h, FluxArgs& a, int dir) {
     const int nt = dir == 1 ? nj : ni;
     a.geo_rows = std::min(nt, 127 / nk + 2);
     size_t gsm = (size_t)a.geo_rows * a.seg * sizeof(Geom);
-#ifdef CUHARM_NO_GEO_STAGE
-    gsm = 1 << 30;
-#endif
     if (gsm > 40 * 1024) { a.geo_rows = 0; gsm = 0; }
     if (a.geo_rows > 0) {
       if (dir == 1) flux_march_kernel<1, RECON, RIEMANN, STAGE, true><<<grid, 128, gsm, h->stream>>>(a);
@@ -256,14 +242,13 @@ int launch_flux(cuharm_ctx* h, const double* P, int dir, double* F, double* cw, 
 }
 
 // one RK2 substep (A34 order): fluxes -> EMFs -> update+inversion+floors -> ghost fill -> repair -> ghost fill
-int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pout, double dtau, int which) {
+int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pout, double dtfac, int which) {
   const Dims& d = h->d;
   unsigned long long* cwmax = h->cnt + (which == 0 ? CNT_CWPRED : CNT_CWSCR);
   // The three flux kernels are independent of one another.  While a graph is being recorded they go on three
   // branches (fork / join through events), so that the drain of one overlaps the ramp-up of the next; launched
   // directly they stay in stream order (that is also the mode in which per-kernel events time them).
   bool fork = false;
-#ifndef CUHARM_NO_FORK
   if (h->capturing) {
     fork = true;
     for (int s = 0; s < 2 && fork; s++)
@@ -272,17 +257,12 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
       if (!h->fj[e] && cudaEventCreateWithFlags(&h->fj[e], cudaEventDisableTiming) != cudaSuccess) fork = false;
     if (!fork) cudaGetLastError();
   }
-#endif
   if (fork) {
     cudaStream_t main_s = h->stream;
     CK(cudaEventRecord(h->fj[0], main_s));
-#ifndef CUHARM_FORK_ORDER
-#define CUHARM_FORK_ORDER 1
-#endif
     // launch order of the three directions (main branch first); measured best on B200: the persistent X3 kernel
     // first, the many-block marching kernels fill in behind it
-    static const int order[3][3] = {{1, 2, 3}, {3, 1, 2}, {1, 3, 2}};
-    const int* od = order[CUHARM_FORK_ORDER];
+    static const int od[3] = {3, 1, 2};
     int rc = launch_flux<false>(h, Pflux, od[0], h->F[od[0] - 1], nullptr, cwmax + od[0] - 1);
     for (int s = 0; s < 2 && !rc; s++) {
       CK(cudaStreamWaitEvent(h->side[s], h->fj[0], 0));
@@ -303,7 +283,8 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
   // That kernel evaluates the edge EMFs itself (flux-CT fused); otherwise they go through emf_kernel and h->E.
   const uintptr_t al = (uintptr_t)Pbase | (uintptr_t)Pflux | (uintptr_t)h->F[0] | (uintptr_t)h->F[1] |
                        (uintptr_t)h->F[2] | (uintptr_t)h->E;
-  const bool tma = h->upd_tma && (d.n3g % 2 == 0) && (al % 16 == 0);
+  // (the staged row starts one zone below the tile, at ng - 1 + c TB: 16-byte aligned only for odd ng)
+  const bool tma = h->upd_tma && (d.n3g % 2 == 0) && (d.ng % 2 == 1) && (al % 16 == 0);
   if (!tma) {
     Timed t_(h, CUHARM_K_EMF);
     EmfArgs a{d, h->F[0], h->F[1], h->F[2], h->E};
@@ -314,7 +295,7 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
   {
     Timed t_(h, CUHARM_K_UPDATE);
     UpdArgs a{d, Pbase, Pflux, Pout, h->F[0], h->F[1], h->F[2], h->E, h->gC, h->conn, h->floors, h->flag, h->list,
-              nfail, h->cnt + CNT_STATS, dtau, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], h->p.gam,
+              nfail, h->cnt + CNT_STATS, reinterpret_cast<const double*>(h->cnt + CNT_CLOCK), dtfac, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], h->p.gam,
               newton_cfg(h->p), floor_cfg(h->p)};
     dim3 grid((d.n3 + 127) / 128, d.n2, d.n1);
     if (tma) {
@@ -324,8 +305,8 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
       const long long nt = (long long)d.n1 * d.n2 * nch;
       const int ntiles = (int)nt;
       const int nb = (int)std::min<long long>(nt, tb == 64 ? h->upd_blocks64 : h->upd_blocks);
-      int wj = 1;  // strip width: the largest divisor of n2 not above CUHARM_UPD_STRIP
-      for (int w = 1; w <= CUHARM_UPD_STRIP && w <= d.n2; w++)
+      int wj = 1;  // strip width: the largest divisor of n2 not above UPD_STRIP
+      for (int w = 1; w <= UPD_STRIP && w <= d.n2; w++)
         if (d.n2 % w == 0) wj = w;
       const bool same = Pflux == Pbase;
       if (tb == 64) {
@@ -355,12 +336,45 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
   return launch_bc(h, Pout, nfail);
 }
 
-int enqueue_step(cuharm_ctx* h, double dt) {
+// the step size is read by the kernels from the device scalar cnt[CNT_CLOCK] (written just before by set_dt_kernel or
+// dt_from_cw_kernel), so this sequence -- and the graph recorded from it -- is the same for every dt
+int enqueue_step(cuharm_ctx* h) {
   // per-step counters: failure counts of the two substeps, the c_w maxima of predictor and corrector
   CK(cudaMemsetAsync(h->cnt + CNT_NFAIL, 0, (CNT_DIVB - CNT_NFAIL) * sizeof(unsigned long long), h->stream));
-  int rc = substep(h, h->prim, h->prim, h->Phalf, 0.5 * dt, 0);  // predictor: fluxes and source from P^n
+  int rc = substep(h, h->prim, h->prim, h->Phalf, 0.5, 0);  // predictor: fluxes and source from P^n, dtau = dt/2
   if (rc) return rc;
-  return substep(h, h->Phalf, h->prim, h->prim, dt, 1);          // corrector: from the half-step state, in place
+  return substep(h, h->Phalf, h->prim, h->prim, 1.0, 1);    // corrector: from the half-step state, in place, dtau = dt
+}
+
+// one step with the step size already in the device scalar: plain launches, or replay of the recorded graph
+int run_step(cuharm_ctx* h) {
+  h->stepped = true;
+  if (!h->use_graph) return enqueue_step(h);
+  if (!h->gexec) {  // record once; dt is not part of the graph
+    cudaGraph_t g = nullptr;
+    const int64_t before = h->launches;
+    // record on a private stream (the caller's may be the legacy default stream, which cannot be captured);
+    // the instantiated graph is then launched on the caller's stream
+    if (!h->cap_stream) CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+    cudaStream_t user = h->stream;
+    CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+    h->stream = h->cap_stream;
+    h->capturing = true;
+    int rc = enqueue_step(h);
+    h->capturing = false;
+    h->stream = user;
+    cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);  // also ends a capture that failed half way
+    h->graph_nodes = h->launches - before;
+    h->launches = before;
+    if (rc) { if (g) cudaGraphDestroy(g); (void)cudaGetLastError(); return rc; }
+    if (e != cudaSuccess) { if (g) cudaGraphDestroy(g); return cuda_fail(e, "cudaStreamEndCapture"); }
+    e = cudaGraphInstantiate(&h->gexec, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { h->gexec = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
+  }
+  CK(cudaGraphLaunch(h->gexec, h->stream));
+  h->launches += h->graph_nodes;
+  return CUHARM_OK;
 }
 
 int check_params(const cuharm_params* p) {
@@ -400,6 +414,10 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
   if (!h) return CUHARM_ENOMEM;
   h->p = *p;
   h->stream = (cudaStream_t)cuda_stream;
+  {  // the device current at creation owns the stream and every later launch
+    const cudaError_t e = cudaGetDevice(&h->dev);
+    if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaGetDevice"); }
+  }
   Dims& d = h->d;
   d.n1 = p->n1; d.n2 = p->n2; d.n3 = p->n3; d.ng = p->ng;
   d.n1g = p->n1 + 2 * p->ng; d.n2g = p->n2 + 2 * p->ng; d.n3g = p->n3 + 2 * p->ng;
@@ -457,13 +475,6 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
       if (sms > 0) h->sms = sms;
     }
-#ifdef CUHARM_NO_ROW
-    h->fluxk_row = false;
-#endif
-#ifdef CUHARM_NO_TMA
-    h->upd_tma = false;
-    h->fluxk_row = false;
-#endif
   }
   *out = h;
   return CUHARM_OK;
@@ -476,7 +487,9 @@ int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_by
   if (((uintptr_t)d_workspace & 255) || ((uintptr_t)d_prim & 15)) return CUHARM_EINVAL;
   const WsLayout L = layout(h->d);
   if (ws_bytes < L.total) return CUHARM_ENOMEM;
+  DevGuard dg_(h);
   const bool same_ws = h->ws == (char*)d_workspace;
+  const bool same_prim = h->prim == d_prim;
   h->prim = d_prim;
   h->ws = (char*)d_workspace;
   h->gC = (Geom*)(h->ws + L.gC); h->gF1 = (Geom*)(h->ws + L.gF1); h->gF2 = (Geom*)(h->ws + L.gF2);
@@ -486,7 +499,8 @@ int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_by
   h->flag = (int*)(h->ws + L.flag); h->list = (int*)(h->ws + L.list);
   h->cnt = (unsigned long long*)(h->ws + L.cnt);
   if (!same_ws) h->have_geom = false;
-  if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+  // a recorded graph holds the array addresses: it stays valid only if both are unchanged
+  if (h->gexec && !(same_ws && same_prim)) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
   h->bound = true;
   h->stepped = false;
   CK(cudaMemsetAsync(h->flag, 0, (size_t)h->d.nz * sizeof(int), h->stream));  // ghost zones always count as good
@@ -503,6 +517,7 @@ int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_by
 int cuharm_metric_precompute(cuharm_handle h) {
   if (!h) return CUHARM_EINVAL;
   if (!h->bound) return CUHARM_ESTATE;
+  DevGuard dg_(h);
   const cuharm_params& p = h->p;
   const Dims& d = h->d;
   GeomArgs a{d.n1g, d.n2g, d.ng, d.n2, p.coords, (p.coords == 0 && p.bc_x2 == 2) ? 1 : 0, p.a, p.R0, p.hslope,
@@ -523,39 +538,39 @@ int cuharm_step(cuharm_handle h, double dt) {
   if (!h) return CUHARM_EINVAL;
   if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
   if (!(dt > 0.0) || !std::isfinite(dt)) return CUHARM_EINVAL;
-  h->stepped = true;
-  if (!h->use_graph) return enqueue_step(h, dt);
-  if (!h->gexec || h->graph_dt != dt) {  // (re)capture: dt is baked into the kernel arguments
-    if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
-    cudaGraph_t g = nullptr;
-    const int64_t before = h->launches;
-    // record on a private stream (the caller's may be the legacy default stream, which cannot be captured);
-    // the instantiated graph is then launched on the caller's stream
-    if (!h->cap_stream) CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
-    cudaStream_t user = h->stream;
-    CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
-    h->stream = h->cap_stream;
-    h->capturing = true;
-    int rc = enqueue_step(h, dt);
-    h->capturing = false;
-    h->stream = user;
-    cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
-    h->graph_nodes = h->launches - before;
-    h->launches = before;
-    if (rc) { if (g) cudaGraphDestroy(g); return rc; }
-    if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
-    e = cudaGraphInstantiate(&h->gexec, g, 0);
-    cudaGraphDestroy(g);
-    if (e != cudaSuccess) { h->gexec = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
-    h->graph_dt = dt;
-  }
-  CK(cudaGraphLaunch(h->gexec, h->stream));
-  h->launches += h->graph_nodes;
+  DevGuard dg_(h);
+  set_dt_kernel<<<1, 1, 0, h->stream>>>(reinterpret_cast<double*>(h->cnt + CNT_CLOCK), dt);
+  h->launches++;
+  CK(cudaGetLastError());
+  return run_step(h);
+}
+
+int cuharm_step_cfl(cuharm_handle h, double xi, double dt_max) {
+  if (!h || !(xi > 0.0) || !std::isfinite(xi) || dt_max != dt_max) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom || !h->stepped) return CUHARM_ESTATE;
+  DevGuard dg_(h);
+  dt_from_cw_kernel<<<1, 1, 0, h->stream>>>(reinterpret_cast<double*>(h->cnt + CNT_CLOCK), h->cnt + CNT_CWPRED, xi, h->dx[0],
+                                            h->dx[1], h->dx[2], dt_max);
+  h->launches++;
+  CK(cudaGetLastError());
+  return run_step(h);
+}
+
+int cuharm_get_time(cuharm_handle h, double* t, double* dt_last) {
+  if (!h || (!t && !dt_last)) return CUHARM_EINVAL;
+  if (!h->bound) return CUHARM_ESTATE;
+  DevGuard dg_(h);
+  double c[2];
+  CK(cudaMemcpyAsync(c, h->cnt + CNT_CLOCK, sizeof(c), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  if (dt_last) *dt_last = c[0];
+  if (t) *t = c[1];
   return CUHARM_OK;
 }
 
 int cuharm_use_graph(cuharm_handle h, int32_t on) {
   if (!h) return CUHARM_EINVAL;
+  DevGuard dg_(h);
   h->use_graph = on != 0;
   if (!on && h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
   return CUHARM_OK;
@@ -565,6 +580,7 @@ int64_t cuharm_launch_count(cuharm_handle h) { return h ? h->launches : 0; }
 
 int cuharm_set_timing(cuharm_handle h, int32_t on) {
   if (!h) return CUHARM_EINVAL;
+  DevGuard dg_(h);
   if (on && h->ev.empty()) {
     h->ev.resize(2 * 8192);
     for (auto& e : h->ev) CK(cudaEventCreate(&e));
@@ -578,6 +594,7 @@ int cuharm_set_timing(cuharm_handle h, int32_t on) {
 
 int cuharm_get_timing(cuharm_handle h, double ms[CUHARM_NCLASS], int64_t count[CUHARM_NCLASS]) {
   if (!h || !ms || !count) return CUHARM_EINVAL;
+  DevGuard dg_(h);
   CK(cudaStreamSynchronize(h->stream));
   for (size_t q = 0; q + 1 < h->ev_used; q += 2) {
     float t = 0.f;
@@ -595,6 +612,7 @@ int cuharm_get_timing(cuharm_handle h, double ms[CUHARM_NCLASS], int64_t count[C
 int cuharm_cons_to_prim(cuharm_handle h, const double* d_U, double* d_prim_inout, int32_t* d_flag) {
   if (!h || !d_U || !d_prim_inout) return CUHARM_EINVAL;
   if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  DevGuard dg_(h);
   const Dims& d = h->d;
   ConvArgs a{d, d_U, d_prim_inout, d_flag, h->gC, h->p.gam, newton_cfg(h->p)};
   cons_to_prim_kernel<<<dim3((d.n3g + 127) / 128, d.n2g, d.n1g), 128, 0, h->stream>>>(a);
@@ -606,6 +624,7 @@ int cuharm_cons_to_prim(cuharm_handle h, const double* d_U, double* d_prim_inout
 int cuharm_prim_to_cons(cuharm_handle h, const double* d_prim, double* d_U) {
   if (!h || !d_prim || !d_U) return CUHARM_EINVAL;
   if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  DevGuard dg_(h);
   const Dims& d = h->d;
   ConvArgs a{d, d_prim, d_U, nullptr, h->gC, h->p.gam, newton_cfg(h->p)};
   prim_to_cons_kernel<<<dim3((d.n3g + 127) / 128, d.n2g, d.n1g), 128, 0, h->stream>>>(a);
@@ -625,13 +644,15 @@ static int dt_from_cw(cuharm_handle h, const unsigned long long* d_cw, double xi
     const double dtl = xi * h->dx[c] / cw;  // dt^l = xi dx^l / max c_w
     inv += 1.0 / dtl;                       // eq. 26
   }
-  *dt_out = 1.0 / inv;
+  const double dt = 1.0 / inv;
+  *dt_out = std::isfinite(dt) && dt > 0.0 ? dt : 0.0;  // a non-finite wave speed anywhere (a NaN enters as +inf): 0
   return CUHARM_OK;
 }
 
 int cuharm_cfl_dt(cuharm_handle h, double xi, double* dt_out) {
   if (!h || !dt_out || !(xi > 0.0)) return CUHARM_EINVAL;
   if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  DevGuard dg_(h);
   unsigned long long* cw = h->cnt + CNT_CWSCR;
   CK(cudaMemsetAsync(cw, 0, 3 * sizeof(unsigned long long), h->stream));
   for (int dir = 1; dir <= 3; dir++) {
@@ -644,6 +665,7 @@ int cuharm_cfl_dt(cuharm_handle h, double xi, double* dt_out) {
 int cuharm_last_cfl_dt(cuharm_handle h, double xi, double* dt_out) {
   if (!h || !dt_out || !(xi > 0.0)) return CUHARM_EINVAL;
   if (!h->bound || !h->have_geom || !h->stepped) return CUHARM_ESTATE;
+  DevGuard dg_(h);
   return dt_from_cw(h, h->cnt + CNT_CWPRED, xi, dt_out);
 }
 
@@ -652,6 +674,7 @@ int cuharm_shell_fluxes(cuharm_handle h, int32_t i, double out[4]) {
   if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
   const Dims& d = h->d;
   if (i < 0 || i >= d.n1) return CUHARM_EINVAL;
+  DevGuard dg_(h);
   // scratch: the head of the EMF array (idle between steps): n2 x 4 partial sums + 4 results
   double* partial = h->E;
   double* res = h->E + (size_t)d.n2 * 4;
@@ -669,6 +692,7 @@ int cuharm_divb(cuharm_handle h, double* max_abs, double* max_norm) {
   if (!h || !max_abs || !max_norm) return CUHARM_EINVAL;
   if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
   const Dims& d = h->d;
+  DevGuard dg_(h);
   const bool two_d = d.n3 == 1;
   const int khi = two_d ? d.ng : ((h->p.bc_x3 == 1) ? d.ng + d.n3 - 1 : d.ng + d.n3 - 2);
   unsigned long long* out = h->cnt + CNT_DIVB;
@@ -690,6 +714,7 @@ int cuharm_divb(cuharm_handle h, double* max_abs, double* max_norm) {
 int cuharm_get_geom(cuharm_handle h, int32_t loc, double* d_out) {
   if (!h || !d_out || loc < 0 || loc > 3) return CUHARM_EINVAL;
   if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  DevGuard dg_(h);
   const int n = h->d.n1g * h->d.n2g;
   const Geom* tab = loc == 1 ? h->gF1 : (loc == 2 ? h->gF2 : h->gC);
   geom_export_kernel<<<(n + 127) / 128, 128, 0, h->stream>>>(tab, h->conn, loc, n, d_out);
@@ -701,12 +726,26 @@ int cuharm_get_geom(cuharm_handle h, int32_t loc, double* d_out) {
 int cuharm_apply_bc(cuharm_handle h, double* d_prim) {
   if (!h || !d_prim) return CUHARM_EINVAL;
   if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  DevGuard dg_(h);
   return launch_bc(h, d_prim, nullptr);
+}
+
+int cuharm_apply_floors(cuharm_handle h, double* d_prim, int32_t* d_mask) {
+  if (!h || !d_prim) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  DevGuard dg_(h);
+  const Dims& d = h->d;
+  FloorArgs a{d, d_prim, d_mask, h->gC, h->floors, h->p.gam, newton_cfg(h->p), floor_cfg(h->p)};
+  floors_kernel<<<dim3((d.n3 + 127) / 128, d.n2, d.n1), 128, 0, h->stream>>>(a);
+  h->launches++;
+  CK(cudaGetLastError());
+  return CUHARM_OK;
 }
 
 int cuharm_flux_dir(cuharm_handle h, const double* d_prim, int32_t dir, double* d_F, double* d_cw) {
   if (!h || !d_prim || !d_F || dir < 1 || dir > 3) return CUHARM_EINVAL;
   if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  DevGuard dg_(h);
   CK(cudaMemsetAsync(d_F, 0, 8 * (size_t)h->d.nz * sizeof(double), h->stream));
   if (d_cw) CK(cudaMemsetAsync(d_cw, 0, (size_t)h->d.nz * sizeof(double), h->stream));
   return launch_flux<true>(h, d_prim, dir, d_F, d_cw, h->cnt + CNT_CWSCR + (dir - 1));
@@ -715,6 +754,7 @@ int cuharm_flux_dir(cuharm_handle h, const double* d_prim, int32_t dir, double* 
 int cuharm_get_stats(cuharm_handle h, int64_t out[8]) {
   if (!h || !out) return CUHARM_EINVAL;
   if (!h->bound) return CUHARM_ESTATE;
+  DevGuard dg_(h);
   CK(cudaMemcpyAsync(out, h->cnt + CNT_STATS, 8 * sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
   return CUHARM_OK;
@@ -722,11 +762,14 @@ int cuharm_get_stats(cuharm_handle h, int64_t out[8]) {
 
 int cuharm_destroy(cuharm_handle h) {
   if (!h) return CUHARM_EINVAL;
+  {
+  DevGuard dg_(h);
   if (h->gexec) cudaGraphExecDestroy(h->gexec);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   for (int k = 0; k < 2; k++) if (h->side[k]) cudaStreamDestroy(h->side[k]);
   for (int k = 0; k < 3; k++) if (h->fj[k]) cudaEventDestroy(h->fj[k]);
   for (auto& e : h->ev) cudaEventDestroy(e);
+  }
   delete h;
   return CUHARM_OK;
 }

@@ -36,9 +36,11 @@ __device__ __forceinline__ unsigned long long warp_max_ull(unsigned long long v)
 }
 
 // max of non-negative doubles through their order-preserving integer image; no floating-point atomics anywhere.
-// Must be reached by all 32 lanes of the warp.
+// A NaN enters as +infinity, so that it is never lost: a non-finite wave speed anywhere makes the eq. 26 time step 0
+// (cuharm_cfl_dt and friends return dt = 0, which cuharm_step rejects).  Must be reached by all 32 lanes of the warp.
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* addr, double v) {
-  const unsigned long long m = warp_max_ull((unsigned long long)__double_as_longlong(v >= 0.0 ? v : 0.0));
+  const double vv = v >= 0.0 ? v : (v != v ? __longlong_as_double(0x7ff0000000000000LL) : 0.0);
+  const unsigned long long m = warp_max_ull((unsigned long long)__double_as_longlong(vv));
   if ((threadIdx.x & 31) == 0 && m > *reinterpret_cast<volatile unsigned long long*>(addr)) atomicMax(addr, m);
 }
 

@@ -9,18 +9,9 @@ namespace cuharm {
 
 // ---------------------------------------------------------------------------------------------------------
 // S1  Boundary conditions (A15).  Order X1, X2, X3, each over the full extended range of the others.
-// kind: 0 outflow (+ inflow check in MKS X1), 1 periodic, 2 polar reflection, 3 fixed (kernel not launched).
+// kind: 0 outflow (+ inflow check in MKS X1), 1 periodic, 2 polar reflection, 3 fixed (ghosts never written).
 // `gate`: if non-null and *gate == 0 the kernel does nothing (second ghost fill, needed only after repairs).
 // ---------------------------------------------------------------------------------------------------------
-struct BcArgs {
-  Dims d;
-  double* P;
-  const Geom* C;
-  int kind, coords;
-  double gamma_max;
-  const unsigned long long* gate;
-};
-
 __device__ __forceinline__ void inflow_check(double q[8], const Geom& G, bool inner, double gamma_max) {
   State S;
   fluid_state(q, G, S);
@@ -37,90 +28,14 @@ __device__ __forceinline__ void inflow_check(double q[8], const Geom& G, bool in
   q[2] = ln * v1; q[3] = ln * v2; q[4] = ln * v3;
 }
 
-__global__ void bc_x1_kernel(BcArgs a) {
-  if (a.gate && *a.gate == 0ull) return;
-  const Dims& d = a.d;
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= d.n3g) return;
-  const int j = blockIdx.y;
-  const int g = blockIdx.z >> 1, side = blockIdx.z & 1;
-  const int ig = side ? (d.ng + d.n1 + g) : (d.ng - 1 - g);
-  int is;
-  if (a.kind == 1) {
-    const int I = side ? (d.n1 + g) : (-1 - g);
-    is = d.ng + ((I % d.n1) + d.n1) % d.n1;  // wraps repeatedly when n1 < ng
-  } else {
-    is = side ? (d.ng + d.n1 - 1) : d.ng;
-  }
-  double q[8];
-  const long long src = is * d.s1 + j * d.s2 + k, dst = ig * d.s1 + j * d.s2 + k;
-#pragma unroll
-  for (int v = 0; v < 8; v++) q[v] = a.P[v * d.nz + src];
-  if (a.kind == 0) {
-    const Geom Gg = load_geom(a.C, ig * d.n2g + j);
-    const double ratio = __ldg(&a.C[is * d.n2g + j].sg) / Gg.sg;  // sqrt(-g) B^i constant across the copy
-    q[5] *= ratio; q[6] *= ratio; q[7] *= ratio;
-    if (a.coords == 0) inflow_check(q, Gg, side == 0, a.gamma_max);
-  }
-#pragma unroll
-  for (int v = 0; v < 8; v++) a.P[v * d.nz + dst] = q[v];
-}
-
-__global__ void bc_x2_kernel(BcArgs a) {
-  if (a.gate && *a.gate == 0ull) return;
-  const Dims& d = a.d;
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= d.n3g) return;
-  const int i = blockIdx.y;
-  const int g = blockIdx.z >> 1, side = blockIdx.z & 1;
-  const int jg = side ? (d.ng + d.n2 + g) : (d.ng - 1 - g);
-  int js;
-  if (a.kind == 1) {
-    const int J = side ? (d.n2 + g) : (-1 - g);
-    js = d.ng + ((J % d.n2) + d.n2) % d.n2;
-  } else if (a.kind == 2) js = side ? (d.ng + d.n2 - 1 - g) : (d.ng + g);
-  else js = side ? (d.ng + d.n2 - 1) : d.ng;
-  const long long src = i * d.s1 + js * d.s2 + k, dst = i * d.s1 + jg * d.s2 + k;
-  double q[8];
-#pragma unroll
-  for (int v = 0; v < 8; v++) q[v] = a.P[v * d.nz + src];
-  if (a.kind == 2) { q[3] = -q[3]; q[6] = -q[6]; }  // utilde^2, B^2 change sign
-  if (a.kind == 0) {
-    const double ratio = __ldg(&a.C[i * d.n2g + js].sg) / __ldg(&a.C[i * d.n2g + jg].sg);
-    q[5] *= ratio; q[6] *= ratio; q[7] *= ratio;
-  }
-#pragma unroll
-  for (int v = 0; v < 8; v++) a.P[v * d.nz + dst] = q[v];
-}
-
-__global__ void bc_x3_kernel(BcArgs a) {
-  if (a.gate && *a.gate == 0ull) return;
-  const Dims& d = a.d;
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;  // over (i,j) columns and the 2*ng ghost slots
-  const int ncol = d.n1g * d.n2g;
-  if (t >= ncol * 2 * d.ng) return;
-  const int slot = t % (2 * d.ng), col = t / (2 * d.ng);
-  const int g = slot >> 1, side = slot & 1;
-  const int kg = side ? (d.ng + d.n3 + g) : (d.ng - 1 - g);
-  int ks;
-  if (a.kind == 1) {
-    const int K = side ? (d.n3 + g) : (-1 - g);
-    ks = d.ng + ((K % d.n3) + d.n3) % d.n3;  // wraps repeatedly when n3 < ng
-  } else {
-    ks = side ? (d.ng + d.n3 - 1) : d.ng;
-  }
-  const long long base = (long long)col * d.n3g;
-#pragma unroll
-  for (int v = 0; v < 8; v++) a.P[v * d.nz + base + kg] = a.P[v * d.nz + base + ks];
-}
-
 // ---------------------------------------------------------------------------------------------------------
-// S1 in one launch.  The three fills above run X1, X2, X3 one after the other, each over the full extended range of
-// the other two directions, so the final content of a ghost zone (i, j, k) is a composition: X3 copies from
+// S1 in one launch.  The rule (A15) is three fills run one after the other -- X1, then X2, then X3, each over
+// the full extended range of the other two directions (the oracle does exactly that) -- so the final content of a
+// ghost zone (i, j, k) is a composition: X3 copies from
 // (i, j, ks) what X2 left there, which X2 took (with its sign flips / rescaling) from (i, js, ks) as X1 left it,
 // which X1 made from the interior zone (is, js, ks).  Every source of that chain is a zone no fill writes
 // (interior, or a ghost of a `fixed` direction), so all ghost zones can be produced at once, in place, from the
-// same inputs and by the same arithmetic in the same order as the three-kernel sequence: bit-identical results.
+// same inputs and by the same arithmetic in the same order as the three sequential fills.
 // Block rows: first the (i, j) rows that are ghosts in X1 or X2 (whole k range), then the rows interior in (i, j)
 // (their 2 ng ghost zones in k only), 21 of those rows per block.
 // ---------------------------------------------------------------------------------------------------------
@@ -158,13 +73,13 @@ __device__ __forceinline__ void bc_zone(const BcAllArgs& a, int i, int j, int k)
   const long long src = is * d.s1 + js * d.s2 + ks;
 #pragma unroll
   for (int v = 0; v < 8; v++) q[v] = a.P[v * d.nz + src];
-  if (gi && a.kind1 == 0) {  // X1 outflow: what bc_x1_kernel does in row js
+  if (gi && a.kind1 == 0) {  // X1 outflow, as seen in row js
     const Geom Gg = load_geom(a.C, i * d.n2g + js);
     const double ratio = __ldg(&a.C[is * d.n2g + js].sg) / Gg.sg;  // sqrt(-g) B^i constant across the copy
     q[5] *= ratio; q[6] *= ratio; q[7] *= ratio;
     if (a.coords == 0) inflow_check(q, Gg, i < d.ng, a.gamma_max);
   }
-  if (gj) {  // X2: what bc_x2_kernel does in column i
+  if (gj) {  // X2, as seen in column i
     if (a.kind2 == 2) { q[3] = -q[3]; q[6] = -q[6]; }  // utilde^2, B^2 change sign
     if (a.kind2 == 0) {
       const double ratio = __ldg(&a.C[i * d.n2g + js].sg) / __ldg(&a.C[i * d.n2g + j].sg);
@@ -255,7 +170,9 @@ struct UpdArgs {
   int* list;                    // failed zones of this substep
   unsigned long long* nfail;    // counter of this substep
   unsigned long long* stats;    // [8]
-  double dtau, idx1, idx2, idx3, gam;
+  const double* dt;  // device scalar: the step size of this RK2 step (written before the step by set_dt / dt_from_cw)
+  double dtfac;      // dtau = dtfac * *dt: 1/2 in the predictor, 1 in the corrector (eq. 25)
+  double idx1, idx2, idx3, gam;
   NewtonCfg nc;
   FloorCfg fc;
 };
@@ -295,7 +212,7 @@ __device__ __forceinline__ void zone_divergence(const UpdArgs& a, const double f
 
 template <bool SAME>
 __device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8], const double pf[8], const double dU[8],
-                                            const Geom& G, const double* cn, double rfl, double ufl,
+                                            const Geom& G, const double* cn, double rfl, double ufl, double dtau,
                                             long long idx, int q2, bool live, int cnt[5]) {
   const Dims& d = a.d;
   // U^n, source, update
@@ -310,11 +227,11 @@ __device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8]
     fluid_state(pf, G, S);
     source_term(pf, S, G, cn, a.gam, src);
   }
-  U[0] = fma(a.dtau, dU[0], U[0]);
+  U[0] = fma(dtau, dU[0], U[0]);
 #pragma unroll
-  for (int v = 1; v < 5; v++) U[v] = fma(a.dtau, src[v - 1] + dU[v], U[v]);
+  for (int v = 1; v < 5; v++) U[v] = fma(dtau, src[v - 1] + dU[v], U[v]);
 #pragma unroll
-  for (int v = 5; v < 8; v++) U[v] = fma(a.dtau, dU[v], U[v]);
+  for (int v = 5; v < 8; v++) U[v] = fma(dtau, dU[v], U[v]);
   double pn[8];
 #pragma unroll
   for (int v = 0; v < 8; v++) pn[v] = pb[v];  // A35: the guess is P^n
@@ -386,7 +303,8 @@ __global__ void __launch_bounds__(128, CUHARM_UPD_MINB) update_kernel(UpdArgs a)
   int cnt[5] = {0, 0, 0, 0, 0};
   double dU[8];
   zone_divergence(a, fx, ex, dU);
-  update_zone<SAME>(a, pb, pf, dU, G, cn, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), idx, q2, live, cnt);
+  update_zone<SAME>(a, pb, pf, dU, G, cn, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), a.dtfac * __ldg(a.dt), idx, q2,
+                    live, cnt);
   update_stats(a, cnt);
 }
 
@@ -536,6 +454,7 @@ __global__ void __launch_bounds__(TB, (CUHARM_UPD_TMA_MINB * 128) / TB) update_t
     }
   };
   if (tile < ntiles) issue(cur, 0);
+  const double dtau = a.dtfac * __ldg(a.dt);
   int cnt_acc[5] = {0, 0, 0, 0, 0};
   for (int n = 0; tile < ntiles; tile += G, n++, cur = nxt) {
     ccur = advance_cnt(ccur);
@@ -588,7 +507,7 @@ __global__ void __launch_bounds__(TB, (CUHARM_UPD_TMA_MINB * 128) / TB) update_t
     // the per-(i,j) records of this tile stay valid in their own (double-buffered) slot for the whole tile
     const double* tb = tab + (n & 1) * 64;
     const Geom Gc = load_geom_shared(tb);
-    update_zone<SAME>(a, pb, pf, dU, Gc, tb + 20, tb[60], tb[61], idx, q2, live, cnt);
+    update_zone<SAME>(a, pb, pf, dU, Gc, tb + 20, tb[60], tb[61], dtau, idx, q2, live, cnt);
 #pragma unroll
     for (int q = 0; q < 5; q++) cnt_acc[q] += cnt[q];
   }
@@ -686,6 +605,65 @@ __global__ void __launch_bounds__(1024) fixup_kernel(FixArgs a) {
   }
   if (repaired) atomicAdd(a.stats + 1, repaired);
   if (lastres) atomicAdd(a.stats + 7, lastres);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S10  The step size lives in a device scalar, so that one recorded CUDA graph serves every dt (eq. 26 gives a new
+// one every step).  clock[0] = dt of the current step, clock[1] = time integrated so far.
+// set_dt_kernel: dt chosen by the caller.  dt_from_cw_kernel: eq. 26 from the c_w maxima the predictor of the
+// previous step recorded ("the next time step"), with the host formula of cuharm_last_cfl_dt written out in
+// the same order (IEEE divisions, no contraction possible), so host and device agree bit for bit.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void set_dt_kernel(double* clock, double dt) {
+  clock[0] = dt;
+  clock[1] += dt;
+}
+
+__global__ void dt_from_cw_kernel(double* clock, const unsigned long long* cw, double xi, double dx1, double dx2, double dx3,
+                                  double dt_max) {
+  const double dx[3] = {dx1, dx2, dx3};
+  double inv = 0.0;
+  for (int c = 0; c < 3; c++) {
+    const double cwc = __longlong_as_double((long long)cw[c]);
+    const double dtl = xi * dx[c] / cwc;  // dt^l = xi dx^l / max c_w
+    inv += 1.0 / dtl;                     // eq. 26
+  }
+  double dt = 1.0 / inv;
+  if (dt_max > 0.0 && dt > dt_max) dt = dt_max;
+  clock[0] = dt;
+  clock[1] += dt;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S9 as a stage of its own (test helper cuharm_apply_floors): eq. 35 floors, eqs. 36-37 ceilings, Lorentz cap on
+// every interior zone of an arbitrary primitive array; mask[zone] = the bit mask of apply_floors.
+// ---------------------------------------------------------------------------------------------------------
+struct FloorArgs {
+  Dims d;
+  double* P;
+  int* mask;
+  const Geom* C;
+  const double* floors;
+  double gam;
+  NewtonCfg nc;
+  FloorCfg fc;
+};
+
+__global__ void __launch_bounds__(128) floors_kernel(FloorArgs a) {
+  const Dims& d = a.d;
+  const int k = d.ng + blockIdx.x * 128 + threadIdx.x;
+  if (k >= d.ng + d.n3) return;
+  const int j = d.ng + blockIdx.y, i = d.ng + blockIdx.z;
+  const long long idx = i * d.s1 + j * d.s2 + k;
+  const int q2 = i * d.n2g + j;
+  const Geom G = load_geom(a.C, q2);
+  double q[8];
+#pragma unroll
+  for (int v = 0; v < 8; v++) q[v] = a.P[v * d.nz + idx];
+  const int m = apply_floors(q, G, a.C + q2, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), a.fc, a.gam, a.nc);
+#pragma unroll
+  for (int v = 0; v < 8; v++) a.P[v * d.nz + idx] = q[v];
+  if (a.mask) a.mask[idx] = m;
 }
 
 // ---------------------------------------------------------------------------------------------------------

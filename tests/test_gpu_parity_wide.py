@@ -1,0 +1,217 @@
+"""GPU parity, second set: the paths the first set (test_gpu_parity.py) never reached — ceilings and Lorentz cap
+(eqs. 36-37), phi-VARYING data on 256-zone rows in the launch configuration bench.py times, the
+headline scheme (PPM + LLF) at 10 steps, 100 steps of the unperturbed torus, even ghost-layer counts, and a step
+size that changes every step under graph replay (eq. 26).  Same error measure and tolerances as the
+first set."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+import paper_2205_02484_b200 as cu  # noqa: E402
+from workloads import config  # noqa: E402
+from workloads.states import minkowski_params, rng  # noqa: E402
+from workloads.torus import fm_torus  # noqa: E402
+
+from test_gpu_parity import both, interior, prim_errors  # noqa: E402
+
+
+# ------------------------------------------------------------------ S9: ceilings and Lorentz cap
+def strong_field_state(p, bscale, gamma_patch):
+    """A magnetised torus with B scaled by `bscale` and a 3 x 3 x 6 patch moving outwards with Lorentz factor
+    `gamma_patch` (utilde^1 = sqrt((Gamma^2 - 1) / g_11))."""
+    prim, _ = fm_torus(p)
+    ng = p["ng"]
+    prim[5:8] *= bscale
+    g11 = oracle.Grid(p).get_geom(0)[4]
+    i0, j0 = ng + 20, ng + 6
+    for di in range(3):
+        for dj in range(3):
+            prim[2, i0 + di, j0 + dj, ng + 2:ng + 8] = np.sqrt((gamma_patch ** 2 - 1.0) / g11[i0 + di, j0 + dj])
+    return prim
+
+
+CEIL_CASES = [
+    # the paper's limits (50, 2.5e3, 50) on a field 300x the torus': b^2/rho > 50 at the torus edge, many failures
+    ("strong field", dict(), 300.0, 80.0),
+    # the torus' own field against tight limits: ceilings fire in ~1e3 zones, hardly any failure
+    ("tight limits", dict(sigma_max=1e-4, b2_over_u_max=1e-2), 1.0, 80.0),
+]
+
+
+@pytest.mark.parametrize("label,kw,bscale,gpatch", CEIL_CASES, ids=[c[0] for c in CEIL_CASES])
+def test_ceilings_and_lorentz_cap_fire_and_match(label, kw, bscale, gpatch):
+    p = config("C4", n1=32, n2=32, n3=20, **kw)
+    prim0 = strong_field_state(p, bscale, gpatch)
+    ref = prim0.copy()
+    g = oracle.Grid(p)
+    g.bind(ref)
+    dt = g.cfl_dt(0.45)
+    s = cu.Solver(p, prim0)
+    g.step(dt)
+    s.step(dt)
+    st, sr = list(s.stats()), [int(x) for x in g.get_stats()]
+    assert sr[4] > 0 and sr[5] > 0, sr                      # ceilings applied, Lorentz caps applied
+    assert st == sr, (st, sr)
+    got = s.prim.cpu().numpy()
+    err = prim_errors(p, got, ref)
+    assert (err < 1e-11).all(), err
+    for _ in range(4):
+        g.step(dt)
+        s.step(dt)
+    st, sr = list(s.stats()), [int(x) for x in g.get_stats()]
+    assert st[:6] == sr[:6], (st, sr)
+    err = prim_errors(p, s.prim.cpu().numpy(), ref, tol=1e-8)
+    assert (err < 1e-8).all(), err
+    assert s.divb()[1] < 1e-12
+    s.close()
+
+
+def test_floors_stage_matches_the_oracle_zone_by_zone():
+    """cuharm_apply_floors against the oracle's C-12 on random states, a third of which violate a floor, a ceiling or
+    the Lorentz cap: masks bit-exact, primitives to 1e-11."""
+    p = config("C4", n1=24, n2=20, n3=36)
+    r = rng(41)
+    shape = (8, p["n1"] + 6, p["n2"] + 6, p["n3"] + 6)
+    prim = np.empty(shape)
+    prim[0] = 10.0 ** r.uniform(-9, 0, shape[1:])
+    prim[1] = 10.0 ** r.uniform(-11, -1, shape[1:])
+    prim[2:5] = r.normal(size=(3,) + shape[1:]) * 10.0 ** r.uniform(-2, 0.3, shape[1:])
+    prim[5:8] = r.normal(size=(3,) + shape[1:]) * 10.0 ** r.uniform(-4, -1, shape[1:])
+    # a few zones beyond the Lorentz cap
+    g = oracle.Grid(p)
+    g11 = g.get_geom(0)[4]
+    hot = r.random(shape[1:]) < 0.02
+    prim[2][hot] = (np.sqrt((70.0 ** 2 - 1.0) / g11)[:, :, None] * np.ones(shape[1:]))[hot]
+    ref = prim.copy()
+    mref = g.apply_floors(ref)
+    s = cu.Solver(p, prim)
+    d = torch.as_tensor(prim).cuda()
+    mgot = s.apply_floors(d).cpu().numpy()
+    got = d.cpu().numpy()
+    assert np.array_equal(interior(p, mgot), interior(p, mref))
+    mi = interior(p, mref)
+    for bit in (1, 2, 4, 8):
+        assert (mi & bit).any(), bit                       # every branch taken somewhere
+    err = prim_errors(p, got, ref)
+    assert (err < 1e-11).all(), err
+    s.close()
+
+
+# ------------------------------------------------------------------ phi-varying data on 256-zone rows (bench launch configuration)
+def test_phi_varying_256_deep_slab_ppm_llf_one_and_ten_steps():
+    """C4's scheme (MKS, PPM + LLF) on a 48 x 40 x 256 slab of the C4 grid with the seeded 3D perturbation, graph
+    replay: two 128-zone tiles per row in update_tma_kernel with their k+-1 halo, nine 29-face chunks per row in the
+    X3 flux kernel, strip-ordered tiles, E^1 / E^2 edges with non-cancelling X3 flux differences."""
+    p = config("C4", n1=48, n2=40, n3=256)
+    prim0, _ = fm_torus(p)
+    ng = p["ng"]
+    assert np.ptp(prim0[1, ng + 24, ng + 20, ng:-ng]) > 0          # phi-dependent input
+    got, ref, s, g, dt = both(p, prim0, 1, graph=True)
+    err = prim_errors(p, got, ref)
+    assert (err < 1e-11).all(), err
+    assert (prim_errors(p, got, ref, whole=True) < 1e-11).all()
+    assert list(s.stats()) == [int(x) for x in g.get_stats()]
+    for _ in range(9):
+        g.step(dt)
+        s.step(dt)
+    err = prim_errors(p, s.prim.cpu().numpy(), ref, tol=1e-8)
+    assert (err < 1e-8).all(), err
+    assert s.divb()[1] < 1e-12
+    assert list(s.stats()[:6]) == [int(x) for x in g.get_stats()[:6]]
+    s.close()
+
+
+def test_hundred_steps_unperturbed_torus():
+    """SURVEY 8(c) parity policy: <= 1e-9 after 100 steps on smooth flows -- the unperturbed (magnetised) torus."""
+    p = config("C4", n1=48, n2=48, n3=4)
+    prim0, _ = fm_torus(p, perturb=0.0)
+    got, ref, s, g, dt = both(p, prim0, 100, graph=True)
+    err = prim_errors(p, got, ref, tol=1e-9)
+    assert (err < 1e-9).all(), err
+    assert s.divb()[1] < 1e-12
+    s.close()
+
+
+# ------------------------------------------------------------------ even ghost-layer count (generic update path)
+@pytest.mark.parametrize("ng", [4, 5])
+def test_other_ghost_layer_counts(ng):
+    p = config("C4", n1=20, n2=16, n3=40, ng=ng)
+    base = config("C4", n1=20, n2=16, n3=40)
+    prim3, _ = fm_torus(base)
+    # re-pad the ng = 3 array to ng layers (the ghost fill overwrites the padding)
+    pad = ng - 3
+    prim0 = np.ascontiguousarray(np.pad(prim3, ((0, 0), (pad, pad), (pad, pad), (pad, pad)), mode="edge"))
+    ref = prim0.copy()
+    g = oracle.Grid(p)
+    g.bind(ref)
+    dt = g.cfl_dt(0.45)
+    s = cu.Solver(p, prim0)
+    s.use_graph(True)
+    for _ in range(2):
+        g.step(dt)
+        s.step(dt)
+    got = s.prim.cpu().numpy()
+    err = prim_errors(p, got, ref)
+    assert (err < 2e-11).all(), err
+    assert (prim_errors(p, got, ref, whole=True) < 2e-11).all()
+    assert s.divb()[1] < 1e-12
+    s.close()
+
+
+# ------------------------------------------------------------------ a new dt every step, one graph
+def test_changing_dt_under_graph_replay_is_bitwise_plain_and_follows_eq26():
+    """cuharm_step_cfl takes dt on the device from eq. 26; under graph replay the same recorded graph serves every
+    dt.  (i) graph replay == plain launches bit for bit over 10 steps with 10 different dt; (ii) the device dt equals
+    the host formula (cuharm_last_cfl_dt) bit for bit; (iii) the run follows the oracle stepped with its own eq. 26."""
+    p = config("C4", n1=32, n2=24, n3=12)
+    prim0, _ = fm_torus(p)
+    ref = prim0.copy()
+    g = oracle.Grid(p)
+    g.bind(ref)
+    dt0 = g.cfl_dt(0.45)
+    s1 = cu.Solver(p, prim0)
+    s2 = cu.Solver(p, prim0)
+    s2.use_graph(True)
+    g.step(dt0); s1.step(dt0); s2.step(dt0)
+    dts, t_sum = [dt0], dt0
+    for n in range(10):
+        expect = s1.last_cfl_dt(0.45)
+        s1.step_cfl(0.45)
+        s2.step_cfl(0.45)
+        t1, d1 = s1.time()
+        t2, d2 = s2.time()
+        assert d1 == expect and d2 == expect, (n, d1, d2, expect)
+        dto = g.last_cfl_dt(0.45)
+        assert abs(dto / d1 - 1.0) < 1e-9
+        g.step(dto)
+        dts.append(d1)
+        t_sum += d1
+        assert t1 == t_sum and t2 == t_sum
+    assert len(set(dts)) == len(dts)                      # dt really changed every step
+    assert torch.equal(s1.prim, s2.prim)
+    n_graph = s2.launch_count()
+    err = prim_errors(p, s1.prim.cpu().numpy(), ref, tol=1e-8)
+    assert (err < 1e-8).all(), err
+    # a host-chosen dt through the same graph, and a capped device dt
+    s1.step(0.5 * dt0); s2.step(0.5 * dt0)
+    s1.step_cfl(0.45, 0.25 * dt0); s2.step_cfl(0.45, 0.25 * dt0)
+    assert s2.time()[1] == 0.25 * dt0
+    assert torch.equal(s1.prim, s2.prim)
+    assert s2.launch_count() > n_graph
+    s1.close(); s2.close()
+
+
+def test_non_finite_wave_speed_gives_zero_dt():
+    p = minkowski_params(8, 8, 8)
+    prim = np.zeros((8, 14, 14, 14))
+    prim[0] = 1.0; prim[1] = 1.0
+    prim[1, 6, 6, 6] = np.nan
+    s = cu.Solver(p, prim)
+    assert s.cfl_dt(0.45) == 0.0
+    with pytest.raises(cu.CuharmError):
+        s.step(0.0)
+    s.close()
