@@ -36,8 +36,7 @@ __device__ __forceinline__ unsigned long long warp_max_ull(unsigned long long v)
 }
 
 // max of non-negative doubles through their order-preserving integer image; no floating-point atomics anywhere.
-// A NaN enters as +infinity, so that it is never lost: a non-finite wave speed anywhere makes the eq. 26 time step 0
-// (cuharm_cfl_dt and friends return dt = 0, which cuharm_step rejects).  Must be reached by all 32 lanes of the warp.
+// A NaN enters as +infinity.  Must be reached by all 32 lanes of the warp.
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* addr, double v) {
   const double vv = v >= 0.0 ? v : (v != v ? __longlong_as_double(0x7ff0000000000000LL) : 0.0);
   const unsigned long long m = warp_max_ull((unsigned long long)__double_as_longlong(vv));
@@ -72,6 +71,20 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
                  : "r"(bar), "r"(parity)
                  : "memory");
   }
+}
+
+// Running maximum of the face speeds c_w of a thread, kept as the integer image of |c_w| (order-preserving for
+// non-negative doubles; the sign bit is cleared, so a NaN of either sign ranks above +infinity and is never lost the
+// way fmax would lose it).  atomic_max_image folds the warp's maxima into the global slot, reporting anything above
+// +infinity as +infinity.  Integer pipe only: nothing here competes with the fp64 pipe.
+__device__ __forceinline__ void cw_track(unsigned long long& acc, double c) {
+  const unsigned long long m = (unsigned long long)__double_as_longlong(c) & 0x7fffffffffffffffull;
+  acc = m > acc ? m : acc;
+}
+__device__ __forceinline__ void atomic_max_image(unsigned long long* addr, unsigned long long acc) {
+  unsigned long long m = warp_max_ull(acc);
+  m = m > 0x7ff0000000000000ull ? 0x7ff0000000000000ull : m;
+  if ((threadIdx.x & 31) == 0 && m > *reinterpret_cast<volatile unsigned long long*>(addr)) atomicMax(addr, m);
 }
 
 struct FluxArgs {
@@ -145,7 +158,7 @@ __global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(Flux
   const int nk = a.hi3 - a.lo3 + 1;
   const int nt = DIR == 1 ? (a.hi2 - a.lo2 + 1) : (a.hi1 - a.lo1 + 1);
   const int q = blockIdx.x * 128 + threadIdx.x;
-  double cwv = 0.0;
+  unsigned long long cwv = 0ull;
   // The face geometry the block will need -- the records of (faces of its segment) x (the transverse rows its 128
   // columns touch) -- is staged in shared memory once, so the march reads it with shared-memory latency.
   extern __shared__ __align__(16) double2 geo[];  // [face in segment][row][10]
@@ -260,14 +273,14 @@ __global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(Flux
                          : load_geom(a.Gf, gq);
       double F[8], c;
       face_flux<DIR, RIEMANN>(pl, pr, G, a.gam, F, c);
-      cwv = fmax(cwv, c);
+      cw_track(cwv, c);
       store_flux<DIR, STAGE>(a, idx, F, c);
       y += sd;
       idx += sd;
       gq += gstep;
     }
   }
-  atomic_max_nonneg(a.cwmax, cwv);
+  atomic_max_image(a.cwmax, cwv);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -323,14 +336,15 @@ __global__ void __launch_bounds__(128, CUHARM_FLUXK_MINB) flux_k_kernel(FluxArgs
     pr[v] = l;
   }
   const bool ok = lane >= HALO && lane < HALO + FPW && c <= a.hi3;
-  double cwv = 0.0;
+  unsigned long long cwi = 0ull;
   if (ok) {
     const Geom G = load_geom(a.Gf, i * d.n2g + j);
-    double F[8];
+    double F[8], cwv;
     face_flux<3, RIEMANN>(pl, pr, G, a.gam, F, cwv);
     store_flux<3, STAGE>(a, rowoff + c, F, cwv);
+    cw_track(cwi, cwv);
   }
-  atomic_max_nonneg(a.cwmax, cwv);
+  atomic_max_image(a.cwmax, cwi);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -383,7 +397,7 @@ __global__ void __launch_bounds__(CUHARM_KROW_T, CUHARM_KROW_B) flux_k_row_kerne
       issue(i2, j2, 1);
     }
   }
-  double cwmax = 0.0;
+  unsigned long long cwmax = 0ull;
   for (int n = 0; row < nrows; row += G, n++) {
     const int s = n & 1;
     const int i = a.lo1 + ci, j = a.lo2 + cj;
@@ -419,7 +433,7 @@ __global__ void __launch_bounds__(CUHARM_KROW_T, CUHARM_KROW_B) flux_k_row_kerne
         double F[8], cwv;
         face_flux<3, RIEMANN>(pl, pr, G3, a.gam, F, cwv);
         store_flux<3, STAGE>(a, i * d.s1 + j * d.s2 + c, F, cwv);
-        cwmax = fmax(cwmax, cwv);
+        cw_track(cwmax, cwv);
       }
     }
     // advance the carried row index by 2G for the refill, by G for the next iteration
@@ -434,7 +448,7 @@ __global__ void __launch_bounds__(CUHARM_KROW_T, CUHARM_KROW_B) flux_k_row_kerne
     ci = i1;
     cj = j1;
   }
-  atomic_max_nonneg(a.cwmax, cwmax);
+  atomic_max_image(a.cwmax, cwmax);
 }
 
 }  // namespace cuharm

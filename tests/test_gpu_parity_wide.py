@@ -35,11 +35,17 @@ def strong_field_state(p, bscale, gamma_patch):
 
 
 CEIL_CASES = [
-    # the paper's limits (50, 2.5e3, 50) on a field 300x the torus': b^2/rho > 50 at the torus edge, many failures
-    ("strong field", dict(), 300.0, 80.0),
-    # the torus' own field against tight limits: ceilings fire in ~1e3 zones, hardly any failure
-    ("tight limits", dict(sigma_max=1e-4, b2_over_u_max=1e-2), 1.0, 80.0),
+    # the paper's ceilings (50, 2.5e3) on a field 300x the torus': b^2/rho > 50 at the torus edge, ~700 failed
+    # inversions per step (repairs incl. the last-resort rule ride along)
+    ("strong field", dict(gamma_max=1.5), 300.0, 2.0),
+    # the torus' own field against tight limits: ceilings fire in ~1e3 zones, few failures
+    ("tight limits", dict(sigma_max=1e-4, b2_over_u_max=1e-2, gamma_max=1.5), 1.0, 2.0),
 ]
+# The Lorentz cap is exercised with Gamma_max = 1.5 against a Gamma = 2 patch, not with the paper's 50 against Gamma =
+# 80: a Gamma = 80 patch next to floor-density zones at rest makes the update of those neighbours a difference of
+# terms 1e5 times larger than the result, and the two sides then differ by 1e-9 in rho there for conditioning
+# reasons (measured: 26 zones above 1e-11, unchanged by two extra Newton updates).  The rescale formula (A12) at the
+# paper's Gamma_max = 50 is compared zone by zone in test_floors_stage_matches_the_oracle_zone_by_zone below.
 
 
 @pytest.mark.parametrize("label,kw,bscale,gpatch", CEIL_CASES, ids=[c[0] for c in CEIL_CASES])
@@ -72,22 +78,39 @@ def test_ceilings_and_lorentz_cap_fire_and_match(label, kw, bscale, gpatch):
 
 def test_floors_stage_matches_the_oracle_zone_by_zone():
     """cuharm_apply_floors against the oracle's C-12 on random states, a third of which violate a floor, a ceiling or
-    the Lorentz cap: masks bit-exact, primitives to 1e-11."""
-    p = config("C4", n1=24, n2=20, n3=36)
+    the Lorentz cap (Gamma = 70 against the paper's 50): masks bit-exact, primitives to 1e-11.  The states are kept
+    where the ceiling's re-inversion is well conditioned (kappa = Gamma^2 (rho + gam u + b^2)/u <~ 100: u/rho >= 0.03,
+    Gamma <= 1.5, b^2/u <= 30 after the ceiling; zones pushed below the u floor and zones beyond the cap carry no
+    field), checked with the oracle itself: a 1e-15 relative perturbation of the input moves its output by < 1e-13."""
+    p = config("C4", n1=24, n2=20, n3=36, sigma_max=10.0, b2_over_u_max=30.0)
     r = rng(41)
     shape = (8, p["n1"] + 6, p["n2"] + 6, p["n3"] + 6)
-    prim = np.empty(shape)
-    prim[0] = 10.0 ** r.uniform(-9, 0, shape[1:])
-    prim[1] = 10.0 ** r.uniform(-11, -1, shape[1:])
-    prim[2:5] = r.normal(size=(3,) + shape[1:]) * 10.0 ** r.uniform(-2, 0.3, shape[1:])
-    prim[5:8] = r.normal(size=(3,) + shape[1:]) * 10.0 ** r.uniform(-4, -1, shape[1:])
-    # a few zones beyond the Lorentz cap
     g = oracle.Grid(p)
-    g11 = g.get_geom(0)[4]
+    geo = g.get_geom(0)
+    sq = [np.sqrt(geo[c])[:, :, None] for c in (4, 7, 9)]            # sqrt(g_11), sqrt(g_22), sqrt(g_33)
+
+    def vectors(amplitude):
+        n = r.normal(size=(3,) + shape[1:])
+        n /= np.sqrt((n ** 2).sum(0))
+        return [amplitude * n[c] / sq[c] for c in range(3)]
+
+    prim = np.empty(shape)
+    prim[0] = 10.0 ** r.uniform(-8, 0, shape[1:])                    # a third below the eq. 35 density floor
+    prim[1] = prim[0] * 10.0 ** r.uniform(-1.5, 0, shape[1:])
+    low = r.random(shape[1:]) < 0.1
+    prim[1][low] *= 1e-6                                             # below the internal-energy floor
+    prim[2:5] = vectors(10.0 ** r.uniform(-2, 0.0, shape[1:]))       # Gamma <= 1.5
+    prim[5:8] = vectors(np.sqrt(prim[1] * 10.0 ** r.uniform(-2, 2.0, shape[1:])))   # b^2/u from 1e-2 to 1e2
     hot = r.random(shape[1:]) < 0.02
-    prim[2][hot] = (np.sqrt((70.0 ** 2 - 1.0) / g11)[:, :, None] * np.ones(shape[1:]))[hot]
+    prim[2][hot] = (np.sqrt(70.0 ** 2 - 1.0) / sq[0] * np.ones(shape[1:]))[hot]    # beyond the Lorentz cap
+    prim[3][hot] = 0.0
+    prim[4][hot] = 0.0
+    prim[5:8, hot | low] = 0.0
     ref = prim.copy()
     mref = g.apply_floors(ref)
+    wiggled = prim * (1.0 + 1e-15 * r.normal(size=prim.shape))
+    g.apply_floors(wiggled)
+    assert (prim_errors(p, wiggled, ref) < 1e-13).all()              # conditioning of the inputs, by the oracle itself
     s = cu.Solver(p, prim)
     d = torch.as_tensor(prim).cuda()
     mgot = s.apply_floors(d).cpu().numpy()
@@ -95,7 +118,7 @@ def test_floors_stage_matches_the_oracle_zone_by_zone():
     assert np.array_equal(interior(p, mgot), interior(p, mref))
     mi = interior(p, mref)
     for bit in (1, 2, 4, 8):
-        assert (mi & bit).any(), bit                       # every branch taken somewhere
+        assert (mi & bit).sum() > 100, bit                 # every branch taken in many zones
     err = prim_errors(p, got, ref)
     assert (err < 1e-11).all(), err
     s.close()
@@ -191,7 +214,8 @@ def test_changing_dt_under_graph_replay_is_bitwise_plain_and_follows_eq26():
         dts.append(d1)
         t_sum += d1
         assert t1 == t_sum and t2 == t_sum
-    assert len(set(dts)) == len(dts)                      # dt really changed every step
+    # dt really changed every step (the first eq. 26 value repeats dt0: the first predictor saw the initial state)
+    assert dts[1] == dts[0] and len(set(dts[1:])) == len(dts) - 1
     assert torch.equal(s1.prim, s2.prim)
     n_graph = s2.launch_count()
     err = prim_errors(p, s1.prim.cpu().numpy(), ref, tol=1e-8)
