@@ -182,7 +182,7 @@ void launch_flux_t(cuharm_ctx* h, FluxArgs& a, int dir) {
     const int wpr = (nk + fpw - 1) / fpw;
     const Dims& d = a.d;
     const bool tma = h->fluxk_row && (d.n3g % 2 == 0) && ((uintptr_t)a.P % 16 == 0);
-    const size_t row_smem = 2 * 8 * (size_t)d.n3g * sizeof(double);
+    const size_t row_smem = KROW_STAGES * 8 * (size_t)d.n3g * sizeof(double);
     bool row_ok = tma && row_smem <= 200 * 1024;
     if (row_ok && row_smem > 48 * 1024)
       row_ok = cudaFuncSetAttribute(flux_k_row_kernel<RECON, RIEMANN, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -199,12 +199,12 @@ void launch_flux_t(cuharm_ctx* h, FluxArgs& a, int dir) {
       flux_k_kernel<RECON, RIEMANN, STAGE><<<grid, 128, 0, h->stream>>>(a);
     }
   } else {
-    const long long cols = (long long)(dir == 1 ? nj : ni) * nk;
     const int nf = dir == 1 ? ni : nj;
+    const int nt = dir == 1 ? nj : ni;
+    const long long cols = (long long)nt * nk;
     a.seg = march_seg(cols, nf, h->sms);
     const dim3 grid((unsigned)((cols + 127) / 128), (unsigned)((nf + a.seg - 1) / a.seg));
     // face geometry staged per block: (rows a block's 128 columns can touch) x (faces per segment) records
-    const int nt = dir == 1 ? nj : ni;
     a.geo_rows = std::min(nt, 127 / nk + 2);
     size_t gsm = (size_t)a.geo_rows * a.seg * sizeof(Geom);
     if (gsm > 40 * 1024) { a.geo_rows = 0; gsm = 0; }

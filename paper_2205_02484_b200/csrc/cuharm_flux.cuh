@@ -123,36 +123,12 @@ __device__ __forceinline__ void store_flux(const FluxArgs& a, long long idx, con
 // cell f-1, and `pre` = y_{f+2}, loaded one iteration ahead so that its DRAM latency hides behind a whole face.
 // ---------------------------------------------------------------------------------------------------------
 // software prefetch distance (faces beyond the register look-ahead) per marching direction; measured on B200 at
-// 256^3: along X1 (plane stride) 2 faces is best, along X2 (row stride) 1 face
-#ifndef CUHARM_MARCH_PF1
-#define CUHARM_MARCH_PF1 2
-#endif
-#ifndef CUHARM_MARCH_PF2
-#define CUHARM_MARCH_PF2 1
-#endif
-#ifndef CUHARM_MARCH_PF
-#define CUHARM_MARCH_PF 1   // 0 = no software prefetch at all
-#endif
-#ifndef CUHARM_PF_LEVEL
-#define CUHARM_PF_LEVEL 1
-#endif
-__device__ __forceinline__ void prefetch_l1(const void* p) {
-#if CUHARM_PF_LEVEL == 1
-  asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
-#else
-  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-#endif
-}
-
-#ifndef CUHARM_MARCH_UNROLL
-#define CUHARM_MARCH_UNROLL 2
-#endif
-#ifndef CUHARM_MARCH_MINB
-#define CUHARM_MARCH_MINB 2
-#endif
+// 256^3: along X1 (plane stride) 2 faces is best, along X2 (row stride) 1 face; into L1
+constexpr int MARCH_PF1 = 2, MARCH_PF2 = 1;
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 template <int DIR, int RECON, int RIEMANN, bool STAGE, bool GEO>
-__global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(FluxArgs a) {
+__global__ void __launch_bounds__(128, 2) flux_march_kernel(FluxArgs a) {
   static_assert(DIR == 1 || DIR == 2, "marching kernel: directions 1 and 2");
   const Dims& d = a.d;
   const int nk = a.hi3 - a.lo3 + 1;
@@ -219,15 +195,13 @@ __global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(Flux
         pre[v] = yv[2 * sd];
       }
     }
-    constexpr int UNR = CUHARM_MARCH_UNROLL;
-#pragma unroll UNR
+#pragma unroll 2
     for (int f = fa; f < fb; f++) {
       double pl[8], pr[8];
       // look-ahead load for the next face (clamped at the end of the array; the clamped value is never used)
       const long long ahead = (f + 3 < nd ? 3 : 2) * sd;
-#if CUHARM_MARCH_PF
       {
-        constexpr int PFD = DIR == 1 ? CUHARM_MARCH_PF1 : CUHARM_MARCH_PF2;
+        constexpr int PFD = DIR == 1 ? MARCH_PF1 : MARCH_PF2;
         const long long far = (f + 3 + PFD < nd ? 3 + PFD : 2) * sd;
 #pragma unroll
         for (int v = 0; v < 8; v++) prefetch_l1(y + v * nz + far);
@@ -236,7 +210,6 @@ __global__ void __launch_bounds__(128, CUHARM_MARCH_MINB) flux_march_kernel(Flux
           prefetch_l1(reinterpret_cast<const char*>(a.Gf + gq + gstep) + 128);
         }
       }
-#endif
 #pragma unroll
       for (int v = 0; v < 8; v++) {
         const double nxt = y[v * nz + ahead];
@@ -293,12 +266,8 @@ struct FluxK {
   static constexpr int FPW = RECON == 0 ? 31 : 29;  // faces per warp
 };
 
-#ifndef CUHARM_FLUXK_MINB
-#define CUHARM_FLUXK_MINB 4
-#endif
-
 template <int RECON, int RIEMANN, bool STAGE>
-__global__ void __launch_bounds__(128, CUHARM_FLUXK_MINB) flux_k_kernel(FluxArgs a) {
+__global__ void __launch_bounds__(128, 4) flux_k_kernel(FluxArgs a) {
   const Dims& d = a.d;
   constexpr int HALO = FluxK<RECON>::HALO, FPW = FluxK<RECON>::FPW;
   const unsigned FULL = 0xffffffffu;
@@ -355,16 +324,15 @@ __global__ void __launch_bounds__(128, CUHARM_FLUXK_MINB) flux_k_kernel(FluxArgs
 // arithmetic of this one), and whole rows keep the copy count low: a warp issues its bulk copies one after the
 // other at ~8 issue slots each.
 // ---------------------------------------------------------------------------------------------------------
-#ifndef CUHARM_KROW_T
-#define CUHARM_KROW_T 128
+#ifndef KROW_NS
+#define KROW_NS 3
 #endif
-#ifndef CUHARM_KROW_B
-#define CUHARM_KROW_B 4
-#endif
+constexpr int KROW_STAGES = KROW_NS;  // rows in the ring of a block
 template <int RECON, int RIEMANN, bool STAGE>
-__global__ void __launch_bounds__(CUHARM_KROW_T, CUHARM_KROW_B) flux_k_row_kernel(FluxArgs a, int wpr) {
-  extern __shared__ __align__(128) double rowbuf[];  // [2][8][n3g]
-  __shared__ __align__(8) unsigned long long mbar2[2];
+__global__ void __launch_bounds__(128, 4) flux_k_row_kernel(FluxArgs a, int wpr) {
+  constexpr int NS = KROW_STAGES;
+  extern __shared__ __align__(128) double rowbuf[];  // [NS][8][n3g]
+  __shared__ __align__(8) unsigned long long mbar2[2 * NS];  // full[NS] (tx count), empty[NS] (one arrival per warp)
   const Dims& d = a.d;
   constexpr int HALO = FluxK<RECON>::HALO, FPW = FluxK<RECON>::FPW;
   const unsigned FULL = 0xffffffffu;
@@ -376,7 +344,8 @@ __global__ void __launch_bounds__(CUHARM_KROW_T, CUHARM_KROW_B) flux_k_row_kerne
   int row = blockIdx.x;
   int ci = row / nj, cj = row % nj;          // carried (i, j) of the current row
   const int di = G / nj, dj = G % nj;
-  auto issue = [&](int i, int j, int stage) {  // lanes 0..7 of warp 0, one variable each
+  auto issue = [&](int r, int stage) {  // lanes 0..7 of warp 0, one variable each; r = row index
+    const int i = r / nj, j = r - i * nj;
     const double* src = a.P + (long long)(a.lo1 + i) * d.s1 + (long long)(a.lo2 + j) * d.s2 + lane * d.nz;
     const unsigned bar = bar0 + 8 * stage;
     if (lane == 0) mbar_expect_tx(bar, 8u * rs * 8u);
@@ -384,25 +353,21 @@ __global__ void __launch_bounds__(CUHARM_KROW_T, CUHARM_KROW_B) flux_k_row_kerne
     bulk_g2s(smem_u32(rowbuf + (stage * 8 + lane) * rs), src, (unsigned)rs * 8u, bar);
   };
   if (threadIdx.x == 0) {
-    mbar_init(bar0, 1);
-    mbar_init(bar0 + 8, 1);
+#pragma unroll
+    for (int s = 0; s < NS; s++) { mbar_init(bar0 + 8 * s, 1); mbar_init(bar0 + 8 * (NS + s), nw); }
     mbar_fence_init();
   }
   __syncthreads();
   if (wib == 0 && lane < 8) {
-    if (row < nrows) issue(ci, cj, 0);
-    if (row + G < nrows) {
-      int i2 = ci + di, j2 = cj + dj;
-      if (j2 >= nj) { j2 -= nj; i2++; }
-      issue(i2, j2, 1);
-    }
+    for (int s = 0; s < NS; s++)
+      if (row + (long long)s * G < nrows) issue(row + s * G, s);
   }
   unsigned long long cwmax = 0ull;
   for (int n = 0; row < nrows; row += G, n++) {
-    const int s = n & 1;
+    const int s = n % NS;
     const int i = a.lo1 + ci, j = a.lo2 + cj;
     const double* st = rowbuf + s * 8 * rs;
-    mbar_wait(bar0 + 8 * s, (n >> 1) & 1);
+    mbar_wait(bar0 + 8 * s, (n / NS) & 1);
     for (int w = wib; w < wpr; w += nw) {
       const int f0 = a.lo3 + w * FPW;
       const int c = f0 - HALO + lane;            // this lane's cell = the cell whose lower face is face c
@@ -436,17 +401,21 @@ __global__ void __launch_bounds__(CUHARM_KROW_T, CUHARM_KROW_B) flux_k_row_kerne
         cw_track(cwmax, cwv);
       }
     }
-    // advance the carried row index by 2G for the refill, by G for the next iteration
-    int i1 = ci + di, j1 = cj + dj;
-    if (j1 >= nj) { j1 -= nj; i1++; }
-    __syncthreads();  // every warp is done with stage s
-    if (wib == 0 && lane < 8 && row + 2 * G < nrows) {
-      int i2 = i1 + di, j2 = j1 + dj;
-      if (j2 >= nj) { j2 -= nj; i2++; }
-      issue(i2, j2, s);
+    // This warp is done with stage s (one arrival per warp; no block-wide barrier: the warps of a block may be a row
+    // apart).  The stage released ONE ROW AGO, which every warp has normally long left, is then refilled by warp 0 with
+    // the row NS - 1 iterations ahead: NS - 1 rows are in flight or landed while a row is being worked on.
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar0 + 8 * (NS + s));
+    // (the wait is executed by every thread -- a spin loop under a thread-dependent condition would cost the warp its
+    // convergence guarantee and every shuffle above an explicit re-synchronisation)
+    const long long rnext = (long long)row + (long long)(NS - 1) * G;  // row of iteration n - 1 + NS
+    if (n >= 1 && rnext < nrows) {
+      mbar_wait(bar0 + 8 * (NS + (n - 1) % NS), ((n - 1) / NS) & 1);
+      if (wib == 0 && lane < 8) issue((int)rnext, (n - 1) % NS);
     }
-    ci = i1;
-    cj = j1;
+    ci += di;
+    cj += dj;
+    if (cj >= nj) { cj -= nj; ci++; }
   }
   atomic_max_image(a.cwmax, cwmax);
 }

@@ -177,10 +177,6 @@ struct UpdArgs {
   FloorCfg fc;
 };
 
-#ifndef CUHARM_UPD_MINB
-#define CUHARM_UPD_MINB 3
-#endif
-
 // Per-zone work once the streamed operands are in registers.  pb = P^n, pf = the state the fluxes were built from
 // (pf is pb in the predictor), fx[6v..6v+5] = F1[i+1], F1[i], F2[j+1], F2[j], F3[k+1], F3[k] of hydro component v,
 // ex = E1 at (0, +j, +k, +j+k), E2 at (0, +i, +k, +i+k), E3 at (0, +i, +j, +i+j).
@@ -269,7 +265,7 @@ __device__ __forceinline__ void update_stats(const UpdArgs& a, const int cnt[5])
 // Generic kernel: per-thread loads (any n3, any alignment).  One thread per interior zone; out-of-range lanes of the
 // ragged tail work on a clamped copy of the last zone and store nothing.
 template <bool SAME>
-__global__ void __launch_bounds__(128, CUHARM_UPD_MINB) update_kernel(UpdArgs a) {
+__global__ void __launch_bounds__(128, 3) update_kernel(UpdArgs a) {
   const Dims& d = a.d;
   const int k = d.ng + blockIdx.x * 128 + threadIdx.x;
   const int j = d.ng + blockIdx.y, i = d.ng + blockIdx.z;
@@ -334,14 +330,12 @@ struct TileCnt { int s, i, jj, c; };  // mixed-radix tile counter: j-strip, i, j
 // Persistent blocks: block b takes tiles b, b + gridDim.x, ...; tile = (i, j, 128-zone chunk of the row), chunk
 // fastest.  One stage per block: the stage is free again as soon as every thread has moved its operands to
 // registers, which is the first thing a tile does, so the copies of tile n+1 fly during the whole of tile n's
-// arithmetic; CUHARM_UPD_TMA_MINB blocks per SM keep that many tiles in flight and enough warps for the
+// arithmetic; UPD_TMA_MINB blocks of 128 threads per SM keep that many tiles in flight and enough warps for the
 // (serial) Newton iteration.
-#ifndef CUHARM_UPD_TMA_MINB
-#define CUHARM_UPD_TMA_MINB 3
-#endif
+constexpr int UPD_TMA_MINB = 3;
 // TB = zones (threads) per tile: 128, or 64 for short rows (n3 <= 64), which would leave half a 128-zone tile idle.
 template <bool SAME, int TB>
-__global__ void __launch_bounds__(TB, (CUHARM_UPD_TMA_MINB * 128) / TB) update_tma_kernel(UpdArgs a, int ntiles, int nch, int wj) {
+__global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kernel(UpdArgs a, int ntiles, int nch, int wj) {
   constexpr int UPD_ROW = upd_row(TB);
   extern __shared__ __align__(128) double rows[];  // [UPD_NROW][UPD_ROW]
   __shared__ __align__(8) unsigned long long mbar[2];  // [0] copies landed (tx count), [1] stage released (TB arrivals)
