@@ -66,6 +66,14 @@ typedef struct {
   int32_t n_x;     /* hyper-exponential radial branch of eq. 39: r = R0 + exp(X + (X - x_b)^n_x) for */
   double r_break;  /* X >= x_b = ln(r_break - R0) (the paper: n_x = 4, r_break = 400 M, r_out = 5e3 M); the grid    */
                    /* stays uniform in X1 from ln(r_in - R0) to the X1 of r_out.  Off unless n_x >= 2, r_break > R0 */
+  int32_t inv_chain;   /* 1: the inversion fallback chain of P:L233-239 on the zones the 2D Newton method fails in:
+                          no result -> 1D method for W by Brent; non-physical result, or 1D failed too -> the
+                          entropy method (eq. 32 in eq. 29, by Brent; eq. 11 advanced for those zones); what still
+                          fails goes to the eq. 34 repair.  0: failures go straight to eq. 34 (A33)               */
+  int32_t brent_maxit; /* iteration cap of the Brent solver                                                       */
+  double beta_min;     /* eq. 33 (A37): zones with p_g / (p_g + b^2/2) < beta_min at the previous time
+                          level take the entropy method as first and only choice; <= 0 disables; needs inv_chain  */
+  double brent_tol;    /* relative tolerance of the Brent solver (A40)                                            */
 } cuharm_params;
 
 /* Create a context for the grid and scheme described by *p (the statement of the problem: spin a, adiabatic

@@ -49,6 +49,10 @@ struct oracle_params {
   int32_t fixup_max_passes;
   int32_t n_x;      // hyper-exponential radial branch of eq. 39: exponent n_X; < 2 = plain exponential
   double r_break;   // radius of the transition X = x_b (the paper: 400 M); used when n_x >= 2 and r_break > R0
+  int32_t inv_chain;    // 1: inversion fallback chain: 2D Newton -> 1D-W Brent -> entropy; 0: straight to eq. 34
+  int32_t brent_maxit;  // iteration cap of the Brent solver
+  double beta_min;      // eq. 33: p_g / (p_g + b^2/2) of P^n below this -> entropy inversion first and only; <= 0 disables
+  double brent_tol;     // relative tolerance of the Brent solver (A40)
 };
 
 }  // extern "C"
@@ -357,8 +361,13 @@ void recon_cell(int recon, const double y[5], double* l, double* r) {
 // C-6  Riemann flux at one face from the two reconstructed states and the FACE metric
 // (P:L139-161).  LLF eq. 17; HLL eq. 20 (A30: denominator guarded).
 // ------------------------------------------------------------------------------------------
+// entropy density S = p_g / rho^(gam-1), the quantity advected by eq. 11
+double entropy_of(double rho, double u, double gam) { return (gam - 1.0) * u / std::pow(rho, gam - 1.0); }
+
+// FS_out (may be null): the same Riemann flux for the entropy equation (eq. 11): conserved sqrt(-g) S u^t, flux
+// sqrt(-g) S u^d, from the same two states and the same wave speeds.
 void face_flux(const double pl[8], const double pr[8], const Geom& G, double gam, int dir, int riemann,
-               double Fbar[8], double* cw_out) {
+               double Fbar[8], double* cw_out, double* FS_out = nullptr) {
   State Sl, Sr;
   fluid_state(pl, G, Sl);
   fluid_state(pr, G, Sr);
@@ -380,6 +389,17 @@ void face_flux(const double pl[8], const double pr[8], const Geom& G, double gam
     } else {
       double den = std::max(cmax + cmin, 1e-300);
       Fbar[v] = (cmax * Fl[v] + cmin * Fr[v] - cmax * cmin * (Ur[v] - Ul[v])) / den;  // eq. 20
+    }
+  }
+  if (FS_out) {
+    double sl = entropy_of(pl[0], pl[1], gam), sr = entropy_of(pr[0], pr[1], gam);
+    double ul = G.sqrtg * sl * Sl.ucon[0], ur = G.sqrtg * sr * Sr.ucon[0];
+    double fl = G.sqrtg * sl * Sl.ucon[dir], fr = G.sqrtg * sr * Sr.ucon[dir];
+    if (riemann == 0) {
+      *FS_out = 0.5 * (fl + fr - cw * (ur - ul));
+    } else {
+      double den = std::max(cmax + cmin, 1e-300);
+      *FS_out = (cmax * fl + cmin * fr - cmax * cmin * (ur - ul)) / den;
     }
   }
 }
@@ -504,6 +524,204 @@ int invert_2d(const double U[8], const Geom& G, double gam, double prim[8], doub
 }
 
 // ------------------------------------------------------------------------------------------
+// the fallback inversions of P:L229-239.  Common set-up: the Noble variables of eqs. 27-28.
+// ------------------------------------------------------------------------------------------
+struct Noble {
+  double D, Qtsq, Bsq, QdB, Qdn, Qcon[4], ncon[4], Bc[4];
+  double Qt[4];   // Qtilde^i, i = 1..3
+  bool finite;
+};
+
+// energy_free: Qtilde^2 and Qtilde^i from the momentum components alone, through the spatial inverse metric
+// gamma^{ij} = g^{ij} - g^{ti} g^{tj} / g^{tt}: "(Qtilde)^2 is independent on Qtilde^0, and therefore computing its value
+// does not require the use of the energy conservation equation" -- the form the entropy method needs, since
+// it is called exactly when the energy variable cannot be trusted.  Otherwise the 4-vector forms of invert_2d.
+void noble_vars(const double U[8], const Geom& G, Noble& N, bool energy_free = false) {
+  double alpha = G.alpha, sg = G.sqrtg;
+  N.D = alpha * U[0] / sg;
+  double Qcov[4];
+  for (int m = 0; m < 4; m++) Qcov[m] = alpha * U[1 + m] / sg;
+  N.Bc[0] = 0.0;
+  for (int i = 1; i < 4; i++) N.Bc[i] = alpha * U[4 + i] / sg;
+  N.finite = std::isfinite(N.D);
+  for (int m = 0; m < 4; m++) N.finite = N.finite && std::isfinite(Qcov[m]) && std::isfinite(N.Bc[m]);
+  for (int m = 0; m < 4; m++) {
+    double v = 0.0;
+    for (int n = 0; n < 4; n++) v += G.gcon[m][n] * Qcov[n];
+    N.Qcon[m] = v;
+  }
+  N.Bsq = 0.0;
+  for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) N.Bsq += G.gcov[i][j] * N.Bc[i] * N.Bc[j];
+  N.QdB = 0.0;
+  for (int i = 1; i < 4; i++) N.QdB += Qcov[i] * N.Bc[i];
+  N.ncon[0] = 1.0 / alpha;
+  for (int i = 1; i < 4; i++) N.ncon[i] = -alpha * G.gcon[0][i];
+  N.Qdn = 0.0;
+  for (int m = 0; m < 4; m++) N.Qdn += Qcov[m] * N.ncon[m];
+  double Qsq = 0.0;
+  for (int m = 0; m < 4; m++) Qsq += N.Qcon[m] * Qcov[m];
+  N.Qtsq = Qsq + N.Qdn * N.Qdn;
+  for (int i = 1; i < 4; i++) N.Qt[i] = N.Qcon[i] + N.ncon[i] * N.Qdn;
+  if (energy_free) {
+    N.finite = std::isfinite(N.D);
+    for (int i = 1; i < 4; i++) N.finite = N.finite && std::isfinite(Qcov[i]) && std::isfinite(N.Bc[i]);
+    N.Qtsq = 0.0;
+    for (int i = 1; i < 4; i++) {
+      double v = 0.0;
+      for (int j = 1; j < 4; j++) v += (G.gcon[i][j] - G.gcon[0][i] * G.gcon[0][j] / G.gcon[0][0]) * Qcov[j];
+      N.Qt[i] = v;
+      N.Qtsq += v * Qcov[i];
+    }
+  }
+}
+
+// residual of eq. 29 at (W, v^2)
+double eq29(const Noble& N, double W, double v2) {
+  return N.Qtsq - v2 * (N.Bsq + W) * (N.Bsq + W) + N.QdB * N.QdB * (N.Bsq + 2.0 * W) / (W * W);
+}
+
+// Brent's method (Brent 1973, "zeroin") for f on [a, b] with f(a) f(b) <= 0.  Stops when the bracket is shorter
+// than |b| (4 eps + tol) or f(b) = 0.  A40: the paper names the method only; the relative tolerance
+// is a parameter, 1e-14 in the workloads -- far below the 1e-10 the paper quotes for Newton, so that two
+// implementations land on the same root to round-off whatever path their bisection / interpolation choices take.
+template <class F>
+bool brent(F f, double a, double b, double fa, double fb, double tol, int maxit, double* root) {
+  if (!(fa * fb <= 0.0)) return false;
+  double c = a, fc = fa, d = b - a, e = d;
+  for (int it = 0; it < maxit; it++) {
+    if ((fb > 0.0 && fc > 0.0) || (fb < 0.0 && fc < 0.0)) { c = a; fc = fa; d = b - a; e = d; }
+    if (std::fabs(fc) < std::fabs(fb)) { a = b; b = c; c = a; fa = fb; fb = fc; fc = fa; }
+    double tol1 = std::fabs(b) * (2.0 * 2.220446049250313e-16 + 0.5 * tol);
+    double xm = 0.5 * (c - b);
+    if (std::fabs(xm) <= tol1 || fb == 0.0) { *root = b; return true; }
+    if (std::fabs(e) >= tol1 && std::fabs(fa) > std::fabs(fb)) {
+      double sfrac = fb / fa, p, q;
+      if (a == c) {
+        p = 2.0 * xm * sfrac;
+        q = 1.0 - sfrac;
+      } else {
+        double qq = fa / fc, r = fb / fc;
+        p = sfrac * (2.0 * xm * qq * (qq - r) - (b - a) * (r - 1.0));
+        q = (qq - 1.0) * (r - 1.0) * (sfrac - 1.0);
+      }
+      if (p > 0.0) q = -q;
+      p = std::fabs(p);
+      double min1 = 3.0 * xm * q - std::fabs(tol1 * q), min2 = std::fabs(e * q);
+      if (2.0 * p < (min1 < min2 ? min1 : min2)) { e = d; d = p / q; }
+      else { d = xm; e = d; }
+    } else {
+      d = xm; e = d;
+    }
+    a = b; fa = fb;
+    if (std::fabs(d) > tol1) b += d;
+    else b += (xm >= 0.0 ? tol1 : -tol1);
+    fb = f(b);
+    if (!std::isfinite(fb)) return false;
+  }
+  return false;
+}
+
+// recover rho, u, utilde^i from (W, v^2) as in the 2D method; returns a failure code of invert_2d
+int recover_prims(const Noble& N, double gam, double W, double v2, double u_given, bool use_u_given, double prim[8]) {
+  if (!(W > 0.0) || !std::isfinite(W)) return 3;
+  if (!(v2 >= 0.0 && v2 < 1.0)) return 4;
+  double lor = 1.0 / std::sqrt(1.0 - v2);
+  double rho = N.D / lor;
+  double w = W * (1.0 - v2);
+  double u = use_u_given ? u_given : (w - rho) / gam;
+  if (!(rho > 0.0)) return 5;
+  if (!(u >= 0.0)) return 6;
+  prim[0] = rho;
+  prim[1] = u;
+  for (int i = 1; i < 4; i++) prim[1 + i] = lor * (N.Qt[i] + N.QdB * N.Bc[i] / W) / (W + N.Bsq);
+  return 0;
+}
+
+// (ii) the 1D method: "analytically expressing v^2 from Equation (30), use its expression in Equation
+// (29) which is then numerically solved using the Brent method".  With s = sqrt(1 - v^2) and eq. 31, eq. 30 (A6 sign)
+// is the quadratic  (B^2/2 + g W) s^2 - g D s + [-Q.n - B^2 + (Q.B)^2/(2 W^2) - W] = 0,  g = (gam-1)/gam,
+// whose constant term is negative wherever a physical state exists, so the root with the plus sign is the positive
+// one.  The quadratic has real roots only above some W_d (its discriminant turns negative below), the eq. 29
+// residual r(W) is negative in a thin band above W_d, crosses zero at the physical root and stays positive beyond
+// (v^2 of eq. 30 decreases, eventually below zero).  A41 (bracket; the paper is silent): from W0 = Gamma^2 w of the
+// guess, double W until r is defined and positive (upper end); halve W from there until r is negative or undefined
+// (lower end); Brent then runs on r extended below W_d by the constant -r(upper end), so that the bracket always
+// carries a sign change and the root, if one exists, is the only sign change of a continuous stretch.
+// Returns 0 or a failure code (2: no bracket / no convergence / root at the edge of validity; 3..6 as invert_2d).
+// "parity unpinned": A41.
+bool v2_from_eq30(const Noble& N, double gam, double W, double* v2) {
+  double g = (gam - 1.0) / gam;
+  double qa = 0.5 * N.Bsq + g * W;
+  double qb = -g * N.D;
+  double qc = -N.Qdn - N.Bsq + N.QdB * N.QdB / (2.0 * W * W) - W;
+  double disc = qb * qb - 4.0 * qa * qc;
+  if (!(disc >= 0.0) || !(qa > 0.0)) return false;
+  double sroot = (-qb + std::sqrt(disc)) / (2.0 * qa);
+  *v2 = 1.0 - sroot * sroot;
+  return std::isfinite(*v2);
+}
+
+int invert_1dw(const double U[8], const Geom& G, double gam, double prim[8], double tol, int maxit) {
+  double guess[8];
+  for (int v = 0; v < 8; v++) guess[v] = prim[v];
+  for (int i = 1; i < 4; i++) prim[4 + i] = U[4 + i] / G.sqrtg;
+  Noble N;
+  noble_vars(U, G, N);
+  if (!N.finite || !(N.D > 0.0)) return 1;
+  double qsq = 0.0;
+  for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) qsq += G.gcov[i][j] * guess[1 + i] * guess[1 + j];
+  double W0 = (1.0 + qsq) * (guess[0] + gam * guess[1]);
+  if (!(W0 > 0.0) || !std::isfinite(W0)) return 3;
+  auto resid = [&](double W) {
+    double v2;
+    if (!v2_from_eq30(N, gam, W, &v2)) return std::nan("");
+    return eq29(N, W, v2);
+  };
+  // bracket search (A41)
+  double wb = W0, fb = resid(wb);
+  for (int k = 0; k < 60 && !(std::isfinite(fb) && fb > 0.0); k++) { wb *= 2.0; fb = resid(wb); }
+  if (!(std::isfinite(fb) && fb > 0.0)) return 2;
+  const double below = -fb;
+  auto rext = [&](double W) { double r = resid(W); return std::isfinite(r) ? r : below; };
+  double wa = 0.5 * wb, fa = rext(wa);
+  for (int k = 0; k < 60 && fa > 0.0; k++) { wa *= 0.5; fa = rext(wa); }
+  if (fa > 0.0) return 2;
+  double W;
+  if (!brent(rext, wa, wb, fa, fb, tol, maxit, &W)) return 2;
+  double v2;
+  if (!v2_from_eq30(N, gam, W, &v2)) return 2;
+  return recover_prims(N, gam, W, v2, 0.0, false, prim);
+}
+
+// (iii) the entropy method (eq. 32): W(v^2) = Gamma D + Gamma gam/(gam-1) (D/Gamma)^(gam-1) calS put
+// into eq. 29, solved for v^2 in [0, 1) by Brent.  A36: eq. 32 holds as printed when its S is the CONSERVED
+// entropy calS = Gamma S = alpha U_S / sqrt(-g) (as D = Gamma rho), S = p_g / rho^(gam-1).
+// The residual is >= 0 at v^2 = 0 and -> -infinity as v^2 -> 1, so [0, 1 - 1e-15] always brackets a root.
+// Returns 0 or: 1 (D <= 0, calS <= 0 or non-finite input), 2 (Brent failed), 3..6 as invert_2d.
+int invert_entropy(const double U[8], double US, const Geom& G, double gam, double prim[8], double tol, int maxit) {
+  for (int i = 1; i < 4; i++) prim[4 + i] = U[4 + i] / G.sqrtg;
+  Noble N;
+  noble_vars(U, G, N, true);
+  double calS = G.alpha * US / G.sqrtg;
+  if (!N.finite || !std::isfinite(calS) || !(N.D > 0.0) || !(calS > 0.0)) return 1;
+  auto Wof = [&](double v2) {
+    double lor = 1.0 / std::sqrt(1.0 - v2);
+    return lor * N.D + lor * (gam / (gam - 1.0)) * std::pow(N.D / lor, gam - 1.0) * calS;  // eq. 32
+  };
+  auto resid = [&](double v2) { return eq29(N, Wof(v2), v2); };
+  double a = 0.0, b = 1.0 - 1e-15;
+  double fa = resid(a), fb = resid(b);
+  if (!std::isfinite(fa) || !std::isfinite(fb)) return 2;
+  double v2;
+  if (fa == 0.0) v2 = 0.0;
+  else if (!brent(resid, a, b, fa, fb, tol, maxit, &v2)) return 2;
+  double lor = 1.0 / std::sqrt(1.0 - v2);
+  double rho = N.D / lor;
+  double pg = (calS / lor) * std::pow(rho, gam - 1.0);   // S rho^(gam-1), S = calS / Gamma
+  return recover_prims(N, gam, Wof(v2), v2, pg / (gam - 1.0), true, prim);
+}
+
+// ------------------------------------------------------------------------------------------
 // C-12  Floors (eqs. 35-37; A9-A12).  "parity unpinned" for the ceiling mechanism
 // (A11) — the paper gives no formula; post-conditions and idempotence are pinned.
 // Returns a bit mask: 1 rho floor, 2 u floor, 4 ceiling applied, 8 Lorentz cap, 16 ceiling
@@ -573,8 +791,10 @@ struct Ctx {
   std::vector<double> rc;           // r at centre
   double* prim;                     // bound, caller-owned
   std::vector<double> F[3], E[3], Phalf, Pnew, cw[3];
+  std::vector<double> FS[3];        // entropy fluxes of eq. 11 (filled only when the fallback chain is on)
   std::vector<int32_t> flag;
   int64_t stats[8];
+  int64_t chain[4];                 // 0 zones sent down the chain, 1 recovered by 1D-W, 2 by the entropy method, 3 entropy-first zones (eq. 33)
   double cwmax[3];
 
   size_t idx(int i, int j, int k) const { return ((size_t)i * n2g + j) * n3g + k; }
@@ -711,7 +931,8 @@ void apply_bc(const Ctx& c, double* P) {
 // d-face index 0..N_d, transverse zones -1..N.  F[v] stored at the index of the zone whose
 // LOWER d-face it is.  cw stored likewise (0 elsewhere).
 // ------------------------------------------------------------------------------------------
-void flux_dir(Ctx& c, const double* P, int dir, std::vector<double>& F, std::vector<double>& CW, double* cwmax) {
+void flux_dir(Ctx& c, const double* P, int dir, std::vector<double>& F, std::vector<double>& CW, double* cwmax,
+              std::vector<double>* FS = nullptr) {
   const int ng = c.ng;
   int n[3] = {c.p.n1, c.p.n2, c.p.n3};
   int lo[3], hi[3];
@@ -723,6 +944,7 @@ void flux_dir(Ctx& c, const double* P, int dir, std::vector<double>& F, std::vec
   e[dir - 1] = 1;
   F.assign(8 * c.nz, 0.0);
   CW.assign(c.nz, 0.0);
+  if (FS) FS->assign(c.nz, 0.0);
   double cmax_all = 0.0;
 #pragma omp parallel for reduction(max : cmax_all) schedule(static)
   for (int i = lo[0]; i <= hi[0]; i++)
@@ -744,8 +966,9 @@ void flux_dir(Ctx& c, const double* P, int dir, std::vector<double>& F, std::vec
           pr[v] = l;  // q^r at the face = lower-face value of the right cell
         }
         const Geom& G = geom_face(c, dir, i, j);
-        double Fb[8], cw;
-        face_flux(pl, pr, G, c.p.gam, dir, c.p.riemann, Fb, &cw);
+        double Fb[8], cw, fs = 0.0;
+        face_flux(pl, pr, G, c.p.gam, dir, c.p.riemann, Fb, &cw, FS ? &fs : nullptr);
+        if (FS) (*FS)[c.idx(i, j, k)] = fs;
         for (int v = 0; v < 8; v++) F[c.vidx(v, i, j, k)] = Fb[v];
         CW[c.idx(i, j, k)] = cw;
         if (cw > cmax_all) cmax_all = cw;
@@ -869,14 +1092,16 @@ void fixup(Ctx& c, double* P) {
 // ------------------------------------------------------------------------------------------
 void substep(Ctx& c, const double* Pflux, const double* Pbase, double dtau, double* Pout, bool record_cw) {
   double cwm[3];
-  for (int d = 1; d <= 3; d++) flux_dir(c, Pflux, d, c.F[d - 1], c.cw[d - 1], &cwm[d - 1]);
+  const bool chain = c.p.inv_chain != 0;
+  for (int d = 1; d <= 3; d++) flux_dir(c, Pflux, d, c.F[d - 1], c.cw[d - 1], &cwm[d - 1], chain ? &c.FS[d - 1] : nullptr);
   if (record_cw) for (int d = 0; d < 3; d++) c.cwmax[d] = cwm[d];
   flux_ct(c);
   const int ng = c.ng, n1 = c.p.n1, n2 = c.p.n2, n3 = c.p.n3;
   std::memcpy(Pout, Pbase, 8 * c.nz * sizeof(double));
   std::fill(c.flag.begin(), c.flag.end(), 0);
   int64_t nfl_rho = 0, nfl_u = 0, nceil = 0, ncap = 0, nits = 0;
-#pragma omp parallel for reduction(+ : nfl_rho, nfl_u, nceil, ncap, nits) schedule(static)
+  int64_t nchain = 0, n1dw = 0, nent = 0, nbeta = 0;
+#pragma omp parallel for reduction(+ : nfl_rho, nfl_u, nceil, ncap, nits, nchain, n1dw, nent, nbeta) schedule(static)
   for (int i = ng; i < ng + n1; i++)
     for (int j = ng; j < ng + n2; j++)
       for (int k = ng; k < ng + n3; k++) {
@@ -901,8 +1126,45 @@ void substep(Ctx& c, const double* Pflux, const double* Pbase, double dtau, doub
         }
         double pn[8];
         for (int v = 0; v < 8; v++) pn[v] = pb[v];  // A35
-        int iters;
-        int flag = invert_2d(U, G, c.p.gam, pn, c.p.newton_tol, c.p.newton_maxit, c.p.newton_extra, &iters);
+        int iters = 0;
+        int flag;
+        if (!chain) {
+          flag = invert_2d(U, G, c.p.gam, pn, c.p.newton_tol, c.p.newton_maxit, c.p.newton_extra, &iters);
+        } else {
+          // the chain of P:L233-239.  The entropy equation (eq. 11) is advanced like the others:
+          // U_S* = sqrt(-g) S u^t (P^n) - dtau div F_S, no source.
+          double US = G.sqrtg * entropy_of(pb[0], pb[1], c.p.gam) * Sb.ucon[0];
+          double divS = (c.FS[0][c.idx(i + 1, j, k)] - c.FS[0][c.idx(i, j, k)]) / c.dx[0] +
+                        (c.FS[1][c.idx(i, j + 1, k)] - c.FS[1][c.idx(i, j, k)]) / c.dx[1] +
+                        (c.FS[2][c.idx(i, j, k + 1)] - c.FS[2][c.idx(i, j, k)]) / c.dx[2];
+          US = US + dtau * (-divS);
+          // eq. 33 (A37): beta = p_g / (p_g + b^2/2) of the primitives at the previous time step
+          double pg = (c.p.gam - 1.0) * pb[1];
+          bool beta_small = c.p.beta_min > 0.0 && pg / (pg + 0.5 * Sb.bsq) < c.p.beta_min;
+          if (beta_small) {
+            nbeta++;
+            flag = invert_entropy(U, US, G, c.p.gam, pn, c.p.brent_tol, c.p.brent_maxit);   // first and only choice
+            if (flag == 0) nent++;
+          } else {
+            flag = invert_2d(U, G, c.p.gam, pn, c.p.newton_tol, c.p.newton_maxit, c.p.newton_extra, &iters);
+            if (flag != 0 && flag != 1) {      // 1: D <= 0 or non-finite input: no method applies
+              nchain++;
+              int f2 = flag;
+              if (flag == 2 || flag == 3) {    // "fails to produce results" -> 1D-W by Brent
+                for (int v = 0; v < 8; v++) pn[v] = pb[v];
+                f2 = invert_1dw(U, G, c.p.gam, pn, c.p.brent_tol, c.p.brent_maxit);
+                if (f2 == 0) n1dw++;
+              }
+              if (f2 != 0) {                   // non-physical values, or 1D-W failed too -> the entropy fix
+                for (int v = 0; v < 8; v++) pn[v] = pb[v];
+                f2 = invert_entropy(U, US, G, c.p.gam, pn, c.p.brent_tol, c.p.brent_maxit);
+                if (f2 == 0) nent++;
+              }
+              if (f2 != 0) { for (int v = 0; v < 5; v++) pn[v] = pb[v]; }   // still failed: the guess stays, eq. 34 repairs
+              flag = f2;
+            }
+          }
+        }
         nits += iters;
         if (flag == 0) {
           int m = apply_floors(c.p, c.rc[g2], G, pn);
@@ -912,6 +1174,7 @@ void substep(Ctx& c, const double* Pflux, const double* Pbase, double dtau, doub
         for (int v = 0; v < 8; v++) Pout[c.vidx(v, i, j, k)] = pn[v];
       }
   c.stats[2] += nfl_rho; c.stats[3] += nfl_u; c.stats[4] += nceil; c.stats[5] += ncap; c.stats[6] += nits;
+  c.chain[0] += nchain; c.chain[1] += n1dw; c.chain[2] += nent; c.chain[3] += nbeta;
   // A34: ghosts are refreshed before the repair (so that ghost donors belong to the same state) and after it
   apply_bc(c, Pout);
   fixup(c, Pout);
@@ -1053,6 +1316,7 @@ int oracle_grid_init(oracle_handle* out, const oracle_params* p) {
   c.Phalf.assign(8 * c.nz, 0.0);
   c.Pnew.assign(8 * c.nz, 0.0);
   for (int s = 0; s < 8; s++) c.stats[s] = 0;
+  for (int s = 0; s < 4; s++) c.chain[s] = 0;
   for (int d = 0; d < 3; d++) c.cwmax[d] = 0.0;
   *out = h;
   return 0;
@@ -1292,6 +1556,42 @@ int oracle_shell_fluxes(oracle_handle h, int32_t i, double out[4]) {
 // 6 Newton iterations, 7 zones repaired by the last-resort rule
 int oracle_get_stats(oracle_handle h, int64_t out[8]) {
   for (int s = 0; s < 8; s++) out[s] = h->c.stats[s];
+  return 0;
+}
+
+// 0 zones sent down the fallback chain, 1 recovered by 1D-W, 2 recovered by the entropy method, 3 entropy-first zones
+int oracle_get_chain_stats(oracle_handle h, int64_t out[4]) {
+  for (int s = 0; s < 4; s++) out[s] = h->c.chain[s];
+  return 0;
+}
+
+// point-level entry points of the fallback inversions (for the pins)
+int oracle_invert_1dw(const double U[8], const double gcov[16], const double gcon[16], double sqrtg, double gam,
+                      double prim_inout[8], double tol, int maxit) {
+  Geom G; geom_from_arrays(gcov, gcon, sqrtg, G);
+  return invert_1dw(U, G, gam, prim_inout, tol, maxit);
+}
+
+int oracle_invert_entropy(const double U[8], double US, const double gcov[16], const double gcon[16], double sqrtg,
+                          double gam, double prim_inout[8], double tol, int maxit) {
+  Geom G; geom_from_arrays(gcov, gcon, sqrtg, G);
+  return invert_entropy(U, US, G, gam, prim_inout, tol, maxit);
+}
+
+// conserved entropy sqrt(-g) S u^t of a primitive state (eq. 11)
+double oracle_entropy_cons(const double prim[8], const double gcov[16], const double gcon[16], double sqrtg, double gam) {
+  Geom G; geom_from_arrays(gcov, gcon, sqrtg, G);
+  State S; fluid_state(prim, G, S);
+  return G.sqrtg * entropy_of(prim[0], prim[1], gam) * S.ucon[0];
+}
+
+// entropy flux of one direction over the faces flux_dir covers (eq. 11), out[nz]
+int oracle_entropy_flux_dir(oracle_handle h, const double* prim, int dir, double* FS_out) {
+  Ctx& c = h->c;
+  std::vector<double> F, CW, FS;
+  double m;
+  flux_dir(c, prim, dir, F, CW, &m, &FS);
+  std::memcpy(FS_out, FS.data(), c.nz * sizeof(double));
   return 0;
 }
 

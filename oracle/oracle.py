@@ -30,6 +30,8 @@ class OracleParams(C.Structure):
         ("newton_maxit", C.c_int32), ("newton_extra", C.c_int32),
         ("fixup_max_passes", C.c_int32), ("n_x", C.c_int32),
         ("r_break", C.c_double),
+        ("inv_chain", C.c_int32), ("brent_maxit", C.c_int32),
+        ("beta_min", C.c_double), ("brent_tol", C.c_double),
     ]
 
 
@@ -61,6 +63,7 @@ def lib():
         L.oracle_slope_mc.restype = C.c_double
         L.oracle_slope_mc.argtypes = [C.c_double] * 3
         L.oracle_get_threads.restype = C.c_int
+        L.oracle_entropy_cons.restype = C.c_double
     return _lib
 
 
@@ -154,6 +157,29 @@ def invert_2d(U, gcov, gcon, sqrtg, gam, guess, tol=1e-10, maxit=30, extra=0):
     flag = lib().oracle_invert_2d(_d(U), _d(gcov), _d(gcon), C.c_double(sqrtg), C.c_double(gam), _d(prim),
                                   C.c_double(tol), int(maxit), int(extra), C.byref(it))
     return prim, flag, it.value
+
+
+def invert_1dw(U, gcov, gcon, sqrtg, gam, guess, tol=1e-14, maxit=200):
+    """(ii) of P:L204: the 1D method for W by Brent."""
+    U = _arr(U, 8); gcov = _arr(gcov, 16); gcon = _arr(gcon, 16)
+    prim = np.array(guess, dtype=np.float64).copy()
+    flag = lib().oracle_invert_1dw(_d(U), _d(gcov), _d(gcon), C.c_double(sqrtg), C.c_double(gam), _d(prim),
+                                   C.c_double(tol), int(maxit))
+    return prim, flag
+
+
+def invert_entropy(U, US, gcov, gcon, sqrtg, gam, guess, tol=1e-14, maxit=200):
+    """(iii) of P:L204: the entropy method (eq. 32 in eq. 29) by Brent.  US = sqrt(-g) S u^t."""
+    U = _arr(U, 8); gcov = _arr(gcov, 16); gcon = _arr(gcon, 16)
+    prim = np.array(guess, dtype=np.float64).copy()
+    flag = lib().oracle_invert_entropy(_d(U), C.c_double(US), _d(gcov), _d(gcon), C.c_double(sqrtg), C.c_double(gam),
+                                       _d(prim), C.c_double(tol), int(maxit))
+    return prim, flag
+
+
+def entropy_cons(prim, gcov, gcon, sqrtg, gam):
+    prim = _arr(prim, 8); gcov = _arr(gcov, 16); gcon = _arr(gcon, 16)
+    return lib().oracle_entropy_cons(_d(prim), _d(gcov), _d(gcon), C.c_double(sqrtg), C.c_double(gam))
 
 
 def apply_floors(params: dict, r, gcov, gcon, sqrtg, prim):
@@ -276,6 +302,17 @@ class Grid:
         out = np.zeros(8, dtype=np.int64)
         lib().oracle_get_stats(self._h, out.ctypes.data_as(C.POINTER(C.c_int64)))
         return out
+
+    def get_chain_stats(self):
+        out = np.zeros(4, dtype=np.int64)
+        lib().oracle_get_chain_stats(self._h, out.ctypes.data_as(C.POINTER(C.c_int64)))
+        return out
+
+    def entropy_flux_dir(self, prim, direction):
+        prim = _arr(prim, 8 * self.nz)
+        FS = np.zeros(self.shape)
+        lib().oracle_entropy_flux_dir(self._h, _d(prim), int(direction), _d(FS))
+        return FS
 
     def get_flags(self):
         out = np.zeros(self.shape, dtype=np.int32)

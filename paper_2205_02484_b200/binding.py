@@ -32,6 +32,8 @@ class CuharmParams(C.Structure):
         ("newton_maxit", C.c_int32), ("newton_extra", C.c_int32),
         ("fixup_max_passes", C.c_int32), ("n_x", C.c_int32),
         ("r_break", C.c_double),
+        ("inv_chain", C.c_int32), ("brent_maxit", C.c_int32),
+        ("beta_min", C.c_double), ("brent_tol", C.c_double),
     ]
 
 

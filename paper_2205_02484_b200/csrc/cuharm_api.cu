@@ -395,6 +395,8 @@ int check_params(const cuharm_params* p) {
     for (int c = 0; c < 3; c++)
       if (!(p->xmax[c] > p->xmin[c])) return CUHARM_EINVAL;
   }
+  if (p->inv_chain < 0 || p->inv_chain > 1) return CUHARM_EINVAL;
+  if (p->inv_chain && (p->brent_maxit < 1 || !(p->brent_tol >= 0.0) || !std::isfinite(p->beta_min))) return CUHARM_EINVAL;
   if ((long long)(p->n1 + 2 * p->ng) * (p->n2 + 2 * p->ng) * (p->n3 + 2 * p->ng) > 2000000000LL) return CUHARM_EINVAL;
   return CUHARM_OK;
 }

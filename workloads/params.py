@@ -28,6 +28,8 @@ def default_params(**kw) -> dict:
         newton_tol=1e-10, newton_maxit=30, newton_extra=0,             # P:L233 (A8: the paper's literal stopping rule)
         fixup_max_passes=4,
         n_x=0, r_break=0.0,            # hyper-exponential radial branch of eq. 39: off; the paper: 4, 400
+        inv_chain=0, brent_maxit=200,  # inversion fallback chain: off on the hot path (A33)
+        beta_min=1e-2, brent_tol=1e-14,   # eq. 33; Brent's relative tolerance (A40)
     )
     d.update(kw)
     if "a" in kw and "r_in" not in kw:
