@@ -62,7 +62,7 @@ typedef struct {
                                                  factor cap (A12); <= 0 disables                    */
   double newton_tol;                          /* |dW/W| criterion of the 2D Newton-Raphson (A8)     */
   int32_t newton_maxit, newton_extra;         /* iteration cap; extra iterations after the criterion is met */
-  int32_t fixup_max_passes;                   /* Jacobi passes of the eq. 34 repair (A13)                   */
+  int32_t fixup_max_passes;                   /* Jacobi passes of the eq. 34 repair (A13), 0..21           */
   int32_t n_x;     /* hyper-exponential radial branch of eq. 39: r = R0 + exp(X + (X - x_b)^n_x) for */
   double r_break;  /* X >= x_b = ln(r_break - R0) (the paper: n_x = 4, r_break = 400 M, r_out = 5e3 M); the grid    */
                    /* stays uniform in X1 from ln(r_in - R0) to the X1 of r_out.  Off unless n_x >= 2, r_break > R0 */
@@ -83,7 +83,8 @@ typedef struct {
 int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stream);
 
 /* Bytes of device workspace cuharm_bind needs: geometry tables, face fluxes F^1..3, edge EMFs, the half-step
- * primitives, the fail mask, counters.  0 if h is NULL. */
+ * primitives, the fail mask, counters (and, with inv_chain = 1, the updated conserved variables of every zone).
+ * 0 if h is NULL. */
 size_t cuharm_workspace_bytes(cuharm_handle h);
 
 /* Borrow the caller's primitive array d_prim (layout above) and workspace (256-byte aligned, ws_bytes >=
@@ -122,6 +123,15 @@ int cuharm_get_time(cuharm_handle h, double* t, double* dt_last);
  * d_flag[zone] (int32, [n1g][n2g][n3g], may be NULL) = 0 ok, 1 D<=0 / non-finite input, 2 no convergence,
  * 3 W<=0 or non-finite, 4 v^2 outside [0,1), 5 rho<=0, 6 u<0.  No floors, no repairs.  Asynchronous. */
 int cuharm_cons_to_prim(cuharm_handle h, const double* d_U, double* d_prim_inout, int32_t* d_flag);
+
+/* One of the two fallback inversions of P:L229-233 on full-grid arrays, like cuharm_cons_to_prim (test helper):
+ * method 1 = the 1D method (v^2 from eq. 30 put into eq. 29, solved for W by Brent), method 2 = the entropy
+ * method (eq. 32 in eq. 29, solved for v^2 by Brent; A36) with d_US[zone] ([n1g][n2g][n3g]) the conserved entropy
+ * sqrt(-g) S u^t, S = p_g / rho^(gam-1) (eq. 11).  Brent's tolerance and iteration cap are
+ * brent_tol / brent_maxit of the parameter block (EINVAL if those are not set).  d_flag as in cuharm_cons_to_prim
+ * (2 also: no bracket / Brent did not converge).  Asynchronous. */
+int cuharm_invert_fallback(cuharm_handle h, int32_t method, const double* d_U, const double* d_US, double* d_prim_inout,
+                           int32_t* d_flag);
 
 /* Primitive -> conserved on full-grid arrays.  Test helper.  Asynchronous. */
 int cuharm_prim_to_cons(cuharm_handle h, const double* d_prim, double* d_U);
@@ -163,6 +173,11 @@ int cuharm_apply_bc(cuharm_handle h, double* d_prim);
  * helper.  Asynchronous. */
 int cuharm_apply_floors(cuharm_handle h, double* d_prim, int32_t* d_mask);
 
+/* The eq. 34 repair (A13) as a stage of its own on an arbitrary primitive array of the bound shape, in
+ * place: the interior zones with d_flag[zone] > 0 (int32, [n1g][n2g][n3g]) are the failed ones; ghost zones count
+ * as good and must hold valid values.  Counters 0, 1, 7 of cuharm_get_stats advance.  Test helper.  Asynchronous. */
+int cuharm_repair(cuharm_handle h, double* d_prim, const int32_t* d_flag);
+
 /* Stage-level test helpers (asynchronous; arrays have the prim layout unless stated):
  * face fluxes of direction dir (1..3) BEFORE flux-CT, d_F[8][zones] stored at the zone whose LOWER dir-face it
  * is, valid on faces 0..N_dir and transverse zones -1..N (eqs. 15-20); d_cw[zones] (may be NULL) = c_w. */
@@ -171,6 +186,11 @@ int cuharm_flux_dir(cuharm_handle h, const double* d_prim, int32_t dir, double* 
 /* out[8] (HOST): 0 failed inversions, 1 zones repaired, 2 rho-floor hits, 3 u-floor hits, 4 ceilings applied,
  * 5 Lorentz caps, 6 Newton iterations, 7 zones repaired by the last-resort rule.  Synchronises. */
 int cuharm_get_stats(cuharm_handle h, int64_t out[8]);
+
+/* out[4] (HOST), the fallback chain of P:L229-239 (inv_chain = 1): 0 zones the 2D method failed in that went down
+ * the chain, 1 of them recovered by the 1D method, 2 zones recovered by the entropy method (from the chain or as an
+ * eq. 33 zone), 3 zones that took the entropy method first and only (eq. 33).  Synchronises. */
+int cuharm_get_chain_stats(cuharm_handle h, int64_t out[4]);
 
 /* Record the two substeps of cuharm_step into a CUDA graph and replay it on later calls (on != 0), or go back
  * to plain launches (on == 0).  Purely a launch-overhead optimisation; results are identical. */

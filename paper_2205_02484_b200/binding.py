@@ -72,8 +72,10 @@ def lib():
         L.cuharm_step_cfl.argtypes = [vp, C.c_double, C.c_double]
         L.cuharm_get_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.cuharm_apply_floors.argtypes = [vp, dp, ip]
+        L.cuharm_repair.argtypes = [vp, dp, ip]
         L.cuharm_cons_to_prim.argtypes = [vp, dp, dp, ip]
         L.cuharm_prim_to_cons.argtypes = [vp, dp, dp]
+        L.cuharm_invert_fallback.argtypes = [vp, C.c_int32, dp, dp, dp, ip]
         L.cuharm_cfl_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
         L.cuharm_last_cfl_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
         L.cuharm_divb.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -82,6 +84,7 @@ def lib():
         L.cuharm_apply_bc.argtypes = [vp, dp]
         L.cuharm_flux_dir.argtypes = [vp, dp, C.c_int32, dp, dp]
         L.cuharm_get_stats.argtypes = [vp, C.POINTER(C.c_int64)]
+        L.cuharm_get_chain_stats.argtypes = [vp, C.POINTER(C.c_int64)]
         L.cuharm_use_graph.argtypes = [vp, C.c_int32]
         L.cuharm_launch_count.argtypes = [vp]
         L.cuharm_launch_count.restype = C.c_int64
@@ -156,6 +159,15 @@ def cuharm_cons_to_prim(h, U, prim_inout, flag=None):
     _check(lib().cuharm_cons_to_prim(h, _dptr(U), _dptr(prim_inout), _dptr(flag)), "cuharm_cons_to_prim")
 
 
+def cuharm_repair(h, prim, flag):
+    _check(lib().cuharm_repair(h, _dptr(prim), _dptr(flag)), "cuharm_repair")
+
+
+def cuharm_invert_fallback(h, method: int, U, US, prim_inout, flag=None):
+    _check(lib().cuharm_invert_fallback(h, int(method), _dptr(U), _dptr(US), _dptr(prim_inout), _dptr(flag)),
+           "cuharm_invert_fallback")
+
+
 def cuharm_prim_to_cons(h, prim, U):
     _check(lib().cuharm_prim_to_cons(h, _dptr(prim), _dptr(U)), "cuharm_prim_to_cons")
 
@@ -200,6 +212,12 @@ def cuharm_flux_dir(h, prim, direction: int, F, cw=None):
 def cuharm_get_stats(h):
     out = (C.c_int64 * 8)()
     _check(lib().cuharm_get_stats(h, out), "cuharm_get_stats")
+    return list(out)
+
+
+def cuharm_get_chain_stats(h):
+    out = (C.c_int64 * 4)()
+    _check(lib().cuharm_get_chain_stats(h, out), "cuharm_get_chain_stats")
     return list(out)
 
 
@@ -269,6 +287,8 @@ class Solver:
     def divb(self): return cuharm_divb(self.h)
     def shell_fluxes(self, i): return cuharm_shell_fluxes(self.h, i)
     def stats(self): return cuharm_get_stats(self.h)
+    def chain_stats(self): return cuharm_get_chain_stats(self.h)
+    def repair(self, prim, flag): cuharm_repair(self.h, prim, flag)
     def use_graph(self, on=True): cuharm_use_graph(self.h, on)
     def launch_count(self): return cuharm_launch_count(self.h)
     def set_timing(self, on=True): cuharm_set_timing(self.h, on)
@@ -292,6 +312,13 @@ class Solver:
         out = guess.clone()
         flag = torch.zeros(self.shape[1:], dtype=torch.int32, device=self.device)
         cuharm_cons_to_prim(self.h, U, out, flag)
+        return out, flag
+
+    def invert_fallback(self, method, U, guess, US=None):
+        import torch
+        out = guess.clone()
+        flag = torch.zeros(self.shape[1:], dtype=torch.int32, device=self.device)
+        cuharm_invert_fallback(self.h, method, U, US, out, flag)
         return out, flag
 
     def flux_dir(self, prim, direction):

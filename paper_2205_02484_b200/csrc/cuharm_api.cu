@@ -33,8 +33,14 @@ int cuda_fail(cudaError_t e, const char* what) {
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 // counters block (unsigned long long slots)
-enum { CNT_STATS = 0, CNT_NFAIL = 8, CNT_CWPRED = 10, CNT_CWSCR = 13, CNT_DIVB = 16, CNT_CLOCK = 18, CNT_TOTAL = 32 };
-// CNT_CLOCK: two doubles, the step size of the current step and the integrated time (set_dt_kernel, dt_from_cw_kernel)
+// [CNT_NFAIL, CNT_STEP_END) is zeroed at the start of every step: failure counts of the two substeps, the c_w maxima of
+// predictor and corrector, and per substep CNT_FIXW slots of repair / fallback-chain scratch ([0] grid-barrier counter of
+// the repair, [1..] zones left waiting after each repair pass, [CNT_FIXW - 1] zones still failed after the chain).
+// CNT_CLOCK: two doubles, the step size of the current step and the integrated time (set_dt_kernel, dt_from_cw_kernel).
+// CNT_CHAIN: the four counters of cuharm_get_chain_stats.
+enum { CNT_STATS = 0, CNT_NFAIL = 8, CNT_CWPRED = 10, CNT_CWSCR = 13, CNT_FIX = 16, CNT_FIXW = 24, CNT_STEP_END = 64,
+       CNT_DIVB = 64, CNT_CLOCK = 66, CNT_CHAIN = 68, CNT_TOTAL = 80 };
+constexpr int FIXUP_MAX_PASSES_CAP = CNT_FIXW - 3;
 
 }  // namespace
 
@@ -48,7 +54,7 @@ struct cuharm_ctx {
   double* prim = nullptr;
   char* ws = nullptr;
   Geom *gC = nullptr, *gF1 = nullptr, *gF2 = nullptr;
-  double *conn = nullptr, *floors = nullptr, *F[3] = {nullptr, nullptr, nullptr}, *E = nullptr, *Phalf = nullptr;
+  double *conn = nullptr, *floors = nullptr, *F[3] = {nullptr, nullptr, nullptr}, *E = nullptr, *Phalf = nullptr, *ustar = nullptr;
   int *flag = nullptr, *list = nullptr;
   unsigned long long* cnt = nullptr;
   bool bound = false, have_geom = false, stepped = false;
@@ -93,10 +99,10 @@ struct DevGuard {
 namespace {
 
 struct WsLayout {
-  size_t gC, gF1, gF2, conn, floors, F[3], E, Phalf, flag, list, cnt, total;
+  size_t gC, gF1, gF2, conn, floors, F[3], E, Phalf, flag, list, cnt, ustar, total;
 };
 
-WsLayout layout(const Dims& d) {
+WsLayout layout(const Dims& d, bool chain) {
   WsLayout L;
   size_t off = 0;
   const size_t ncol = (size_t)d.n1g * d.n2g, nz = (size_t)d.nz;
@@ -112,11 +118,13 @@ WsLayout layout(const Dims& d) {
   L.flag = take(nz * sizeof(int));
   L.list = take(nz * sizeof(int));
   L.cnt = take(CNT_TOTAL * sizeof(unsigned long long));
+  L.ustar = take(chain ? 8 * nz * sizeof(double) : 0);  // U* of every zone, only with the fallback chain on
   L.total = off;
   return L;
 }
 
 NewtonCfg newton_cfg(const cuharm_params& p) { return NewtonCfg{p.newton_tol, p.newton_maxit, p.newton_extra}; }
+ChainCfg chain_cfg(const cuharm_params& p) { return ChainCfg{p.inv_chain, p.brent_maxit, p.beta_min, p.brent_tol}; }
 FloorCfg floor_cfg(const cuharm_params& p) {
   return FloorCfg{p.sigma_max, p.b2_over_u_max, p.gamma_max, p.sigma_max > 0.0 ? 1.0 / p.sigma_max : 0.0,
                   p.b2_over_u_max > 0.0 ? 1.0 / p.b2_over_u_max : 0.0};
@@ -296,7 +304,7 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
     Timed t_(h, CUHARM_K_UPDATE);
     UpdArgs a{d, Pbase, Pflux, Pout, h->F[0], h->F[1], h->F[2], h->E, h->gC, h->conn, h->floors, h->flag, h->list,
               nfail, h->cnt + CNT_STATS, reinterpret_cast<const double*>(h->cnt + CNT_CLOCK), dtfac, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], h->p.gam,
-              newton_cfg(h->p), floor_cfg(h->p)};
+              newton_cfg(h->p), floor_cfg(h->p), chain_cfg(h->p), h->ustar};
     dim3 grid((d.n3 + 127) / 128, d.n2, d.n1);
     if (tma) {
       const int tb = d.n3 <= 64 ? 64 : 128;
@@ -309,27 +317,49 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
       for (int w = 1; w <= UPD_STRIP && w <= d.n2; w++)
         if (d.n2 % w == 0) wj = w;
       const bool same = Pflux == Pbase;
-      if (tb == 64) {
-        if (same) update_tma_kernel<true, 64><<<nb, 64, smem, h->stream>>>(a, ntiles, nch, wj);
-        else update_tma_kernel<false, 64><<<nb, 64, smem, h->stream>>>(a, ntiles, nch, wj);
+      auto go = [&](auto kern, int threads) { kern<<<nb, threads, smem, h->stream>>>(a, ntiles, nch, wj); };
+      if (h->p.inv_chain) {
+        if (tb == 64) same ? go(update_tma_kernel<true, 64, true>, 64) : go(update_tma_kernel<false, 64, true>, 64);
+        else same ? go(update_tma_kernel<true, 128, true>, 128) : go(update_tma_kernel<false, 128, true>, 128);
       } else {
-        if (same) update_tma_kernel<true, 128><<<nb, 128, smem, h->stream>>>(a, ntiles, nch, wj);
-        else update_tma_kernel<false, 128><<<nb, 128, smem, h->stream>>>(a, ntiles, nch, wj);
+        if (tb == 64) same ? go(update_tma_kernel<true, 64, false>, 64) : go(update_tma_kernel<false, 64, false>, 64);
+        else same ? go(update_tma_kernel<true, 128, false>, 128) : go(update_tma_kernel<false, 128, false>, 128);
       }
     } else {
-      if (Pflux == Pbase) update_kernel<true><<<grid, 128, 0, h->stream>>>(a);
-      else update_kernel<false><<<grid, 128, 0, h->stream>>>(a);
+      const bool same = Pflux == Pbase;
+      if (h->p.inv_chain) {
+        if (same) update_kernel<true, true><<<grid, 128, 0, h->stream>>>(a);
+        else update_kernel<false, true><<<grid, 128, 0, h->stream>>>(a);
+      } else {
+        if (same) update_kernel<true, false><<<grid, 128, 0, h->stream>>>(a);
+        else update_kernel<false, false><<<grid, 128, 0, h->stream>>>(a);
+      }
     }
     h->launches++;
   }
   CK(cudaGetLastError());
+  if (h->p.inv_chain) {  // 1D-W and entropy methods on the listed zones, before anything reads Pout
+    Timed t_(h, CUHARM_K_FIXUP);
+    ChainArgs a{d, Pflux, Pout, h->gC, h->gF1, h->gF2, h->floors, h->flag, h->list, h->ustar, nfail,
+                h->cnt + CNT_FIX + which * CNT_FIXW + CNT_FIXW - 1, h->cnt + CNT_STATS, h->cnt + CNT_CHAIN,
+                reinterpret_cast<const double*>(h->cnt + CNT_CLOCK), dtfac, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], h->p.gam,
+                newton_cfg(h->p), floor_cfg(h->p), chain_cfg(h->p)};
+    const int nb = 2 * h->sms, rc_ = h->p.recon, rm_ = h->p.riemann;
+    if (rc_ == 0 && rm_ == 0) chain_kernel<0, 0><<<nb, 128, 0, h->stream>>>(a);
+    else if (rc_ == 0) chain_kernel<0, 1><<<nb, 128, 0, h->stream>>>(a);
+    else if (rm_ == 0) chain_kernel<1, 0><<<nb, 128, 0, h->stream>>>(a);
+    else chain_kernel<1, 1><<<nb, 128, 0, h->stream>>>(a);
+    h->launches++;
+    CK(cudaGetLastError());
+  }
   int rc = launch_bc(h, Pout, nullptr);
   if (rc) return rc;
   {
     Timed t_(h, CUHARM_K_FIXUP);
-    FixArgs a{d, Pout, h->flag, h->list, nfail, h->cnt + CNT_STATS, h->gC, h->floors, h->p.fixup_max_passes, h->p.gam,
-              newton_cfg(h->p), floor_cfg(h->p)};
-    fixup_kernel<<<1, 1024, 0, h->stream>>>(a);
+    unsigned long long* fixw = h->cnt + CNT_FIX + which * CNT_FIXW;
+    FixArgs a{d, Pout, h->flag, h->list, nfail, h->p.inv_chain ? fixw + CNT_FIXW - 1 : nullptr, h->cnt + CNT_STATS, fixw, h->gC,
+              h->floors, h->p.fixup_max_passes, h->p.gam, newton_cfg(h->p), floor_cfg(h->p)};
+    fixup_kernel<<<h->sms, FIX_THREADS, 0, h->stream>>>(a);  // at most one block per multiprocessor (grid barrier)
     h->launches++;
   }
   CK(cudaGetLastError());
@@ -340,7 +370,7 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
 // dt_from_cw_kernel), so this sequence -- and the graph recorded from it -- is the same for every dt
 int enqueue_step(cuharm_ctx* h) {
   // per-step counters: failure counts of the two substeps, the c_w maxima of predictor and corrector
-  CK(cudaMemsetAsync(h->cnt + CNT_NFAIL, 0, (CNT_DIVB - CNT_NFAIL) * sizeof(unsigned long long), h->stream));
+  CK(cudaMemsetAsync(h->cnt + CNT_NFAIL, 0, (CNT_STEP_END - CNT_NFAIL) * sizeof(unsigned long long), h->stream));
   int rc = substep(h, h->prim, h->prim, h->Phalf, 0.5, 0);  // predictor: fluxes and source from P^n, dtau = dt/2
   if (rc) return rc;
   return substep(h, h->Phalf, h->prim, h->prim, 1.0, 1);    // corrector: from the half-step state, in place, dtau = dt
@@ -386,7 +416,8 @@ int check_params(const cuharm_params* p) {
     if (bcs[c] < 0 || bcs[c] > 3) return CUHARM_EINVAL;
   if (p->bc_x1 == 2 || p->bc_x3 == 2) return CUHARM_EINVAL;  // the polar reflection belongs to X2
   if (p->bc_x2 == 2 && p->n2 < p->ng) return CUHARM_EINVAL;  // a mirror image needs ng interior zones
-  if (!(p->gam > 1.0) || !(p->newton_tol > 0.0) || p->newton_maxit < 1 || p->newton_extra < 0 || p->fixup_max_passes < 0)
+  if (!(p->gam > 1.0) || !(p->newton_tol > 0.0) || p->newton_maxit < 1 || p->newton_extra < 0 || p->fixup_max_passes < 0 ||
+      p->fixup_max_passes > FIXUP_MAX_PASSES_CAP)
     return CUHARM_EINVAL;
   if (p->coords == 0) {
     if (!(p->r_in - p->R0 > 0.0) || !(p->r_out > p->r_in) || !(std::fabs(p->a) <= 1.0)) return CUHARM_EINVAL;
@@ -468,8 +499,11 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
       blocks = sms * per;  // persistent grid: every SM filled with as many blocks as fit
       return true;
     };
-    h->upd_tma = setup(update_tma_kernel<true, 128>, update_tma_kernel<false, 128>, 128, h->upd_blocks) &&
-                 setup(update_tma_kernel<true, 64>, update_tma_kernel<false, 64>, 64, h->upd_blocks64);
+    h->upd_tma = p->inv_chain
+                     ? setup(update_tma_kernel<true, 128, true>, update_tma_kernel<false, 128, true>, 128, h->upd_blocks) &&
+                           setup(update_tma_kernel<true, 64, true>, update_tma_kernel<false, 64, true>, 64, h->upd_blocks64)
+                     : setup(update_tma_kernel<true, 128, false>, update_tma_kernel<false, 128, false>, 128, h->upd_blocks) &&
+                           setup(update_tma_kernel<true, 64, false>, update_tma_kernel<false, 64, false>, 64, h->upd_blocks64);
     if (!h->upd_tma) cudaGetLastError();
     {
       int dev = 0, sms = 0;
@@ -482,12 +516,12 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
   return CUHARM_OK;
 }
 
-size_t cuharm_workspace_bytes(cuharm_handle h) { return h ? layout(h->d).total : 0; }
+size_t cuharm_workspace_bytes(cuharm_handle h) { return h ? layout(h->d, h->p.inv_chain != 0).total : 0; }
 
 int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_bytes) {
   if (!h || !d_prim || !d_workspace) return CUHARM_EINVAL;
   if (((uintptr_t)d_workspace & 255) || ((uintptr_t)d_prim & 15)) return CUHARM_EINVAL;
-  const WsLayout L = layout(h->d);
+  const WsLayout L = layout(h->d, h->p.inv_chain != 0);
   if (ws_bytes < L.total) return CUHARM_ENOMEM;
   DevGuard dg_(h);
   const bool same_ws = h->ws == (char*)d_workspace;
@@ -500,6 +534,7 @@ int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_by
   h->E = (double*)(h->ws + L.E); h->Phalf = (double*)(h->ws + L.Phalf);
   h->flag = (int*)(h->ws + L.flag); h->list = (int*)(h->ws + L.list);
   h->cnt = (unsigned long long*)(h->ws + L.cnt);
+  h->ustar = h->p.inv_chain ? (double*)(h->ws + L.ustar) : nullptr;
   if (!same_ws) h->have_geom = false;
   // a recorded graph holds the array addresses: it stays valid only if both are unchanged
   if (h->gexec && !(same_ws && same_prim)) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
@@ -618,6 +653,20 @@ int cuharm_cons_to_prim(cuharm_handle h, const double* d_U, double* d_prim_inout
   const Dims& d = h->d;
   ConvArgs a{d, d_U, d_prim_inout, d_flag, h->gC, h->p.gam, newton_cfg(h->p)};
   cons_to_prim_kernel<<<dim3((d.n3g + 127) / 128, d.n2g, d.n1g), 128, 0, h->stream>>>(a);
+  h->launches++;
+  CK(cudaGetLastError());
+  return CUHARM_OK;
+}
+
+int cuharm_invert_fallback(cuharm_handle h, int32_t method, const double* d_U, const double* d_US, double* d_prim_inout,
+                           int32_t* d_flag) {
+  if (!h || !d_U || !d_prim_inout || method < 1 || method > 2 || (method == 2 && !d_US)) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  if (h->p.brent_maxit < 1 || !(h->p.brent_tol >= 0.0)) return CUHARM_EINVAL;
+  DevGuard dg_(h);
+  const Dims& d = h->d;
+  FallbackArgs a{d, d_U, d_US, d_prim_inout, d_flag, h->gC, h->p.gam, method, chain_cfg(h->p)};
+  fallback_kernel<<<dim3((d.n3g + 127) / 128, d.n2g, d.n1g), 128, 0, h->stream>>>(a);
   h->launches++;
   CK(cudaGetLastError());
   return CUHARM_OK;
@@ -744,6 +793,25 @@ int cuharm_apply_floors(cuharm_handle h, double* d_prim, int32_t* d_mask) {
   return CUHARM_OK;
 }
 
+int cuharm_repair(cuharm_handle h, double* d_prim, const int32_t* d_flag) {
+  if (!h || !d_prim || !d_flag) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  DevGuard dg_(h);
+  const Dims& d = h->d;
+  unsigned long long* nfail = h->cnt + CNT_NFAIL;
+  unsigned long long* fixw = h->cnt + CNT_FIX;
+  CK(cudaMemsetAsync(h->cnt + CNT_NFAIL, 0, (CNT_STEP_END - CNT_NFAIL) * sizeof(unsigned long long), h->stream));
+  repair_list_kernel<<<dim3((d.n3g + 127) / 128, d.n2g, d.n1g), 128, 0, h->stream>>>(d, d_flag, h->flag, h->list, nfail);
+  FixArgs a{d, d_prim, h->flag, h->list, nfail, nullptr, h->cnt + CNT_STATS, fixw, h->gC, h->floors, h->p.fixup_max_passes,
+            h->p.gam, newton_cfg(h->p), floor_cfg(h->p)};
+  fixup_kernel<<<h->sms, FIX_THREADS, 0, h->stream>>>(a);
+  h->launches += 2;
+  CK(cudaGetLastError());
+  // the library's flag array goes back to "all good" (its state between steps)
+  CK(cudaMemsetAsync(h->flag, 0, (size_t)d.nz * sizeof(int), h->stream));
+  return CUHARM_OK;
+}
+
 int cuharm_flux_dir(cuharm_handle h, const double* d_prim, int32_t dir, double* d_F, double* d_cw) {
   if (!h || !d_prim || !d_F || dir < 1 || dir > 3) return CUHARM_EINVAL;
   if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
@@ -758,6 +826,15 @@ int cuharm_get_stats(cuharm_handle h, int64_t out[8]) {
   if (!h->bound) return CUHARM_ESTATE;
   DevGuard dg_(h);
   CK(cudaMemcpyAsync(out, h->cnt + CNT_STATS, 8 * sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return CUHARM_OK;
+}
+
+int cuharm_get_chain_stats(cuharm_handle h, int64_t out[4]) {
+  if (!h || !out) return CUHARM_EINVAL;
+  if (!h->bound) return CUHARM_ESTATE;
+  DevGuard dg_(h);
+  CK(cudaMemcpyAsync(out, h->cnt + CNT_CHAIN, 4 * sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
   return CUHARM_OK;
 }

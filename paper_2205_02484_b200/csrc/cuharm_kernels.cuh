@@ -4,6 +4,7 @@
 // every geometry read is a broadcast (the metric is phi-independent).
 #pragma once
 #include "cuharm_flux.cuh"
+#include "cuharm_chain.cuh"
 
 namespace cuharm {
 
@@ -175,6 +176,8 @@ struct UpdArgs {
   double idx1, idx2, idx3, gam;
   NewtonCfg nc;
   FloorCfg fc;
+  ChainCfg cc;    // fallback chain: when on, U* of every zone goes to ustar and the zones of eq. 33 are
+  double* ustar;  // listed without trying the 2D method; chain_kernel then works through the list
 };
 
 // Per-zone work once the streamed operands are in registers.  pb = P^n, pf = the state the fluxes were built from
@@ -206,7 +209,7 @@ __device__ __forceinline__ void zone_divergence(const UpdArgs& a, const double f
   }
 }
 
-template <bool SAME>
+template <bool SAME, bool CHAIN>
 __device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8], const double pf[8], const double dU[8],
                                             const Geom& G, const double* cn, double rfl, double ufl, double dtau,
                                             long long idx, int q2, bool live, int cnt[5]) {
@@ -216,6 +219,11 @@ __device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8]
   fluid_state(pb, G, S);
   double U[8];
   flux_vector<0>(pb, S, G, a.gam, U);
+  bool ent_first = false;
+  if (CHAIN && a.cc.beta_min > 0.0) {  // eq. 33: beta of P^n, p_g / (p_g + b^2/2), IEEE division
+    const double pg = (a.gam - 1.0) * pb[1];
+    ent_first = pg / (pg + 0.5 * S.bsq) < a.cc.beta_min;
+  }
   double src[4];
   if (SAME) {
     source_term(pb, S, G, cn, a.gam, src);
@@ -232,7 +240,21 @@ __device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8]
 #pragma unroll
   for (int v = 0; v < 8; v++) pn[v] = pb[v];  // A35: the guess is P^n
   int its = 0;
-  const int flag = invert_2d(U, G, a.gam, pn, a.nc, its);
+  int flag;
+  if (CHAIN) {
+    if (live) {
+#pragma unroll
+      for (int v = 0; v < 8; v++) a.ustar[v * d.nz + idx] = U[v];
+    }
+    if (ent_first) {
+      flag = KIND_ENTROPY_FIRST;
+      pn[5] = U[5] * G.isg; pn[6] = U[6] * G.isg; pn[7] = U[7] * G.isg;
+    } else {
+      flag = invert_2d(U, G, a.gam, pn, a.nc, its);
+    }
+  } else {
+    flag = invert_2d(U, G, a.gam, pn, a.nc, its);
+  }
   int m = 0;
   if (flag == 0) {
     m = apply_floors(pn, G, a.C + q2, rfl, ufl, a.fc, a.gam, a.nc);
@@ -264,7 +286,7 @@ __device__ __forceinline__ void update_stats(const UpdArgs& a, const int cnt[5])
 
 // Generic kernel: per-thread loads (any n3, any alignment).  One thread per interior zone; out-of-range lanes of the
 // ragged tail work on a clamped copy of the last zone and store nothing.
-template <bool SAME>
+template <bool SAME, bool CHAIN>
 __global__ void __launch_bounds__(128, 3) update_kernel(UpdArgs a) {
   const Dims& d = a.d;
   const int k = d.ng + blockIdx.x * 128 + threadIdx.x;
@@ -299,7 +321,7 @@ __global__ void __launch_bounds__(128, 3) update_kernel(UpdArgs a) {
   int cnt[5] = {0, 0, 0, 0, 0};
   double dU[8];
   zone_divergence(a, fx, ex, dU);
-  update_zone<SAME>(a, pb, pf, dU, G, cn, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), a.dtfac * __ldg(a.dt), idx, q2,
+  update_zone<SAME, CHAIN>(a, pb, pf, dU, G, cn, __ldg(a.floors + 2 * q2), __ldg(a.floors + 2 * q2 + 1), a.dtfac * __ldg(a.dt), idx, q2,
                     live, cnt);
   update_stats(a, cnt);
 }
@@ -334,7 +356,7 @@ struct TileCnt { int s, i, jj, c; };  // mixed-radix tile counter: j-strip, i, j
 // (serial) Newton iteration.
 constexpr int UPD_TMA_MINB = 3;
 // TB = zones (threads) per tile: 128, or 64 for short rows (n3 <= 64), which would leave half a 128-zone tile idle.
-template <bool SAME, int TB>
+template <bool SAME, int TB, bool CHAIN>
 __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kernel(UpdArgs a, int ntiles, int nch, int wj) {
   constexpr int UPD_ROW = upd_row(TB);
   extern __shared__ __align__(128) double rows[];  // [UPD_NROW][UPD_ROW]
@@ -501,7 +523,7 @@ __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kern
     // the per-(i,j) records of this tile stay valid in their own (double-buffered) slot for the whole tile
     const double* tb = tab + (n & 1) * 64;
     const Geom Gc = load_geom_shared(tb);
-    update_zone<SAME>(a, pb, pf, dU, Gc, tb + 20, tb[60], tb[61], dtau, idx, q2, live, cnt);
+    update_zone<SAME, CHAIN>(a, pb, pf, dU, Gc, tb + 20, tb[60], tb[61], dtau, idx, q2, live, cnt);
 #pragma unroll
     for (int q = 0; q < 5; q++) cnt_acc[q] += cnt[q];
   }
@@ -510,21 +532,30 @@ __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kern
 
 // ---------------------------------------------------------------------------------------------------------
 // S8  Repair of zones whose inversion failed (eq. 34; A13): deterministic Jacobi passes over the
-// (short) list of failed zones.  Pass m: a still-bad zone whose 4 face neighbours in the (I,J) plane were all
+// list of failed zones.  Pass m: a still-bad zone whose 4 face neighbours in the (I,J) plane were all
 // good at the start of the pass takes their mean; else the 4 diagonal neighbours; else it waits; in the last
 // pass leftovers take the mean of whatever good zones exist among the 8 neighbours.  Only rho, u, utilde^i are
 // replaced; floors are re-applied to the repaired zone.  flag > 0: bad; flag = -(m+1): repaired in
-// pass m, i.e. good from pass m+1 on — which is what makes the passes Jacobi without a snapshot: donors are
-// zones that are not written in the current pass.  One block: failures are rare (none in the first 1000 steps
-// of the torus workloads); the list has room for every zone, so a pathological step is slow but still right.
+// pass m, i.e. good from pass m+1 on -- which is what makes the passes Jacobi without a snapshot: donors are
+// zones that are not written in the current pass.
+//
+// Grid-wide: the list is dealt to min(gridDim.x, ceil(nf / 256)) blocks (the others leave at once), and the passes
+// are separated by a grid barrier on a device counter (monotonic, zeroed with the per-step counters).  The grid has
+// at most one block per multiprocessor, so every participating block is resident as soon as whatever else shares
+// the device drains: the barrier cannot deadlock.  With nothing failed (every step of the torus workloads' first
+// 1000) the kernel is one read and an exit; with a handful of failures one block does the work without touching the
+// barrier; a step with 1e6 failures is spread over the whole device.  Reads of flags and donors bypass L1 (other
+// blocks write them between passes).
 // ---------------------------------------------------------------------------------------------------------
 struct FixArgs {
   Dims d;
   double* P;
   int* flag;
   const int* list;
-  const unsigned long long* nfail;
+  const unsigned long long* nfail;   // entries of the list
+  const unsigned long long* nbad;    // zones still failed after the fallback chain (null: every entry of the list)
   unsigned long long* stats;
+  unsigned long long* sync;          // [0] barrier counter, [1 + pass] zones left waiting after pass
   const Geom* C;
   const double* floors;
   int max_passes;
@@ -535,25 +566,42 @@ struct FixArgs {
 
 __device__ __forceinline__ bool zone_good(int f, int pass) { return f == 0 || (f < 0 && -f - 1 < pass); }
 
-__global__ void __launch_bounds__(1024) fixup_kernel(FixArgs a) {
+constexpr int FIX_THREADS = 256;
+
+__device__ __forceinline__ void fix_grid_barrier(unsigned long long* bar, unsigned long long target) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(bar, 1ull);
+    while (*reinterpret_cast<volatile unsigned long long*>(bar) < target) __nanosleep(64);
+    __threadfence();
+  }
+  __syncthreads();
+}
+
+__global__ void __launch_bounds__(FIX_THREADS) fixup_kernel(FixArgs a) {
   const Dims& d = a.d;
   const unsigned long long nf = *a.nfail;
   if (nf == 0ull) return;
-  if (threadIdx.x == 0) atomicAdd(a.stats + 0, nf);
+  const unsigned long long want = (nf + FIX_THREADS - 1) / FIX_THREADS;
+  const unsigned nb = (unsigned)(want < gridDim.x ? want : gridDim.x);  // participating blocks
+  if (blockIdx.x >= nb) return;
+  if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(a.stats + 0, a.nbad ? *a.nbad : nf);
   const long long fo[4] = {d.s1, -d.s1, d.s2, -d.s2};
   const long long dg[4] = {d.s1 + d.s2, d.s1 - d.s2, -d.s1 + d.s2, -d.s1 - d.s2};
   unsigned long long repaired = 0ull, lastres = 0ull;
+  const unsigned long long stride = (unsigned long long)nb * FIX_THREADS;
   for (int pass = 0; pass <= a.max_passes; pass++) {
     const bool last = pass == a.max_passes;
     int left = 0;
-    for (unsigned long long e = threadIdx.x; e < nf; e += blockDim.x) {
+    for (unsigned long long e = (unsigned long long)blockIdx.x * FIX_THREADS + threadIdx.x; e < nf; e += stride) {
       const long long idx = a.list[e];
-      if (a.flag[idx] <= 0) continue;
+      if (__ldcg(a.flag + idx) <= 0) continue;
       bool fg = true, dgood = true;
 #pragma unroll
       for (int m = 0; m < 4; m++) {
-        fg = fg && zone_good(a.flag[idx + fo[m]], pass);
-        dgood = dgood && zone_good(a.flag[idx + dg[m]], pass);
+        fg = fg && zone_good(__ldcg(a.flag + idx + fo[m]), pass);
+        dgood = dgood && zone_good(__ldcg(a.flag + idx + dg[m]), pass);
       }
       double q[8];
       if (fg || dgood) {
@@ -562,7 +610,7 @@ __global__ void __launch_bounds__(1024) fixup_kernel(FixArgs a) {
         for (int v = 0; v < 5; v++) {
           double s = 0.0;
 #pragma unroll
-          for (int m = 0; m < 4; m++) s += a.P[v * d.nz + idx + st[m]];
+          for (int m = 0; m < 4; m++) s += __ldcg(a.P + v * d.nz + idx + st[m]);
           q[v] = 0.25 * s;
         }
       } else if (last) {
@@ -572,20 +620,20 @@ __global__ void __launch_bounds__(1024) fixup_kernel(FixArgs a) {
           for (int dj = -1; dj <= 1; dj++) {
             if (!di && !dj) continue;
             const long long n = idx + di * d.s1 + dj * d.s2;
-            if (!zone_good(a.flag[n], pass)) continue;
+            if (!zone_good(__ldcg(a.flag + n), pass)) continue;
             cnt++;
 #pragma unroll
-            for (int v = 0; v < 5; v++) s[v] += a.P[v * d.nz + n];
+            for (int v = 0; v < 5; v++) s[v] += __ldcg(a.P + v * d.nz + n);
           }
 #pragma unroll
-        for (int v = 0; v < 5; v++) q[v] = cnt > 0 ? s[v] / cnt : a.P[v * d.nz + idx];
+        for (int v = 0; v < 5; v++) q[v] = cnt > 0 ? s[v] / cnt : __ldcg(a.P + v * d.nz + idx);
         lastres++;
       } else {
         left = 1;
         continue;
       }
 #pragma unroll
-      for (int v = 5; v < 8; v++) q[v] = a.P[v * d.nz + idx];
+      for (int v = 5; v < 8; v++) q[v] = __ldcg(a.P + v * d.nz + idx);
       const int q2 = (int)(idx / d.s2);  // = i * n2g + j
       const Geom G = load_geom(a.C, q2);
       apply_floors(q, G, a.C + q2, a.floors[2 * q2], a.floors[2 * q2 + 1], a.fc, a.gam, a.nc);
@@ -594,11 +642,34 @@ __global__ void __launch_bounds__(1024) fixup_kernel(FixArgs a) {
       a.flag[idx] = -(pass + 1);
       repaired++;
     }
-    __threadfence_block();
-    if (!__syncthreads_or(left)) break;
+    if (last) break;
+    // anything left waiting anywhere?  (one atomic per block that has some; read after the barrier)
+    const int any = __syncthreads_or(left);
+    if (nb == 1) {
+      __threadfence_block();
+      if (!any) break;
+    } else {
+      if (any && threadIdx.x == 0) atomicAdd(a.sync + 1 + pass, 1ull);
+      fix_grid_barrier(a.sync, (unsigned long long)nb * (pass + 1));
+      if (__ldcg(a.sync + 1 + pass) == 0ull) break;
+    }
   }
   if (repaired) atomicAdd(a.stats + 1, repaired);
   if (lastres) atomicAdd(a.stats + 7, lastres);
+}
+
+// Stage-level test helper (cuharm_repair): the list of failed zones from a caller's flag array (interior zones with
+// flag > 0 -> list, everything else -> 0 in the library's own flag array), so that fixup_kernel can be run on any
+// pattern of failures.  The order of the list is irrelevant: the passes are Jacobi.
+__global__ void __launch_bounds__(128) repair_list_kernel(Dims d, const int* flag_in, int* flag, int* list, unsigned long long* nfail) {
+  const int k = blockIdx.x * 128 + threadIdx.x;
+  if (k >= d.n3g) return;
+  const int j = blockIdx.y, i = blockIdx.z;
+  const long long idx = i * d.s1 + j * d.s2 + k;
+  const bool in = i >= d.ng && i < d.ng + d.n1 && j >= d.ng && j < d.ng + d.n2 && k >= d.ng && k < d.ng + d.n3;
+  const int f = in && flag_in[idx] > 0 ? flag_in[idx] : 0;
+  flag[idx] = f;
+  if (f) list[atomicAdd(nfail, 1ull)] = (int)idx;
 }
 
 // ---------------------------------------------------------------------------------------------------------
