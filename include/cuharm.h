@@ -74,6 +74,10 @@ typedef struct {
   double beta_min;     /* eq. 33 (A37): zones with p_g / (p_g + b^2/2) < beta_min at the previous time
                           level take the entropy method as first and only choice; <= 0 disables; needs inv_chain  */
   double brent_tol;    /* relative tolerance of the Brent solver (A40)                                            */
+  int32_t polar_damp;  /* 1: after inversion + floors of every substep utilde^2 of the two zones nearest each pole is
+                          replaced by the straight line in X^2 through zero at the pole and the third zone's value
+                          ("interpolation to zero at the pole"; A16).  Needs bc_x2 = 2 and n2 >= 6.  0: off     */
+  int32_t reserved;    /* must be 0                                                                               */
 } cuharm_params;
 
 /* Create a context for the grid and scheme described by *p (the statement of the problem: spin a, adiabatic

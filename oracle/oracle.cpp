@@ -53,6 +53,8 @@ struct oracle_params {
   int32_t brent_maxit;  // iteration cap of the Brent solver
   double beta_min;      // eq. 33: p_g / (p_g + b^2/2) of P^n below this -> entropy inversion first and only; <= 0 disables
   double brent_tol;     // relative tolerance of the Brent solver (A40)
+  int32_t polar_damp;   // 1: the polar velocity of the two zones nearest each pole is interpolated to zero at the pole (A16)
+  int32_t reserved;     // keeps the block a multiple of 8 bytes; must be 0
 };
 
 }  // extern "C"
@@ -1088,6 +1090,30 @@ void fixup(Ctx& c, double* P) {
 }
 
 // ------------------------------------------------------------------------------------------
+// SURVEY 8(f)3, second half -- "to increase the numerical stability in the polar region, the polar component of the
+// 4-velocity in the two cells closest to the pole is modified, by an interpolation to zero at the pole".
+// A16 (the paper gives no formula): in the two zones nearest each pole, J = 0, 1 and J = N2-1, N2-2, the primitive
+// utilde^2 is replaced by the straight line in X^2 through zero at the pole (X^2 = -1 or +1) and the value of the
+// third zone (J = 2 or N2-3) of the same (I, K).  Applied to the result of inversion + floors of every substep, before
+// the ghost fill (whose reflection continues the same line across the pole); only with the polar reflection in X^2
+// and at least 6 zones.  "parity unpinned" for the choice of variable and anchor zone; the linearity is pinned.
+// ------------------------------------------------------------------------------------------
+void polar_damp(Ctx& c, double* P) {
+  const int ng = c.ng, n1 = c.p.n1, n2 = c.p.n2, n3 = c.p.n3;
+  if (c.p.bc_x2 != 2 || n2 < 6) return;
+  auto X2 = [&](int J) { return c.x0[1] + (J + 0.5) * c.dx[1]; };   // centre of zone J (interior numbering)
+  const double north = c.x0[1], south = c.x0[1] + n2 * c.dx[1];
+  for (int i = ng; i < ng + n1; i++)
+    for (int k = ng; k < ng + n3; k++)
+      for (int m = 0; m < 2; m++) {
+        double a = P[c.vidx(3, i, ng + 2, k)];
+        P[c.vidx(3, i, ng + m, k)] = a * (X2(m) - north) / (X2(2) - north);
+        double b = P[c.vidx(3, i, ng + n2 - 3, k)];
+        P[c.vidx(3, i, ng + n2 - 1 - m, k)] = b * (south - X2(n2 - 1 - m)) / (south - X2(n2 - 3));
+      }
+}
+
+// ------------------------------------------------------------------------------------------
 // C-9  One RK2 substep (eq. 25; A5 source added; A34 order; A35 guess).
 // ------------------------------------------------------------------------------------------
 void substep(Ctx& c, const double* Pflux, const double* Pbase, double dtau, double* Pout, bool record_cw) {
@@ -1175,6 +1201,7 @@ void substep(Ctx& c, const double* Pflux, const double* Pbase, double dtau, doub
       }
   c.stats[2] += nfl_rho; c.stats[3] += nfl_u; c.stats[4] += nceil; c.stats[5] += ncap; c.stats[6] += nits;
   c.chain[0] += nchain; c.chain[1] += n1dw; c.chain[2] += nent; c.chain[3] += nbeta;
+  if (c.p.polar_damp) polar_damp(c, Pout);   // P:L311; A16
   // A34: ghosts are refreshed before the repair (so that ghost donors belong to the same state) and after it
   apply_bc(c, Pout);
   fixup(c, Pout);
@@ -1355,6 +1382,9 @@ int oracle_bind(oracle_handle h, double* prim) {
 }
 
 int oracle_apply_bc(oracle_handle h, double* prim) { apply_bc(h->c, prim); return 0; }
+
+// stage-level: the polar-velocity interpolation of P:L311 (A16) on a caller-provided primitive array, in place
+int oracle_polar_damp(oracle_handle h, double* prim) { polar_damp(h->c, prim); return 0; }
 
 // one full RK2 step in place (eq. 25)
 int oracle_step(oracle_handle h, double dt) {

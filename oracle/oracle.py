@@ -32,6 +32,7 @@ class OracleParams(C.Structure):
         ("r_break", C.c_double),
         ("inv_chain", C.c_int32), ("brent_maxit", C.c_int32),
         ("beta_min", C.c_double), ("brent_tol", C.c_double),
+        ("polar_damp", C.c_int32), ("reserved", C.c_int32),
     ]
 
 
@@ -239,6 +240,11 @@ class Grid:
     def apply_bc(self, prim: np.ndarray):
         assert prim.dtype == np.float64 and prim.flags.c_contiguous and prim.shape == (8,) + self.shape
         lib().oracle_apply_bc(self._h, _d(prim))
+
+    def polar_damp(self, prim: np.ndarray):
+        """P:L311 (A16) as a stage: utilde^2 of the two zones nearest each pole interpolated to zero at the pole."""
+        assert prim.dtype == np.float64 and prim.flags.c_contiguous and prim.shape == (8,) + self.shape
+        lib().oracle_polar_damp(self._h, _d(prim))
 
     def step(self, dt: float):
         rc = lib().oracle_step(self._h, C.c_double(dt))

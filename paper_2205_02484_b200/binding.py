@@ -34,6 +34,7 @@ class CuharmParams(C.Structure):
         ("r_break", C.c_double),
         ("inv_chain", C.c_int32), ("brent_maxit", C.c_int32),
         ("beta_min", C.c_double), ("brent_tol", C.c_double),
+        ("polar_damp", C.c_int32), ("reserved", C.c_int32),
     ]
 
 

@@ -352,6 +352,12 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
     h->launches++;
     CK(cudaGetLastError());
   }
+  if (h->p.polar_damp) {  // P:L311; A16
+    Timed t_(h, CUHARM_K_BC);
+    polar_damp_kernel<<<dim3((d.n3 + 127) / 128, d.n1, 2), 128, 0, h->stream>>>(d, Pout);
+    h->launches++;
+    CK(cudaGetLastError());
+  }
   int rc = launch_bc(h, Pout, nullptr);
   if (rc) return rc;
   {
@@ -426,6 +432,8 @@ int check_params(const cuharm_params* p) {
     for (int c = 0; c < 3; c++)
       if (!(p->xmax[c] > p->xmin[c])) return CUHARM_EINVAL;
   }
+  if (p->polar_damp < 0 || p->polar_damp > 1 || p->reserved != 0) return CUHARM_EINVAL;
+  if (p->polar_damp && (p->bc_x2 != 2 || p->n2 < 6)) return CUHARM_EINVAL;
   if (p->inv_chain < 0 || p->inv_chain > 1) return CUHARM_EINVAL;
   if (p->inv_chain && (p->brent_maxit < 1 || !(p->brent_tol >= 0.0) || !std::isfinite(p->beta_min))) return CUHARM_EINVAL;
   if ((long long)(p->n1 + 2 * p->ng) * (p->n2 + 2 * p->ng) * (p->n3 + 2 * p->ng) > 2000000000LL) return CUHARM_EINVAL;

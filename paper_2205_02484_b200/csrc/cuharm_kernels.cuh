@@ -658,6 +658,22 @@ __global__ void __launch_bounds__(FIX_THREADS) fixup_kernel(FixArgs a) {
   if (lastres) atomicAdd(a.stats + 7, lastres);
 }
 
+// P:L311 (A16): utilde^2 of the two zones nearest each pole <- the straight line in X^2 through zero at the pole and
+// the value of the third zone of the same (i, k): weights (m + 1/2) / (2 + 1/2), m = 0, 1 (uniform spacing in X^2).
+// One thread per (i, k) and pole.  Runs on the output of the update kernel, before the ghost fill.
+__global__ void __launch_bounds__(128) polar_damp_kernel(Dims d, double* P) {
+  const int k = d.ng + blockIdx.x * 128 + threadIdx.x;
+  if (k >= d.ng + d.n3) return;
+  const int i = d.ng + blockIdx.y;
+  double* u2 = P + 3 * d.nz + i * d.s1 + k;
+  const bool south = blockIdx.z != 0;
+  const int j2 = south ? d.ng + d.n2 - 3 : d.ng + 2;   // anchor row
+  const int step = south ? 1 : -1;                      // towards the pole
+  const double a = u2[j2 * d.s2];
+  u2[(j2 + step) * d.s2] = a * (1.5 / 2.5);
+  u2[(j2 + 2 * step) * d.s2] = a * (0.5 / 2.5);
+}
+
 // Stage-level test helper (cuharm_repair): the list of failed zones from a caller's flag array (interior zones with
 // flag > 0 -> list, everything else -> 0 in the library's own flag array), so that fixup_kernel can be run on any
 // pattern of failures.  The order of the list is irrelevant: the passes are Jacobi.
