@@ -54,7 +54,7 @@ struct cuharm_ctx {
   double* prim = nullptr;
   char* ws = nullptr;
   Geom *gC = nullptr, *gF1 = nullptr, *gF2 = nullptr;
-  double *conn = nullptr, *floors = nullptr, *F[3] = {nullptr, nullptr, nullptr}, *E = nullptr, *Phalf = nullptr, *ustar = nullptr;
+  double *conn = nullptr, *srcw = nullptr, *floors = nullptr, *F[3] = {nullptr, nullptr, nullptr}, *E = nullptr, *Phalf = nullptr, *ustar = nullptr;
   int *flag = nullptr, *list = nullptr;
   unsigned long long* cnt = nullptr;
   bool bound = false, have_geom = false, stepped = false;
@@ -99,7 +99,7 @@ struct DevGuard {
 namespace {
 
 struct WsLayout {
-  size_t gC, gF1, gF2, conn, floors, F[3], E, Phalf, flag, list, cnt, ustar, total;
+  size_t gC, gF1, gF2, conn, srcw, floors, F[3], E, Phalf, flag, list, cnt, ustar, total;
 };
 
 WsLayout layout(const Dims& d, bool chain) {
@@ -111,6 +111,7 @@ WsLayout layout(const Dims& d, bool chain) {
   L.gF1 = take(ncol * sizeof(Geom));
   L.gF2 = take(ncol * sizeof(Geom));
   L.conn = take(ncol * 40 * sizeof(double));
+  L.srcw = take(ncol * 14 * sizeof(double));
   L.floors = take(ncol * 2 * sizeof(double));
   for (int k = 0; k < 3; k++) L.F[k] = take(7 * nz * sizeof(double));
   L.E = take(3 * nz * sizeof(double));
@@ -168,7 +169,7 @@ int launch_bc(cuharm_ctx* h, double* P, const unsigned long long* gate) {
 // waves x (faces per segment + 0.6) among the counts that keep segments at least 16 faces long.
 int march_seg(long long columns, int nfaces, int sms) {
   const long long col_blocks = (columns + 127) / 128;
-  const long long slots = 2LL * (sms > 0 ? sms : 148);
+  const long long slots = (long long)MARCH_MINB * (sms > 0 ? sms : 148);
   const int maxseg = nfaces >= 32 ? nfaces / 16 : 1;
   int best = 1;
   double best_cost = 1e300;
@@ -302,7 +303,7 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
   unsigned long long* nfail = h->cnt + CNT_NFAIL + which;
   {
     Timed t_(h, CUHARM_K_UPDATE);
-    UpdArgs a{d, Pbase, Pflux, Pout, h->F[0], h->F[1], h->F[2], h->E, h->gC, h->conn, h->floors, h->flag, h->list,
+    UpdArgs a{d, Pbase, Pflux, Pout, h->F[0], h->F[1], h->F[2], h->E, h->gC, h->srcw, h->floors, h->flag, h->list,
               nfail, h->cnt + CNT_STATS, reinterpret_cast<const double*>(h->cnt + CNT_CLOCK), dtfac, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], h->p.gam,
               newton_cfg(h->p), floor_cfg(h->p), chain_cfg(h->p), h->ustar};
     dim3 grid((d.n3 + 127) / 128, d.n2, d.n1);
@@ -537,7 +538,7 @@ int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_by
   h->prim = d_prim;
   h->ws = (char*)d_workspace;
   h->gC = (Geom*)(h->ws + L.gC); h->gF1 = (Geom*)(h->ws + L.gF1); h->gF2 = (Geom*)(h->ws + L.gF2);
-  h->conn = (double*)(h->ws + L.conn); h->floors = (double*)(h->ws + L.floors);
+  h->conn = (double*)(h->ws + L.conn); h->srcw = (double*)(h->ws + L.srcw); h->floors = (double*)(h->ws + L.floors);
   for (int k = 0; k < 3; k++) h->F[k] = (double*)(h->ws + L.F[k]);
   h->E = (double*)(h->ws + L.E); h->Phalf = (double*)(h->ws + L.Phalf);
   h->flag = (int*)(h->ws + L.flag); h->list = (int*)(h->ws + L.list);
@@ -567,7 +568,7 @@ int cuharm_metric_precompute(cuharm_handle h) {
   const Dims& d = h->d;
   GeomArgs a{d.n1g, d.n2g, d.ng, d.n2, p.coords, (p.coords == 0 && p.bc_x2 == 2) ? 1 : 0, p.a, p.R0, p.hslope,
              h->xb, h->nx, h->x0[0], h->x0[1], h->dx[0], h->dx[1], p.rho_fl_coef, p.rho_fl_pow, p.rho_fl_abs, p.u_fl_coef,
-             p.u_fl_pow, p.u_fl_abs, h->gC, h->gF1, h->gF2, h->conn, h->floors};
+             p.u_fl_pow, p.u_fl_abs, h->gC, h->gF1, h->gF2, h->conn, h->srcw, h->floors};
   const int n = d.n1g * d.n2g;
   geom_kernel<<<(n + 63) / 64, 64, 0, h->stream>>>(a);
   h->launches++;

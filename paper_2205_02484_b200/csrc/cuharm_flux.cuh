@@ -128,7 +128,10 @@ constexpr int MARCH_PF1 = 2, MARCH_PF2 = 1;
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 template <int DIR, int RECON, int RIEMANN, bool STAGE, bool GEO>
-__global__ void __launch_bounds__(128, 2) flux_march_kernel(FluxArgs a) {
+#ifndef MARCH_MINB
+#define MARCH_MINB 2
+#endif
+__global__ void __launch_bounds__(128, MARCH_MINB) flux_march_kernel(FluxArgs a) {
   static_assert(DIR == 1 || DIR == 2, "marching kernel: directions 1 and 2");
   const Dims& d = a.d;
   const int nk = a.hi3 - a.lo3 + 1;

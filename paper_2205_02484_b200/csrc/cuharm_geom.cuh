@@ -16,7 +16,8 @@ struct GeomArgs {
   double x0_1, x0_2, dx1, dx2;
   double rho_fl_coef, rho_fl_pow, rho_fl_abs, u_fl_coef, u_fl_pow, u_fl_abs;
   Geom *C, *F1, *F2;
-  double* conn;    // [n1g*n2g][40]
+  double* conn;    // [n1g*n2g][40]  (export helper only)
+  double* srcw;    // [n1g*n2g][14]  source weights (source_weights below)
   double* floors;  // [n1g*n2g][2]
 };
 
@@ -94,8 +95,9 @@ __device__ inline void mks_geom(const GeomArgs& A, double X1, double X2, bool on
   G.pad = 0.0;
 }
 
-// Gamma^l_{nk} = 1/2 g^{ls} (d_n g_{sk} + d_k g_{sn} - d_s g_{nk}); the metric depends on X1, X2 only.
-__device__ inline void mks_conn(const GeomArgs& A, double X1, double X2, const Geom& G, double* out40) {
+// d_c g_{mn} (c = 1, 2; the metric depends on X1, X2 only) in closed form: eq. 38 differentiated in r and theta and
+// pushed through the diagonal Jacobian J = diag(1, r', theta', 1), including the dJ/dX terms (A19).
+__device__ inline void mks_dmetric(const GeomArgs& A, double X1, double X2, double dg[4][4][4]) {
   const MksPoint p = mks_point(A, X1, X2);
   const double a = A.a, r = p.r;
   const double sn = sin(p.th), cs = cos(p.th);
@@ -123,7 +125,6 @@ __device__ inline void mks_conn(const GeomArgs& A, double X1, double X2, const G
   const double J[4] = {1.0, p.rp, p.thp, 1.0};
   const double J1[4] = {0.0, p.rpp, 0.0, 0.0};   // dJ/dX1 = r'' (= r' on the plain exponential branch)
   const double J2[4] = {0.0, 0.0, p.thpp, 0.0};  // dJ/dX2
-  double dg[4][4][4];                            // dg[m][n][c] = d_c g_{mn}
   for (int m = 0; m < 4; m++)
     for (int n = 0; n < 4; n++) {
       dg[m][n][0] = 0.0;
@@ -131,6 +132,10 @@ __device__ inline void mks_conn(const GeomArgs& A, double X1, double X2, const G
       dg[m][n][1] = (J1[m] * J[n] + J[m] * J1[n]) * k[m][n] + J[m] * J[n] * kr[m][n] * p.rp;
       dg[m][n][2] = (J2[m] * J[n] + J[m] * J2[n]) * k[m][n] + J[m] * J[n] * kt[m][n] * p.thp;
     }
+}
+
+// Gamma^l_{nk} = 1/2 g^{ls} (d_n g_{sk} + d_k g_{sn} - d_s g_{nk})
+__device__ inline void mks_conn(const double dg[4][4][4], const Geom& G, double* out40) {
   double gc[4][4] = {};
   gc[0][0] = G.c00; gc[0][1] = gc[1][0] = G.c01; gc[0][3] = gc[3][0] = G.c03; gc[1][1] = G.c11;
   gc[1][3] = gc[3][1] = G.c13; gc[2][2] = G.c22; gc[3][3] = G.c33;
@@ -145,17 +150,29 @@ __device__ inline void mks_conn(const GeomArgs& A, double X1, double X2, const G
   }
 }
 
+// Source weights.  With T^{kl} symmetric, eq. 7's S_nu = sqrt(-g) T^k_l Gamma^l_{nu k} = sqrt(-g) T^{ks} Gamma_{s nu k}
+// and the last two terms of Gamma_{s nu k} = (d_nu g_{sk} + d_k g_{s nu} - d_s g_{nu k})/2 are antisymmetric in (k, s):
+// S_nu = (1/2) sqrt(-g) T^{kl} d_nu g_{kl}, a sum over the 7 metric entries that do not vanish identically (the
+// off-diagonal ones counted twice), for nu = 1, 2 (nu = t, phi: zero, the metric depends on neither).
+// w[7 (nu - 1) + e] = sqrt(-g) x (1/2 or 1) x d_nu g_e, e over 00 01 03 11 13 22 33.
+__device__ inline void source_weights(const double dg[4][4][4], double sg, double* w14) {
+  const int em[7] = {0, 0, 0, 1, 1, 2, 3}, en[7] = {0, 1, 3, 1, 3, 2, 3};
+  for (int nu = 1; nu <= 2; nu++)
+    for (int e = 0; e < 7; e++) w14[7 * (nu - 1) + e] = sg * (em[e] == en[e] ? 0.5 : 1.0) * dg[em[e]][en[e]][nu];
+}
+
 __global__ void geom_kernel(GeomArgs A) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= A.n1g * A.n2g) return;
   const int i = t / A.n2g, j = t % A.n2g;
   const int I = i - A.ng, Jz = j - A.ng;
   Geom C, F1, F2;
-  double cn[40];
+  double cn[40], sw[14];
   double rc = 1.0;
   if (A.coords == 1) {
     flat_geom(C); flat_geom(F1); flat_geom(F2);
     for (int s = 0; s < 40; s++) cn[s] = 0.0;
+    for (int s = 0; s < 14; s++) sw[s] = 0.0;
   } else {
     // the same rounding as a plain product-then-sum: keeps the face coordinate of the polar faces exact
     const double X1c = __dadd_rn(A.x0_1, __dmul_rn(I + 0.5, A.dx1)), X2c = __dadd_rn(A.x0_2, __dmul_rn(Jz + 0.5, A.dx2));
@@ -164,11 +181,15 @@ __global__ void geom_kernel(GeomArgs A) {
     mks_geom(A, X1f, X2c, false, F1);
     const bool axis = A.polar_bc && (Jz == 0 || Jz == A.n2);
     mks_geom(A, X1c, X2f, axis, F2);
-    mks_conn(A, X1c, X2c, C, cn);
+    double dg[4][4][4];
+    mks_dmetric(A, X1c, X2c, dg);
+    mks_conn(dg, C, cn);
+    source_weights(dg, C.sg, sw);
     rc = mks_point(A, X1c, X2c).r;
   }
   A.C[t] = C; A.F1[t] = F1; A.F2[t] = F2;
   for (int s = 0; s < 40; s++) A.conn[(size_t)t * 40 + s] = cn[s];
+  for (int s = 0; s < 14; s++) A.srcw[(size_t)t * 14 + s] = sw[s];
   A.floors[2 * t + 0] = fmax(A.rho_fl_abs, A.rho_fl_coef * pow(rc, A.rho_fl_pow));  // eq. 35 (A9)
   A.floors[2 * t + 1] = fmax(A.u_fl_abs, A.u_fl_coef * pow(rc, A.u_fl_pow));
 }

@@ -165,7 +165,7 @@ struct UpdArgs {
   double* Pout;
   const double *F1, *F2, *F3, *E;
   const Geom* C;
-  const double* conn;
+  const double* srcw;   // [n1g*n2g][14] source weights
   const double* floors;
   int* flag;
   int* list;                    // failed zones of this substep
@@ -316,8 +316,12 @@ __global__ void __launch_bounds__(128, 3) update_kernel(UpdArgs a) {
     ex[8] = __ldg(E3); ex[9] = __ldg(E3 + d.s1); ex[10] = __ldg(E3 + d.s2); ex[11] = __ldg(E3 + d.s1 + d.s2);
   }
   const Geom G = load_geom(a.C, q2);
-  double cn[40];
-  load_conn(a.conn + (size_t)q2 * 40, cn);
+  double cn[14];
+#pragma unroll
+  for (int s = 0; s < 7; s++) {
+    const double2 v = __ldg(reinterpret_cast<const double2*>(a.srcw + (size_t)q2 * 14) + s);
+    cn[2 * s] = v.x; cn[2 * s + 1] = v.y;
+  }
   int cnt[5] = {0, 0, 0, 0, 0};
   double dU[8];
   zone_divergence(a, fx, ex, dU);
@@ -339,7 +343,7 @@ __global__ void __launch_bounds__(128, 3) update_kernel(UpdArgs a) {
 // and div B stays at round-off exactly as with the stored EMFs.
 __host__ __device__ constexpr int upd_row(int tb) { return tb + 4; }  // doubles per staged row: 1 + TB + 1 (k+1) + 2 pad, a multiple of 16 B
 constexpr int UPD_NROW = 63;   // 8 P^n, 8 P-flux, 10 F1, 10 F2, 5 F3 (hydro), 22 induction-flux rows
-constexpr int UPD_TAB = 62;    // doubles of per-(i,j) records staged behind the rows: Geom 20, connection 40, floors 2
+constexpr int UPD_TAB = 36;    // doubles of per-(i,j) records staged behind the rows: Geom 20, source weights 14, floors 2
 __host__ __device__ constexpr int upd_smem(int tb) { return (UPD_NROW * upd_row(tb) + 2 * 64) * 8; }  // dynamic shared memory per block
 
 // Stage rows: 0..7 P^n; 8..15 P-flux; 16..25 F1 hydro, (i+1, i) per component; 26..35 F2 hydro, (j+1, j) per component;
@@ -402,7 +406,7 @@ __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kern
   // and the tile indices), so each bulk copy is a handful of uniform-datapath instructions; per-lane operands would
   // make the compiler serialise the lanes in an elect loop that waits on the previous copy.
   constexpr int NWARP = TB / 32;
-  double* const tab = rows + UPD_NROW * UPD_ROW;  // two slots of [20] geometry record, [40] connection, [2] floors
+  double* const tab = rows + UPD_NROW * UPD_ROW;  // two slots of [20] geometry record, [14] source weights, [2] floors
   // Rows are dealt to the warps in four groups of contiguous stage rows (two groups for 64-thread blocks), and
   // inside a group the source addresses are walked with running byte pointers (one 64-bit add per row or less),
   // following the row table above.
@@ -465,8 +469,8 @@ __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kern
       const size_t q = (size_t)(d.ng + x.i) * d.n2g + (d.ng + x.j);
       double* const tb = tab + slot * 64;
       bulk_g2s(smem_u32(tb), a.C + q, 160u, bar0);
-      bulk_g2s(smem_u32(tb + 20), a.conn + q * 40, 320u, bar0);
-      bulk_g2s(smem_u32(tb + 60), a.floors + q * 2, 16u, bar0);
+      bulk_g2s(smem_u32(tb + 20), a.srcw + q * 14, 112u, bar0);
+      bulk_g2s(smem_u32(tb + 34), a.floors + q * 2, 16u, bar0);
     }
   };
   if (tile < ntiles) issue(cur, 0);
@@ -523,7 +527,7 @@ __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kern
     // the per-(i,j) records of this tile stay valid in their own (double-buffered) slot for the whole tile
     const double* tb = tab + (n & 1) * 64;
     const Geom Gc = load_geom_shared(tb);
-    update_zone<SAME, CHAIN>(a, pb, pf, dU, Gc, tb + 20, tb[60], tb[61], dtau, idx, q2, live, cnt);
+    update_zone<SAME, CHAIN>(a, pb, pf, dU, Gc, tb + 20, tb[34], tb[35], dtau, idx, q2, live, cnt);
 #pragma unroll
     for (int q = 0; q < 5; q++) cnt_acc[q] += cnt[q];
   }

@@ -335,47 +335,31 @@ __device__ __forceinline__ void face_flux(const double pl[8], const double pr[8]
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Geometric source S_nu = sqrt(-g) T^kappa_lambda Gamma^lambda_{nu kappa} (eq. 7; eq. 14).
-// conn: 40 doubles, Gamma^l_{nk} with l-major and the (n,k) pair order 00 01 02 03 11 12 13 22 23 33.
+// Geometric source S_nu = sqrt(-g) T^kappa_lambda Gamma^lambda_{nu kappa} (eq. 7; eq. 14),
+// evaluated as (1/2) sqrt(-g) T^{kl} d_nu g_{kl} (identical: T^{kl} is symmetric, see source_weights in
+// cuharm_geom.cuh).  sw: the 14 precomputed weights of this (i, j): sqrt(-g) x (1/2 | 1) x d_nu g_e for nu = 1, 2 and
+// e over the metric entries 00 01 03 11 13 22 33.  nu = t and nu = phi vanish identically (the metric depends on
+// neither: energy and angular-momentum conservation) and are not formed.  src = (S_t, S_1, S_2, S_3).
 // ---------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ constexpr int pair_index(int n, int k) {
-  // index of the unordered pair (n,k) in 00 01 02 03 11 12 13 22 23 33
-  const int lo = n < k ? n : k, hi = n < k ? k : n;
-  return lo * 4 - (lo * (lo - 1)) / 2 + (hi - lo);
-}
-
-__device__ __forceinline__ void load_conn(const double* __restrict__ conn, double cn[40]) {
-  const double2* c2 = reinterpret_cast<const double2*>(conn);
-#pragma unroll
-  for (int s = 0; s < 20; s++) { const double2 v = __ldg(c2 + s); cn[2 * s] = v.x; cn[2 * s + 1] = v.y; }
-}
-
-template <bool KILLING = true>
-__device__ __forceinline__ void source_term(const double q[8], const State& S, const Geom& G, const double* cn,
-                                            double gam, double src[4]) {
+__device__ __forceinline__ void source_term(const double q[8], const State& S, const Geom& G, const double* sw, double gam,
+                                            double src[4]) {
   const double pg = (gam - 1.0) * q[1];
   const double w = q[0] + q[1] + pg;
   const double eta = w + S.bsq;
   const double ptot = fma(0.5, S.bsq, pg);
-  const double uc[4] = {S.u0, S.u1, S.u2, S.u3}, ul[4] = {S.l0, S.l1, S.l2, S.l3};
-  const double bc[4] = {S.b0, S.b1, S.b2, S.b3}, bl[4] = {S.m0, S.m1, S.m2, S.m3};
-  // nu = t and nu = phi: T^k_l Gamma^l_{nu k} = (1/2) T^{kl} d_nu g_kl vanishes identically because the metric
-  // depends on neither t nor phi (energy and angular-momentum conservation); the contraction would return its own
-  // round-off, so the two sums are not formed (KILLING = true).  Minkowski: Gamma = 0 altogether.
-  double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-#pragma unroll
-  for (int k = 0; k < 4; k++) {
-    const double eu = eta * uc[k];
-#pragma unroll
-    for (int l = 0; l < 4; l++) {
-      const double T = fma(eu, ul[l], -bc[k] * bl[l]) + (k == l ? ptot : 0.0);  // T^k_l
-      if (!KILLING) s0 = fma(T, cn[l * 10 + pair_index(0, k)], s0);
-      s1 = fma(T, cn[l * 10 + pair_index(1, k)], s1);
-      s2 = fma(T, cn[l * 10 + pair_index(2, k)], s2);
-      if (!KILLING) s3 = fma(T, cn[l * 10 + pair_index(3, k)], s3);
-    }
-  }
-  src[0] = G.sg * s0; src[1] = G.sg * s1; src[2] = G.sg * s2; src[3] = G.sg * s3;
+  const double e0 = eta * S.u0, e1 = eta * S.u1, e2 = eta * S.u2, e3 = eta * S.u3;
+  // T^{kl} = (w + b^2) u^k u^l + (p + b^2/2) g^{kl} - b^k b^l  (eq. 5), the 7 entries that meet a non-zero d g_{kl}
+  const double T00 = fma(e0, S.u0, fma(ptot, G.c00, -S.b0 * S.b0));
+  const double T01 = fma(e0, S.u1, fma(ptot, G.c01, -S.b0 * S.b1));
+  const double T03 = fma(e0, S.u3, -S.b0 * S.b3);  // g^{t phi} = 0
+  const double T11 = fma(e1, S.u1, fma(ptot, G.c11, -S.b1 * S.b1));
+  const double T13 = fma(e1, S.u3, fma(ptot, G.c13, -S.b1 * S.b3));
+  const double T22 = fma(e2, S.u2, fma(ptot, G.c22, -S.b2 * S.b2));
+  const double T33 = fma(e3, S.u3, fma(ptot, G.c33, -S.b3 * S.b3));
+  src[0] = 0.0;
+  src[1] = fma(T00, sw[0], fma(T01, sw[1], fma(T03, sw[2], fma(T11, sw[3], fma(T13, sw[4], fma(T22, sw[5], T33 * sw[6]))))));
+  src[2] = fma(T00, sw[7], fma(T01, sw[8], fma(T03, sw[9], fma(T11, sw[10], fma(T13, sw[11], fma(T22, sw[12], T33 * sw[13]))))));
+  src[3] = 0.0;
 }
 
 // ---------------------------------------------------------------------------------------------------------
