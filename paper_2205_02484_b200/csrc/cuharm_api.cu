@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -12,6 +13,7 @@
 #include "../../include/cuharm.h"
 #include "cuharm_geom.cuh"
 #include "cuharm_kernels.cuh"
+#include "cuharm_update_tmap.cuh"
 
 using namespace cuharm;
 
@@ -54,7 +56,7 @@ struct cuharm_ctx {
   double* prim = nullptr;
   char* ws = nullptr;
   Geom *gC = nullptr, *gF1 = nullptr, *gF2 = nullptr;
-  double *conn = nullptr, *srcw = nullptr, *floors = nullptr, *F[3] = {nullptr, nullptr, nullptr}, *E = nullptr, *Phalf = nullptr, *ustar = nullptr;
+  double *conn = nullptr, *srcw = nullptr, *rec = nullptr, *floors = nullptr, *F[3] = {nullptr, nullptr, nullptr}, *E = nullptr, *Phalf = nullptr, *ustar = nullptr;
   int *flag = nullptr, *list = nullptr;
   unsigned long long* cnt = nullptr;
   bool bound = false, have_geom = false, stepped = false;
@@ -68,6 +70,11 @@ struct cuharm_ctx {
   int64_t t_n[CUHARM_NCLASS] = {0};
   // graph
   bool upd_tma = false;  // update_tma_kernel usable (shared-memory opt-in succeeded)
+  bool upd_tmap = false; // update_tmap_kernel usable (opt-in succeeded, tensor maps of the bound arrays encoded)
+  bool tmap_enable = true;
+  int tmap_blocks = 0, tmap_blocks64 = 0;
+  bool maps_ok = false;
+  UpdMaps maps;
   int upd_blocks = 0, upd_blocks64 = 0;  // its persistent grid sizes (128- and 64-zone tiles)
   int sms = 148;         // multiprocessors of the device
   double xb = 0.0;       // eq. 39: X1 of the exponential -> hyper-exponential transition
@@ -99,7 +106,7 @@ struct DevGuard {
 namespace {
 
 struct WsLayout {
-  size_t gC, gF1, gF2, conn, srcw, floors, F[3], E, Phalf, flag, list, cnt, ustar, total;
+  size_t gC, gF1, gF2, conn, srcw, rec, floors, F[3], E, Phalf, flag, list, cnt, ustar, total;
 };
 
 WsLayout layout(const Dims& d, bool chain) {
@@ -112,6 +119,7 @@ WsLayout layout(const Dims& d, bool chain) {
   L.gF2 = take(ncol * sizeof(Geom));
   L.conn = take(ncol * 40 * sizeof(double));
   L.srcw = take(ncol * 14 * sizeof(double));
+  L.rec = take(ncol * 36 * sizeof(double));
   L.floors = take(ncol * 2 * sizeof(double));
   for (int k = 0; k < 3; k++) L.F[k] = take(7 * nz * sizeof(double));
   L.E = take(3 * nz * sizeof(double));
@@ -122,6 +130,48 @@ WsLayout layout(const Dims& d, bool chain) {
   L.ustar = take(chain ? 8 * nz * sizeof(double) : 0);  // U* of every zone, only with the fallback chain on
   L.total = off;
   return L;
+}
+
+// Tensor maps of the bound arrays for update_tmap_kernel (box list in cuharm_update_tmap.cuh): 4-D [component][i][j][k],
+// 8-byte elements, zero fill outside the array.  The driver's encoder is reached through the runtime
+// (cudaGetDriverEntryPoint), so the library keeps linking against the CUDA runtime only.
+bool encode_update_maps(cuharm_ctx* h) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static EncodeFn encode = nullptr;
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+      (void)cudaGetLastError();
+      return false;
+    }
+    encode = (EncodeFn)fn;
+  }
+  const Dims& d = h->d;
+  if (d.n3g % 2) return false;  // strides must be multiples of 16 bytes
+  const int tb = d.n3 <= 64 ? 64 : 128;
+  struct Box { double* base; int ncomp; unsigned bj, bi, bc; };
+  const Box boxes[TMAP_NBOX] = {
+      {h->prim, 8, 1, 1, 8}, {h->Phalf, 8, 1, 1, 8},
+      {h->F[0], 7, 1, 2, 5}, {h->F[1], 7, 2, 1, 5}, {h->F[2], 7, 1, 1, 5},
+      {h->F[1], 7, 2, 1, 1}, {h->F[2], 7, 3, 1, 1}, {h->F[2], 7, 1, 3, 1}, {h->F[0], 7, 1, 2, 1},
+      {h->F[0], 7, 3, 2, 1}, {h->F[1], 7, 2, 3, 1}};
+  for (int b = 0; b < TMAP_NBOX; b++) {
+    if ((uintptr_t)boxes[b].base % 16) return false;
+    const cuuint64_t dims[4] = {(cuuint64_t)d.n3g, (cuuint64_t)d.n2g, (cuuint64_t)d.n1g, (cuuint64_t)boxes[b].ncomp};
+    const cuuint64_t strides[3] = {(cuuint64_t)d.s2 * 8, (cuuint64_t)d.s1 * 8, (cuuint64_t)d.nz * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)(tb + 2), boxes[b].bj, boxes[b].bi, boxes[b].bc};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    if (tmap_rows(b) != (int)(boxes[b].bj * boxes[b].bi * boxes[b].bc)) return false;
+    const CUresult r = encode(&h->maps.m[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, boxes[b].base, dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return false;
+  }
+  return true;
 }
 
 NewtonCfg newton_cfg(const cuharm_params& p) { return NewtonCfg{p.newton_tol, p.newton_maxit, p.newton_extra}; }
@@ -168,7 +218,7 @@ int launch_bc(cuharm_ctx* h, double* P, const unsigned long long* gate) {
 // extra cell) and the 2 x SMs resident blocks run in waves, so the segment count is chosen to minimise
 // waves x (faces per segment + 0.6) among the counts that keep segments at least 16 faces long.
 int march_seg(long long columns, int nfaces, int sms) {
-  const long long col_blocks = (columns + 127) / 128;
+  const long long col_blocks = (columns + MARCH_T - 1) / MARCH_T;
   const long long slots = (long long)MARCH_MINB * (sms > 0 ? sms : 148);
   const int maxseg = nfaces >= 32 ? nfaces / 16 : 1;
   int best = 1;
@@ -212,17 +262,17 @@ void launch_flux_t(cuharm_ctx* h, FluxArgs& a, int dir) {
     const int nt = dir == 1 ? nj : ni;
     const long long cols = (long long)nt * nk;
     a.seg = march_seg(cols, nf, h->sms);
-    const dim3 grid((unsigned)((cols + 127) / 128), (unsigned)((nf + a.seg - 1) / a.seg));
+    const dim3 grid((unsigned)((cols + MARCH_T - 1) / MARCH_T), (unsigned)((nf + a.seg - 1) / a.seg));
     // face geometry staged per block: (rows a block's 128 columns can touch) x (faces per segment) records
-    a.geo_rows = std::min(nt, 127 / nk + 2);
+    a.geo_rows = std::min(nt, (MARCH_T - 1) / nk + 2);
     size_t gsm = (size_t)a.geo_rows * a.seg * sizeof(Geom);
     if (gsm > 40 * 1024) { a.geo_rows = 0; gsm = 0; }
     if (a.geo_rows > 0) {
-      if (dir == 1) flux_march_kernel<1, RECON, RIEMANN, STAGE, true><<<grid, 128, gsm, h->stream>>>(a);
-      else flux_march_kernel<2, RECON, RIEMANN, STAGE, true><<<grid, 128, gsm, h->stream>>>(a);
+      if (dir == 1) flux_march_kernel<1, RECON, RIEMANN, STAGE, true><<<grid, MARCH_T, gsm, h->stream>>>(a);
+      else flux_march_kernel<2, RECON, RIEMANN, STAGE, true><<<grid, MARCH_T, gsm, h->stream>>>(a);
     } else {
-      if (dir == 1) flux_march_kernel<1, RECON, RIEMANN, STAGE, false><<<grid, 128, 0, h->stream>>>(a);
-      else flux_march_kernel<2, RECON, RIEMANN, STAGE, false><<<grid, 128, 0, h->stream>>>(a);
+      if (dir == 1) flux_march_kernel<1, RECON, RIEMANN, STAGE, false><<<grid, MARCH_T, 0, h->stream>>>(a);
+      else flux_march_kernel<2, RECON, RIEMANN, STAGE, false><<<grid, MARCH_T, 0, h->stream>>>(a);
     }
   }
 }
@@ -293,8 +343,12 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
   const uintptr_t al = (uintptr_t)Pbase | (uintptr_t)Pflux | (uintptr_t)h->F[0] | (uintptr_t)h->F[1] |
                        (uintptr_t)h->F[2] | (uintptr_t)h->E;
   // (the staged row starts one zone below the tile, at ng - 1 + c TB: 16-byte aligned only for odd ng)
-  const bool tma = h->upd_tma && (d.n3g % 2 == 0) && (d.ng % 2 == 1) && (al % 16 == 0);
-  if (!tma) {
+  // tensor-map staging: the same restriction (a box that starts 8 bytes off a 16-byte boundary faults on B200, measured);
+  // it serves the library's own arrays (the maps hold their addresses)
+  const bool tmap = h->maps_ok && (d.n3g % 2 == 0) && (d.ng % 2 == 1) && Pbase == h->prim &&
+                    (Pflux == h->prim || Pflux == h->Phalf);
+  const bool tma = !tmap && h->upd_tma && (d.n3g % 2 == 0) && (d.ng % 2 == 1) && (al % 16 == 0);
+  if (!tma && !tmap) {
     Timed t_(h, CUHARM_K_EMF);
     EmfArgs a{d, h->F[0], h->F[1], h->F[2], h->E};
     emf_kernel<<<dim3((d.n3 + 1 + 127) / 128, d.n2 + 1, d.n1 + 1), 128, 0, h->stream>>>(a);
@@ -307,7 +361,26 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
               nfail, h->cnt + CNT_STATS, reinterpret_cast<const double*>(h->cnt + CNT_CLOCK), dtfac, 1.0 / h->dx[0], 1.0 / h->dx[1], 1.0 / h->dx[2], h->p.gam,
               newton_cfg(h->p), floor_cfg(h->p), chain_cfg(h->p), h->ustar};
     dim3 grid((d.n3 + 127) / 128, d.n2, d.n1);
-    if (tma) {
+    if (tmap) {
+      const int tb = d.n3 <= 64 ? 64 : 128;
+      const size_t smem = tmap_smem(tb);
+      const int nch = (d.n3 + tb - 1) / tb;
+      const long long nt = (long long)d.n1 * d.n2 * nch;
+      const int ntiles = (int)nt;
+      const int nb = (int)std::min<long long>(nt, tb == 64 ? h->tmap_blocks64 : h->tmap_blocks);
+      int wj = 1;  // strip width: the largest divisor of n2 not above UPD_STRIP
+      for (int w = 1; w <= UPD_STRIP && w <= d.n2; w++)
+        if (d.n2 % w == 0) wj = w;
+      const bool same = Pflux == Pbase;
+      auto go = [&](auto kern, int threads) { kern<<<nb, threads, smem, h->stream>>>(a, h->maps, h->rec, ntiles, nch, wj); };
+      if (h->p.inv_chain) {
+        if (tb == 64) same ? go(update_tmap_kernel<true, 64, true>, 64) : go(update_tmap_kernel<false, 64, true>, 64);
+        else same ? go(update_tmap_kernel<true, 128, true>, 128) : go(update_tmap_kernel<false, 128, true>, 128);
+      } else {
+        if (tb == 64) same ? go(update_tmap_kernel<true, 64, false>, 64) : go(update_tmap_kernel<false, 64, false>, 64);
+        else same ? go(update_tmap_kernel<true, 128, false>, 128) : go(update_tmap_kernel<false, 128, false>, 128);
+      }
+    } else if (tma) {
       const int tb = d.n3 <= 64 ? 64 : 128;
       const size_t smem = upd_smem(tb);
       const int nch = (d.n3 + tb - 1) / tb;
@@ -497,8 +570,8 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
     for (int c = 0; c < 3; c++) { h->x0[c] = p->xmin[c]; h->dx[c] = (p->xmax[c] - p->xmin[c]) / n[c]; }
   }
   {  // opt in to the dynamic shared memory of the bulk-copy update kernel (67.5 KB per block)
-    auto setup = [&](auto kern_t, auto kern_f, int tb, int& blocks) {
-      const int smem = upd_smem(tb);
+    auto setup = [&](auto kern_t, auto kern_f, int tb, int& blocks, int smem_bytes = 0) {
+      const int smem = smem_bytes ? smem_bytes : upd_smem(tb);
       int dev = 0, sms = 0, per = 0;
       if (cudaFuncSetAttribute(kern_t, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return false;
       if (cudaFuncSetAttribute(kern_f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return false;
@@ -514,6 +587,14 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
                      : setup(update_tma_kernel<true, 128, false>, update_tma_kernel<false, 128, false>, 128, h->upd_blocks) &&
                            setup(update_tma_kernel<true, 64, false>, update_tma_kernel<false, 64, false>, 64, h->upd_blocks64);
     if (!h->upd_tma) cudaGetLastError();
+    // the tensor-map version of the same kernel (the maps themselves are encoded at bind time, for the bound arrays)
+    h->upd_tmap = p->inv_chain
+                      ? setup(update_tmap_kernel<true, 128, true>, update_tmap_kernel<false, 128, true>, 128, h->tmap_blocks, tmap_smem(128)) &&
+                            setup(update_tmap_kernel<true, 64, true>, update_tmap_kernel<false, 64, true>, 64, h->tmap_blocks64, tmap_smem(64))
+                      : setup(update_tmap_kernel<true, 128, false>, update_tmap_kernel<false, 128, false>, 128, h->tmap_blocks, tmap_smem(128)) &&
+                            setup(update_tmap_kernel<true, 64, false>, update_tmap_kernel<false, 64, false>, 64, h->tmap_blocks64, tmap_smem(64));
+    if (!h->upd_tmap) cudaGetLastError();
+    h->tmap_enable = std::getenv("CUHARM_NO_TMAP") == nullptr;
     {
       int dev = 0, sms = 0;
       cudaGetDevice(&dev);
@@ -538,7 +619,7 @@ int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_by
   h->prim = d_prim;
   h->ws = (char*)d_workspace;
   h->gC = (Geom*)(h->ws + L.gC); h->gF1 = (Geom*)(h->ws + L.gF1); h->gF2 = (Geom*)(h->ws + L.gF2);
-  h->conn = (double*)(h->ws + L.conn); h->srcw = (double*)(h->ws + L.srcw); h->floors = (double*)(h->ws + L.floors);
+  h->conn = (double*)(h->ws + L.conn); h->srcw = (double*)(h->ws + L.srcw); h->rec = (double*)(h->ws + L.rec); h->floors = (double*)(h->ws + L.floors);
   for (int k = 0; k < 3; k++) h->F[k] = (double*)(h->ws + L.F[k]);
   h->E = (double*)(h->ws + L.E); h->Phalf = (double*)(h->ws + L.Phalf);
   h->flag = (int*)(h->ws + L.flag); h->list = (int*)(h->ws + L.list);
@@ -547,6 +628,7 @@ int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_by
   if (!same_ws) h->have_geom = false;
   // a recorded graph holds the array addresses: it stays valid only if both are unchanged
   if (h->gexec && !(same_ws && same_prim)) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+  h->maps_ok = h->upd_tmap && h->tmap_enable && encode_update_maps(h);
   h->bound = true;
   h->stepped = false;
   CK(cudaMemsetAsync(h->flag, 0, (size_t)h->d.nz * sizeof(int), h->stream));  // ghost zones always count as good
@@ -568,7 +650,7 @@ int cuharm_metric_precompute(cuharm_handle h) {
   const Dims& d = h->d;
   GeomArgs a{d.n1g, d.n2g, d.ng, d.n2, p.coords, (p.coords == 0 && p.bc_x2 == 2) ? 1 : 0, p.a, p.R0, p.hslope,
              h->xb, h->nx, h->x0[0], h->x0[1], h->dx[0], h->dx[1], p.rho_fl_coef, p.rho_fl_pow, p.rho_fl_abs, p.u_fl_coef,
-             p.u_fl_pow, p.u_fl_abs, h->gC, h->gF1, h->gF2, h->conn, h->srcw, h->floors};
+             p.u_fl_pow, p.u_fl_abs, h->gC, h->gF1, h->gF2, h->conn, h->srcw, h->floors, h->rec};
   const int n = d.n1g * d.n2g;
   geom_kernel<<<(n + 63) / 64, 64, 0, h->stream>>>(a);
   h->launches++;

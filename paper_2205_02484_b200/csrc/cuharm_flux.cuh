@@ -127,27 +127,29 @@ __device__ __forceinline__ void store_flux(const FluxArgs& a, long long idx, con
 constexpr int MARCH_PF1 = 2, MARCH_PF2 = 1;
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
+// 128 threads x 2 blocks per multiprocessor = the full register file at 255 registers per thread.  Measured on B200
+// (256^3, PPM + LLF, ms per launch): 128 x 2 at 254 registers 0.59; capped at 232 registers 0.59; 64-thread blocks at
+// 224 / 200 registers (no spills, 8 / 10 warps) 0.63 / 0.67; 168 registers (12 warps, 440 bytes spilled) 0.80 -- the
+// kernel lives on instruction-level parallelism inside a warp, not on occupancy.
+constexpr int MARCH_T = 128, MARCH_MINB = 2;
 template <int DIR, int RECON, int RIEMANN, bool STAGE, bool GEO>
-#ifndef MARCH_MINB
-#define MARCH_MINB 2
-#endif
-__global__ void __launch_bounds__(128, MARCH_MINB) flux_march_kernel(FluxArgs a) {
+__global__ void __launch_bounds__(MARCH_T, MARCH_MINB) flux_march_kernel(FluxArgs a) {
   static_assert(DIR == 1 || DIR == 2, "marching kernel: directions 1 and 2");
   const Dims& d = a.d;
   const int nk = a.hi3 - a.lo3 + 1;
   const int nt = DIR == 1 ? (a.hi2 - a.lo2 + 1) : (a.hi1 - a.lo1 + 1);
-  const int q = blockIdx.x * 128 + threadIdx.x;
+  const int q = blockIdx.x * MARCH_T + threadIdx.x;
   unsigned long long cwv = 0ull;
   // The face geometry the block will need -- the records of (faces of its segment) x (the transverse rows its 128
   // columns touch) -- is staged in shared memory once, so the march reads it with shared-memory latency.
   extern __shared__ __align__(16) double2 geo[];  // [face in segment][row][10]
-  const int t_first = (DIR == 1 ? a.lo2 : a.lo1) + (blockIdx.x * 128) / nk;
+  const int t_first = (DIR == 1 ? a.lo2 : a.lo1) + (blockIdx.x * MARCH_T) / nk;
   if (GEO) {
     const int f0 = (DIR == 1 ? a.lo1 : a.lo2) + blockIdx.y * a.seg;
     const int f1 = min(f0 + a.seg, (DIR == 1 ? a.hi1 : a.hi2) + 1);
     const int t_max = DIR == 1 ? a.hi2 : a.hi1;
     const int nrec = (f1 - f0) * a.geo_rows;
-    for (int e = threadIdx.x; e < nrec * 10; e += 128) {
+    for (int e = threadIdx.x; e < nrec * 10; e += MARCH_T) {
       const int rec = e / 10, w = e - rec * 10;
       const int f = f0 + rec / a.geo_rows, tt = min(t_first + rec % a.geo_rows, t_max);
       const int g = DIR == 1 ? f * d.n2g + tt : tt * d.n2g + f;

@@ -19,6 +19,7 @@ struct GeomArgs {
   double* conn;    // [n1g*n2g][40]  (export helper only)
   double* srcw;    // [n1g*n2g][14]  source weights (source_weights below)
   double* floors;  // [n1g*n2g][2]
+  double* rec;     // [n1g*n2g][36]  centre geometry record (20) + source weights (14) + floors (2), one bulk copy per tile
 };
 
 struct MksPoint {
@@ -192,6 +193,12 @@ __global__ void geom_kernel(GeomArgs A) {
   for (int s = 0; s < 14; s++) A.srcw[(size_t)t * 14 + s] = sw[s];
   A.floors[2 * t + 0] = fmax(A.rho_fl_abs, A.rho_fl_coef * pow(rc, A.rho_fl_pow));  // eq. 35 (A9)
   A.floors[2 * t + 1] = fmax(A.u_fl_abs, A.u_fl_coef * pow(rc, A.u_fl_pow));
+  double* rec = A.rec + (size_t)t * 36;
+  const double* cg = reinterpret_cast<const double*>(&A.C[t]);
+  for (int s = 0; s < 20; s++) rec[s] = cg[s];
+  for (int s = 0; s < 14; s++) rec[20 + s] = sw[s];
+  rec[34] = A.floors[2 * t + 0];
+  rec[35] = A.floors[2 * t + 1];
 }
 
 // expand a table to the caller's SoA layout (include/cuharm.h, cuharm_get_geom)

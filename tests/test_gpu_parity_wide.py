@@ -239,3 +239,27 @@ def test_non_finite_wave_speed_gives_zero_dt():
     with pytest.raises(cu.CuharmError):
         s.step(0.0)
     s.close()
+
+
+# ------------------------------------------------------------------ tensor-map vs one-dimensional bulk-copy staging
+def test_tensor_map_update_kernel_is_bitwise_the_row_copy_kernel(monkeypatch):
+    """update_tmap_kernel (12 tensor-map boxes per tile) against update_tma_kernel (63 row copies per tile; selected by
+    CUHARM_NO_TMAP=1 at grid_init, the fallback when the driver's tensor-map encoder is unavailable): same tiles, same
+    arithmetic, same expression per edge EMF -> identical bits, for both tile widths and a ragged last tile."""
+    for name, kw in (("C4", dict(n1=20, n2=16, n3=150)), ("C3", dict(n1=24, n2=16, n3=40))):
+        p = config(name, **kw)
+        prim0, _ = fm_torus(p)
+        res = []
+        for no_tmap in (False, True):
+            if no_tmap:
+                monkeypatch.setenv("CUHARM_NO_TMAP", "1")
+            else:
+                monkeypatch.delenv("CUHARM_NO_TMAP", raising=False)
+            s = cu.Solver(p, prim0)
+            dt = s.cfl_dt(0.45)
+            for _ in range(3):
+                s.step(dt)
+            res.append((s.prim.cpu().numpy().copy(), list(s.stats()), s.divb()))
+            s.close()
+        monkeypatch.delenv("CUHARM_NO_TMAP", raising=False)
+        assert np.array_equal(res[0][0], res[1][0]) and res[0][1] == res[1][1] and res[0][2] == res[1][2]
