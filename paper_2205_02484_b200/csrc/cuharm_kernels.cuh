@@ -543,7 +543,7 @@ __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kern
 // pass m, i.e. good from pass m+1 on -- which is what makes the passes Jacobi without a snapshot: donors are
 // zones that are not written in the current pass.
 //
-// Grid-wide: the list is dealt to min(gridDim.x, ceil(nf / 256)) blocks (the others leave at once), and the passes
+// Grid-wide: the list is dealt to min(gridDim.x, ceil(nf / 512)) blocks (the others leave at once), and the passes
 // are separated by a grid barrier on a device counter (monotonic, zeroed with the per-step counters).  The grid has
 // at most one block per multiprocessor, so every participating block is resident as soon as whatever else shares
 // the device drains: the barrier cannot deadlock.  With nothing failed (every step of the torus workloads' first
@@ -570,7 +570,7 @@ struct FixArgs {
 
 __device__ __forceinline__ bool zone_good(int f, int pass) { return f == 0 || (f < 0 && -f - 1 < pass); }
 
-constexpr int FIX_THREADS = 256;
+constexpr int FIX_THREADS = 512;
 
 __device__ __forceinline__ void fix_grid_barrier(unsigned long long* bar, unsigned long long target) {
   __syncthreads();
