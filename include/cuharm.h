@@ -21,6 +21,10 @@
  *     phi source terms (the metric depends on neither).  `coords` in {0, 1} is the only geometry the library
  *     accepts; a metric with another zero pattern needs other kernels.
  *
+ *   - One environment switch, read by cuharm_grid_init: CUHARM_NO_TMAP=1 makes the update kernel stage its tiles with
+ *     one-dimensional bulk copies instead of tensor-map copies (the path taken anyway when the driver's tensor-map
+ *     encoder is unavailable); results are bit-identical (tests/test_gpu_parity_wide.py compares the two).
+ *
  * Array layout (device, fp64, C order, the last index fastest):
  *   prim[8][n1+2ng][n2+2ng][n3+2ng], variables (rho, u, utilde^1, utilde^2, utilde^3, B^1, B^2, B^3)
  *   (eq. 10).  All vector components are coordinate components in (X^1, X^2, X^3).  Zone (I,J,K) has its
