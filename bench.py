@@ -384,6 +384,66 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_decomposed(args):
+    """--decompose: the grid cut into WORLD_SIZE slabs along X1, one per rank / GPU (paper_2205_02484_b200/slab.py: halo
+    exchange over NCCL after every substep, max of the face speeds over the ranks), strong scaling: the whole job is ONE
+    grid.  Not measured on more than one GPU in this build; with one rank it times the split-step
+    path (plain launches, one host synchronisation per substep for the repair's counts) against the replayed graph."""
+    import numpy as np
+    import torch
+    import paper_2205_02484_b200 as cu
+    from paper_2205_02484_b200 import slab
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    p, prim_host = make_workload(args.config)
+    mine = np.ascontiguousarray(prim_host[:, slab.slab_slice(p, world, rank)])
+    eng = cu.Solver(slab.slab_params(p, world, rank), torch.from_numpy(mine).pin_memory(), device=f"cuda:{local}")
+    if world > 1:
+        me = slab.SlabRank(eng, p, rank, world)
+    else:
+        me = slab.SlabGroup([eng], p)
+    dt = me.cfl_dt(0.45)
+    for _ in range(max(args.warmup, 3)):
+        me.step(dt)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        me.step(dt)
+    e1.record()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    zones = p["n1"] * p["n2"] * p["n3"]
+    if rank == 0:
+        peak, peak_src, _ = peaks()
+        value = zones * args.steps / (ms * 1e-3)
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+                          "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                          "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": f"{args.config}: one {p['n1']}x{p['n2']}x{p['n3']} grid in {world} slab(s) along X1",
+                                     "parallelism": f"slab decomposition x{world}, halo exchange per substep", "dt": dt},
+                          "roofline": {"bound": "hbm", "kernel": "whole step", "achieved": value * B_ALG / 1e9 / world, "peak": peak,
+                                       "unit": "GB/s", "frac": value * B_ALG / (peak * 1e9) / world, "traffic": None, "peak_source": peak_src},
+                          "gpu_launches": int(eng.launch_count())}), flush=True)
+    eng.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def run_repair_scaling(args):
     """Cost of the eq. 34 repair (cuharm_repair: list build + the grid-wide repair kernel) on the headline grid for
     1e3 / 1e5 / 1e6 failed zones: random isolated zones plus 4 x 3 patches (diagonal stencil, later
@@ -449,12 +509,15 @@ def main():
     ap.add_argument("--sustain-warm-s", type=float, default=2.0, help="sustained leg: load before its timed region")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cfl-each-step", action="store_true", help="a new dt every step from eq. 26 (cuharm_step_cfl)")
+    ap.add_argument("--decompose", action="store_true", help="one grid cut into WORLD_SIZE slabs (strong scaling) instead of replicas")
     ap.add_argument("--repair-scaling", action="store_true", help="time the eq. 34 repair at 1e3 / 1e5 / 1e6 failed zones")
     ap.add_argument("--threads", type=int, default=0, help="reference arm: OpenMP threads of the oracle (0 = all)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.repair_scaling:
         run_repair_scaling(args)
+    elif args.decompose and args.impl == "ours":
+        run_decomposed(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

@@ -81,6 +81,12 @@ typedef struct {
   int32_t polar_damp;  /* 1: after inversion + floors of every substep utilde^2 of the two zones nearest each pole is
                           replaced by the straight line in X^2 through zero at the pole and the third zone's value
                           ("interpolation to zero at the pole"; A16).  Needs bc_x2 = 2 and n2 >= 6.  0: off     */
+  int32_t n1_global;   /* Slab decomposition along X1 (P:L271-273 splits the grid among GPUs).  > 0: this   */
+  int32_t i_offset;    /* grid is the slab of zones i_offset .. i_offset + n1 - 1 of a grid with n1_global zones in X1:  */
+  int32_t slab_lo;     /* coordinates, spacing and geometry are the full grid's.  slab_lo / slab_hi = 1: the lower /     */
+  int32_t slab_hi;     /* upper X1 side is internal: its ghost zones are never written by the ghost fill -- the caller  */
+                       /* copies the neighbouring slab's outermost ng interior planes there (halo exchange) after every */
+                       /* cuharm_substep.  0 everywhere: the whole grid (default)                                       */
   int32_t reserved;    /* must be 0                                                                               */
 } cuharm_params;
 
@@ -121,6 +127,43 @@ int cuharm_step(cuharm_handle h, double dt);
  * (dt_max <= 0: no cap) -- the value cuharm_last_cfl_dt would return, bit for bit, without the read-back and the
  * synchronisation.  Asynchronous.  Errors: ESTATE (no previous step since bind), EINVAL (xi not finite or <= 0). */
 int cuharm_step_cfl(cuharm_handle h, double xi, double dt_max);
+
+/* The same step in two calls, for a caller that exchanges halo planes between slabs (n1_global > 0): cuharm_set_dt
+ * puts the step size into the device scalar (and advances the integrated time); cuharm_substep(h, 0) is the predictor
+ * (P^n -> the half-step array, which lives in the workspace at byte offset cuharm_half_offset, layout of d_prim);
+ * cuharm_substep(h, 1) is the corrector (in place into d_prim).  After substep 0 the halo planes of the half-step array,
+ * after substep 1 those of d_prim must be refreshed from the neighbouring slabs before the next call.  The sequence
+ * set_dt, substep 0, substep 1 enqueues exactly what cuharm_step(h, dt) enqueues (plain launches).
+ * Errors: as cuharm_step; cuharm_substep(h, 1) before (h, 0): ESTATE.
+ *
+ * The eq. 34 repair (A13) reads neighbours across an internal boundary, and a zone repaired in one Jacobi pass is a
+ * donor in the next.  For slabs whose failed zones may lie next to an internal boundary the substep therefore comes in
+ * pieces as well, with a halo exchange of the substep's array AND of the flag array (int32 [n1g][n2g][n3g] in the
+ * workspace at byte offset cuharm_flag_offset; flags ride with the halo) between them:
+ *   cuharm_substep_update(h, which)        fluxes, update, inversion, floors, first ghost fill
+ *   [exchange array + flags]
+ *   cuharm_repair_pass(h, which, pass, out) for pass = 0, 1, ... <= fixup_max_passes: ONE Jacobi pass over this slab's
+ *                                          failed zones; out[0] = failed zones of this slab in this substep, out[1] =
+ *                                          zones still waiting (HOST pointer; synchronises); [exchange array + flags]
+ *                                          after every pass in which any slab had failed zones; stop when the sum of
+ *                                          out[1] over the slabs is 0 (or after pass fixup_max_passes, the last-resort one)
+ *   cuharm_substep_finish(h, which)        second ghost fill (needed only if any slab had failed zones); [exchange array]
+ * With the exchanges in place every pass sees exactly what the single-domain repair sees. */
+int cuharm_set_dt(cuharm_handle h, double dt);
+int cuharm_substep(cuharm_handle h, int32_t which);
+int cuharm_substep_update(cuharm_handle h, int32_t which);
+int cuharm_repair_pass(cuharm_handle h, int32_t which, int32_t pass, int64_t out[2]);
+int cuharm_substep_finish(cuharm_handle h, int32_t which);
+size_t cuharm_half_offset(cuharm_handle h);
+size_t cuharm_flag_offset(cuharm_handle h);
+
+/* Maxima of the face speeds c_w per direction: of the predictor of the last step (cuharm_last_cw), or of the bound
+ * primitives (cuharm_cfl_cw; overwrites the flux workspace) -- what cuharm_last_cfl_dt / cuharm_cfl_dt reduce; and eq. 26
+ * from a given triple (cuharm_dt_of_cw; host arithmetic only), so that a caller can take the maximum over slabs in
+ * between.  cw: HOST pointer to 3 doubles (+infinity where a speed was not finite).  The first two synchronise. */
+int cuharm_last_cw(cuharm_handle h, double cw[3]);
+int cuharm_cfl_cw(cuharm_handle h, double cw[3]);
+int cuharm_dt_of_cw(cuharm_handle h, double xi, const double cw[3], double* dt_out);
 
 /* Integrated time since cuharm_bind (*t, the sum of the step sizes) and the size of the last step (*dt_last);
  * either pointer may be NULL.  HOST pointers.  Synchronises. */

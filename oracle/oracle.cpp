@@ -54,6 +54,12 @@ struct oracle_params {
   double beta_min;      // eq. 33: p_g / (p_g + b^2/2) of P^n below this -> entropy inversion first and only; <= 0 disables
   double brent_tol;     // relative tolerance of the Brent solver (A40)
   int32_t polar_damp;   // 1: the polar velocity of the two zones nearest each pole is interpolated to zero at the pole (A16)
+  // this grid is a slab of a larger one, split along X1 (P:L271-273 splits along theta; the
+  // choice of direction is free).  n1_global > 0: the full grid has n1_global zones in X1 and this slab holds zones
+  // i_offset .. i_offset + n1 - 1 of it (coordinates, spacing and geometry are those of the full grid); slab_lo /
+  // slab_hi = 1: the lower / upper X1 side is an internal boundary whose ghost zones are filled by the neighbouring
+  // slab (halo exchange), never by the X1 boundary rule.
+  int32_t n1_global, i_offset, slab_lo, slab_hi;
   int32_t reserved;     // keeps the block a multiple of 8 bytes; must be 0
 };
 
@@ -821,7 +827,7 @@ void build_geometry(Ctx& c) {
   c.rc.assign(n, 1.0);
   for (int i = 0; i < c.n1g; i++)
     for (int j = 0; j < c.n2g; j++) {
-      int I = i - c.ng, J = j - c.ng;
+      int I = i - c.ng + (p.n1_global > 0 ? p.i_offset : 0), J = j - c.ng;   // global zone index in X1
       double X1c = c.x0[0] + (I + 0.5) * c.dx[0], X2c = c.x0[1] + (J + 0.5) * c.dx[1];
       double X1f = c.x0[0] + I * c.dx[0], X2f = c.x0[1] + J * c.dx[1];
       size_t q = (size_t)i * c.n2g + j;
@@ -866,6 +872,7 @@ void apply_bc(const Ctx& c, double* P) {
   if (c.p.bc_x1 != 3) {
     for (int g = 0; g < ng; g++)
       for (int side = 0; side < 2; side++) {
+        if (c.p.n1_global > 0 && (side ? c.p.slab_hi : c.p.slab_lo)) continue;  // internal side: the halo exchange fills it
         int ig = side ? (ng + n1 + g) : (ng - 1 - g);
         int is;
         if (c.p.bc_x1 == 1) is = side ? (ng + g) : (ng + n1 - 1 - g);
@@ -1026,67 +1033,79 @@ void flux_ct(Ctx& c) {
 // C-11  Fix-up of failed zones (eq. 34; A13 deterministic Jacobi passes).
 // "parity unpinned": stencil choice / pass order are DESIGN.md conventions.
 // ------------------------------------------------------------------------------------------
-void fixup(Ctx& c, double* P) {
+// One Jacobi pass over the zones flagged in `fl` (> 0 or any non-zero: failed); donors are read from a snapshot of P
+// taken at the start of the pass and must be good at the start of the pass; zones repaired in this pass are cleared in
+// `fl` at its end.  Returns the number of zones left waiting.
+int64_t fixup_pass(Ctx& c, double* P, std::vector<int32_t>& fl, int pass) {
   const int ng = c.ng, n1 = c.p.n1, n2 = c.p.n2, n3 = c.p.n3;
-  int64_t nbad = 0;
-  for (size_t q = 0; q < c.nz; q++) if (c.flag[q]) nbad++;
+  const int fo[4][2] = {{1, 0}, {-1, 0}, {0, 1}, {0, -1}};
+  const int dg[4][2] = {{1, 1}, {1, -1}, {-1, 1}, {-1, -1}};
+  bool last = (pass == c.p.fixup_max_passes);
+  std::vector<int32_t> flnew(fl);
+  std::vector<double> snap(P, P + 5 * c.nz);
+  int64_t left = 0;
+  for (int i = ng; i < ng + n1; i++)
+    for (int j = ng; j < ng + n2; j++)
+      for (int k = ng; k < ng + n3; k++) {
+        size_t q = c.idx(i, j, k);
+        if (!fl[q]) continue;
+        bool facegood = true, diaggood = true;
+        for (int m = 0; m < 4; m++) {
+          if (fl[c.idx(i + fo[m][0], j + fo[m][1], k)]) facegood = false;
+          if (fl[c.idx(i + dg[m][0], j + dg[m][1], k)]) diaggood = false;
+        }
+        const int(*st)[2] = nullptr;
+        if (facegood) st = fo; else if (diaggood) st = dg;
+        if (st) {
+          for (int v = 0; v < 5; v++) {
+            double sum = 0.0;
+            for (int m = 0; m < 4; m++) sum += snap[c.vidx(v, i + st[m][0], j + st[m][1], k)];
+            P[c.vidx(v, i, j, k)] = 0.25 * sum;
+          }
+        } else if (last) {
+          int cnt = 0;
+          double sum[5] = {0, 0, 0, 0, 0};
+          for (int di = -1; di <= 1; di++)
+            for (int dj = -1; dj <= 1; dj++) {
+              if (!di && !dj) continue;
+              if (fl[c.idx(i + di, j + dj, k)]) continue;
+              cnt++;
+              for (int v = 0; v < 5; v++) sum[v] += snap[c.vidx(v, i + di, j + dj, k)];
+            }
+          if (cnt > 0) for (int v = 0; v < 5; v++) P[c.vidx(v, i, j, k)] = sum[v] / cnt;
+          c.stats[7]++;
+        } else {
+          left++;
+          continue;
+        }
+        flnew[q] = 0;
+        c.stats[1]++;
+        // floors on the repaired zone (A34)
+        double q8[8];
+        get_prim(c, P, i, j, k, q8);
+        size_t g2 = (size_t)i * c.n2g + j;
+        apply_floors(c.p, c.rc[g2], c.gc[g2], q8);
+        for (int v = 0; v < 5; v++) P[c.vidx(v, i, j, k)] = q8[v];
+      }
+  fl.swap(flnew);
+  return left;
+}
+
+int64_t interior_failed(const Ctx& c) {
+  int64_t n = 0;
+  for (int i = c.ng; i < c.ng + c.p.n1; i++)
+    for (int j = c.ng; j < c.ng + c.p.n2; j++)
+      for (int k = c.ng; k < c.ng + c.p.n3; k++) if (c.flag[c.idx(i, j, k)]) n++;
+  return n;
+}
+
+void fixup(Ctx& c, double* P) {
+  int64_t nbad = interior_failed(c);
   c.stats[0] += nbad;
   if (!nbad) return;
   std::vector<int32_t> fl(c.flag);
-  std::vector<double> snap(5 * c.nz);
-  const int fo[4][2] = {{1, 0}, {-1, 0}, {0, 1}, {0, -1}};
-  const int dg[4][2] = {{1, 1}, {1, -1}, {-1, 1}, {-1, -1}};
-  for (int pass = 0; pass <= c.p.fixup_max_passes; pass++) {
-    bool last = (pass == c.p.fixup_max_passes);
-    std::vector<int32_t> flnew(fl);
-    std::memcpy(snap.data(), P, 5 * c.nz * sizeof(double));
-    int64_t left = 0;
-    for (int i = ng; i < ng + n1; i++)
-      for (int j = ng; j < ng + n2; j++)
-        for (int k = ng; k < ng + n3; k++) {
-          size_t q = c.idx(i, j, k);
-          if (!fl[q]) continue;
-          bool facegood = true, diaggood = true;
-          for (int m = 0; m < 4; m++) {
-            if (fl[c.idx(i + fo[m][0], j + fo[m][1], k)]) facegood = false;
-            if (fl[c.idx(i + dg[m][0], j + dg[m][1], k)]) diaggood = false;
-          }
-          const int(*st)[2] = nullptr;
-          if (facegood) st = fo; else if (diaggood) st = dg;
-          if (st) {
-            for (int v = 0; v < 5; v++) {
-              double sum = 0.0;
-              for (int m = 0; m < 4; m++) sum += snap[c.vidx(v, i + st[m][0], j + st[m][1], k)];
-              P[c.vidx(v, i, j, k)] = 0.25 * sum;
-            }
-          } else if (last) {
-            int cnt = 0;
-            double sum[5] = {0, 0, 0, 0, 0};
-            for (int di = -1; di <= 1; di++)
-              for (int dj = -1; dj <= 1; dj++) {
-                if (!di && !dj) continue;
-                if (fl[c.idx(i + di, j + dj, k)]) continue;
-                cnt++;
-                for (int v = 0; v < 5; v++) sum[v] += snap[c.vidx(v, i + di, j + dj, k)];
-              }
-            if (cnt > 0) for (int v = 0; v < 5; v++) P[c.vidx(v, i, j, k)] = sum[v] / cnt;
-            c.stats[7]++;
-          } else {
-            left++;
-            continue;
-          }
-          flnew[q] = 0;
-          c.stats[1]++;
-          // floors on the repaired zone (A34)
-          double q8[8];
-          get_prim(c, P, i, j, k, q8);
-          size_t g2 = (size_t)i * c.n2g + j;
-          apply_floors(c.p, c.rc[g2], c.gc[g2], q8);
-          for (int v = 0; v < 5; v++) P[c.vidx(v, i, j, k)] = q8[v];
-        }
-    fl.swap(flnew);
-    if (!left) break;
-  }
+  for (int pass = 0; pass <= c.p.fixup_max_passes; pass++)
+    if (!fixup_pass(c, P, fl, pass)) break;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1116,7 +1135,7 @@ void polar_damp(Ctx& c, double* P) {
 // ------------------------------------------------------------------------------------------
 // C-9  One RK2 substep (eq. 25; A5 source added; A34 order; A35 guess).
 // ------------------------------------------------------------------------------------------
-void substep(Ctx& c, const double* Pflux, const double* Pbase, double dtau, double* Pout, bool record_cw) {
+void substep(Ctx& c, const double* Pflux, const double* Pbase, double dtau, double* Pout, bool record_cw, bool with_repair = true) {
   double cwm[3];
   const bool chain = c.p.inv_chain != 0;
   for (int d = 1; d <= 3; d++) flux_dir(c, Pflux, d, c.F[d - 1], c.cw[d - 1], &cwm[d - 1], chain ? &c.FS[d - 1] : nullptr);
@@ -1124,7 +1143,9 @@ void substep(Ctx& c, const double* Pflux, const double* Pbase, double dtau, doub
   flux_ct(c);
   const int ng = c.ng, n1 = c.p.n1, n2 = c.p.n2, n3 = c.p.n3;
   std::memcpy(Pout, Pbase, 8 * c.nz * sizeof(double));
-  std::fill(c.flag.begin(), c.flag.end(), 0);
+  for (int i = ng; i < ng + n1; i++)   // (flags outside the interior are never set by this loop: with slabs they hold
+    for (int j = ng; j < ng + n2; j++)  //  the neighbour's flags, refreshed by the halo exchange)
+      for (int k = ng; k < ng + n3; k++) c.flag[c.idx(i, j, k)] = 0;
   int64_t nfl_rho = 0, nfl_u = 0, nceil = 0, ncap = 0, nits = 0;
   int64_t nchain = 0, n1dw = 0, nent = 0, nbeta = 0;
 #pragma omp parallel for reduction(+ : nfl_rho, nfl_u, nceil, ncap, nits, nchain, n1dw, nent, nbeta) schedule(static)
@@ -1204,6 +1225,7 @@ void substep(Ctx& c, const double* Pflux, const double* Pbase, double dtau, doub
   if (c.p.polar_damp) polar_damp(c, Pout);   // P:L311; A16
   // A34: ghosts are refreshed before the repair (so that ghost donors belong to the same state) and after it
   apply_bc(c, Pout);
+  if (!with_repair) return;
   fixup(c, Pout);
   apply_bc(c, Pout);
 }
@@ -1330,11 +1352,11 @@ int oracle_grid_init(oracle_handle* out, const oracle_params* p) {
   c.nz = (size_t)c.n1g * c.n2g * c.n3g;
   if (p->coords == 0) {
     c.x0[0] = std::log(p->r_in - p->R0);
-    c.dx[0] = (radial_inverse(*p, p->r_out) - c.x0[0]) / p->n1;   // uniform in X up to the X of r_out
+    c.dx[0] = (radial_inverse(*p, p->r_out) - c.x0[0]) / (p->n1_global > 0 ? p->n1_global : p->n1);   // uniform in X up to the X of r_out
     c.x0[1] = -1.0; c.dx[1] = 2.0 / p->n2;
     c.x0[2] = 0.0;  c.dx[2] = 2.0 * PI / p->n3;
   } else {
-    int n[3] = {p->n1, p->n2, p->n3};
+    int n[3] = {p->n1_global > 0 ? p->n1_global : p->n1, p->n2, p->n3};
     for (int d = 0; d < 3; d++) { c.x0[d] = p->xmin[d]; c.dx[d] = (p->xmax[d] - p->xmin[d]) / n[d]; }
   }
   build_geometry(c);
@@ -1393,6 +1415,64 @@ int oracle_step(oracle_handle h, double dt) {
   substep(c, c.prim, c.prim, 0.5 * dt, c.Phalf.data(), true);
   substep(c, c.Phalf.data(), c.prim, dt, c.Pnew.data(), false);
   std::memcpy(c.prim, c.Pnew.data(), 8 * c.nz * sizeof(double));
+  return 0;
+}
+
+// Slab decomposition: the two substeps of eq. 25 as calls of their own, so that the caller can exchange
+// the halo planes of the half-step array between them and of the primitive array after them.
+//   which = 0: predictor, P^n -> the half-step array (oracle_half);  which = 1: corrector, in place into the bound array.
+int oracle_substep(oracle_handle h, int which, double dt) {
+  Ctx& c = h->c;
+  if (!c.prim) return -2;
+  if (which == 0) {
+    substep(c, c.prim, c.prim, 0.5 * dt, c.Phalf.data(), true);
+  } else {
+    substep(c, c.Phalf.data(), c.prim, dt, c.Pnew.data(), false);
+    std::memcpy(c.prim, c.Pnew.data(), 8 * c.nz * sizeof(double));
+  }
+  return 0;
+}
+// ... and the substep itself in pieces, for slabs whose failed zones may lie next to an internal boundary: the repair's
+// Jacobi passes one by one, with a halo exchange of the array and of the flags (oracle_flags) between them.
+int oracle_substep_update(oracle_handle h, int which, double dt) {
+  Ctx& c = h->c;
+  if (!c.prim) return -2;
+  if (which == 0) substep(c, c.prim, c.prim, 0.5 * dt, c.Phalf.data(), true, false);
+  else substep(c, c.Phalf.data(), c.prim, dt, c.Pnew.data(), false, false);
+  return 0;
+}
+// out[0] = failed zones of this slab (interior) at the start of pass 0 (0 in later passes), out[1] = zones left waiting
+int oracle_repair_pass(oracle_handle h, int which, int pass, int64_t out[2]) {
+  Ctx& c = h->c;
+  double* P = which == 0 ? c.Phalf.data() : c.Pnew.data();
+  out[0] = 0;
+  if (pass == 0) { out[0] = interior_failed(c); c.stats[0] += out[0]; }
+  out[1] = fixup_pass(c, P, c.flag, pass);
+  return 0;
+}
+int oracle_substep_finish(oracle_handle h, int which) {
+  Ctx& c = h->c;
+  apply_bc(c, which == 0 ? c.Phalf.data() : c.Pnew.data());
+  return 0;
+}
+// the corrector works into a scratch array; this copies it over the bound primitives (end of the step)
+int oracle_commit(oracle_handle h) { std::memcpy(h->c.prim, h->c.Pnew.data(), 8 * h->c.nz * sizeof(double)); return 0; }
+double* oracle_new(oracle_handle h) { return h->c.Pnew.data(); }
+int32_t* oracle_flags(oracle_handle h) { return h->c.flag.data(); }
+double* oracle_half(oracle_handle h) { return h->c.Phalf.data(); }
+// the three face-speed maxima the predictor of the last step saw, and eq. 26 from a given triple (after a max over slabs)
+int oracle_last_cw(oracle_handle h, double cw[3]) { for (int d = 0; d < 3; d++) cw[d] = h->c.cwmax[d]; return 0; }
+int oracle_dt_of_cw(oracle_handle h, double xi, const double cw[3], double* dt_out) {
+  double inv = 0.0;
+  for (int d = 0; d < 3; d++) inv += cw[d] / (xi * h->c.dx[d]);
+  *dt_out = 1.0 / inv;
+  return 0;
+}
+// face-speed maxima of the bound primitives (what oracle_cfl_dt reduces)
+int oracle_cfl_cw(oracle_handle h, double cw[3]) {
+  Ctx& c = h->c;
+  if (!c.prim) return -2;
+  for (int d = 1; d <= 3; d++) flux_dir(c, c.prim, d, c.F[d - 1], c.cw[d - 1], &cw[d - 1]);
   return 0;
 }
 

@@ -32,7 +32,9 @@ class OracleParams(C.Structure):
         ("r_break", C.c_double),
         ("inv_chain", C.c_int32), ("brent_maxit", C.c_int32),
         ("beta_min", C.c_double), ("brent_tol", C.c_double),
-        ("polar_damp", C.c_int32), ("reserved", C.c_int32),
+        ("polar_damp", C.c_int32),
+        ("n1_global", C.c_int32), ("i_offset", C.c_int32), ("slab_lo", C.c_int32), ("slab_hi", C.c_int32),
+        ("reserved", C.c_int32),
     ]
 
 
@@ -240,6 +242,53 @@ class Grid:
     def apply_bc(self, prim: np.ndarray):
         assert prim.dtype == np.float64 and prim.flags.c_contiguous and prim.shape == (8,) + self.shape
         lib().oracle_apply_bc(self._h, _d(prim))
+
+    # ---- slab decomposition: split step, half-step array, face-speed maxima
+    def substep(self, which: int, dt: float):
+        assert lib().oracle_substep(self._h, int(which), C.c_double(dt)) == 0
+
+    def substep_update(self, which: int, dt: float):
+        assert lib().oracle_substep_update(self._h, int(which), C.c_double(dt)) == 0
+
+    def repair_pass(self, which: int, npass: int):
+        out = np.zeros(2, dtype=np.int64)
+        lib().oracle_repair_pass(self._h, int(which), int(npass), out.ctypes.data_as(C.POINTER(C.c_int64)))
+        return int(out[0]), int(out[1])
+
+    def substep_finish(self, which: int):
+        lib().oracle_substep_finish(self._h, int(which))
+
+    def commit(self):
+        lib().oracle_commit(self._h)
+
+    def new(self) -> np.ndarray:
+        lib().oracle_new.restype = _dp
+        return np.ctypeslib.as_array(lib().oracle_new(self._h), shape=(8,) + self.shape)
+
+    def flags(self) -> np.ndarray:
+        lib().oracle_flags.restype = _ip
+        return np.ctypeslib.as_array(lib().oracle_flags(self._h), shape=self.shape)
+
+    def half(self) -> np.ndarray:
+        lib().oracle_half.restype = _dp
+        ptr = lib().oracle_half(self._h)
+        return np.ctypeslib.as_array(ptr, shape=(8,) + self.shape)
+
+    def last_cw(self):
+        out = np.zeros(3)
+        lib().oracle_last_cw(self._h, _d(out))
+        return out
+
+    def cfl_cw(self):
+        out = np.zeros(3)
+        assert lib().oracle_cfl_cw(self._h, _d(out)) == 0
+        return out
+
+    def dt_of_cw(self, xi: float, cw) -> float:
+        cw = np.ascontiguousarray(cw, dtype=np.float64)
+        dt = C.c_double()
+        lib().oracle_dt_of_cw(self._h, C.c_double(xi), _d(cw), C.byref(dt))
+        return dt.value
 
     def polar_damp(self, prim: np.ndarray):
         """P:L311 (A16) as a stage: utilde^2 of the two zones nearest each pole interpolated to zero at the pole."""

@@ -34,7 +34,9 @@ class CuharmParams(C.Structure):
         ("r_break", C.c_double),
         ("inv_chain", C.c_int32), ("brent_maxit", C.c_int32),
         ("beta_min", C.c_double), ("brent_tol", C.c_double),
-        ("polar_damp", C.c_int32), ("reserved", C.c_int32),
+        ("polar_damp", C.c_int32),
+        ("n1_global", C.c_int32), ("i_offset", C.c_int32), ("slab_lo", C.c_int32), ("slab_hi", C.c_int32),
+        ("reserved", C.c_int32),
     ]
 
 
@@ -71,6 +73,18 @@ def lib():
         L.cuharm_metric_precompute.argtypes = [vp]
         L.cuharm_step.argtypes = [vp, C.c_double]
         L.cuharm_step_cfl.argtypes = [vp, C.c_double, C.c_double]
+        L.cuharm_set_dt.argtypes = [vp, C.c_double]
+        L.cuharm_substep.argtypes = [vp, C.c_int32]
+        L.cuharm_substep_update.argtypes = [vp, C.c_int32]
+        L.cuharm_repair_pass.argtypes = [vp, C.c_int32, C.c_int32, C.POINTER(C.c_int64)]
+        L.cuharm_substep_finish.argtypes = [vp, C.c_int32]
+        L.cuharm_flag_offset.argtypes = [vp]
+        L.cuharm_flag_offset.restype = C.c_size_t
+        L.cuharm_half_offset.argtypes = [vp]
+        L.cuharm_half_offset.restype = C.c_size_t
+        L.cuharm_last_cw.argtypes = [vp, C.POINTER(C.c_double)]
+        L.cuharm_cfl_cw.argtypes = [vp, C.POINTER(C.c_double)]
+        L.cuharm_dt_of_cw.argtypes = [vp, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.cuharm_get_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.cuharm_apply_floors.argtypes = [vp, dp, ip]
         L.cuharm_repair.argtypes = [vp, dp, ip]
@@ -216,6 +230,55 @@ def cuharm_get_stats(h):
     return list(out)
 
 
+def cuharm_set_dt(h, dt: float):
+    _check(lib().cuharm_set_dt(h, float(dt)), "cuharm_set_dt")
+
+
+def cuharm_substep(h, which: int):
+    _check(lib().cuharm_substep(h, int(which)), "cuharm_substep")
+
+
+def cuharm_substep_update(h, which: int):
+    _check(lib().cuharm_substep_update(h, int(which)), "cuharm_substep_update")
+
+
+def cuharm_repair_pass(h, which: int, npass: int):
+    out = (C.c_int64 * 2)()
+    _check(lib().cuharm_repair_pass(h, int(which), int(npass), out), "cuharm_repair_pass")
+    return int(out[0]), int(out[1])
+
+
+def cuharm_substep_finish(h, which: int):
+    _check(lib().cuharm_substep_finish(h, int(which)), "cuharm_substep_finish")
+
+
+def cuharm_flag_offset(h) -> int:
+    return int(lib().cuharm_flag_offset(h))
+
+
+def cuharm_half_offset(h) -> int:
+    return int(lib().cuharm_half_offset(h))
+
+
+def cuharm_last_cw(h):
+    out = (C.c_double * 3)()
+    _check(lib().cuharm_last_cw(h, out), "cuharm_last_cw")
+    return list(out)
+
+
+def cuharm_cfl_cw(h):
+    out = (C.c_double * 3)()
+    _check(lib().cuharm_cfl_cw(h, out), "cuharm_cfl_cw")
+    return list(out)
+
+
+def cuharm_dt_of_cw(h, xi: float, cw) -> float:
+    arr = (C.c_double * 3)(*[float(x) for x in cw])
+    dt = C.c_double()
+    _check(lib().cuharm_dt_of_cw(h, float(xi), arr, C.byref(dt)), "cuharm_dt_of_cw")
+    return dt.value
+
+
 def cuharm_get_chain_stats(h):
     out = (C.c_int64 * 4)()
     _check(lib().cuharm_get_chain_stats(h, out), "cuharm_get_chain_stats")
@@ -289,6 +352,34 @@ class Solver:
     def shell_fluxes(self, i): return cuharm_shell_fluxes(self.h, i)
     def stats(self): return cuharm_get_stats(self.h)
     def chain_stats(self): return cuharm_get_chain_stats(self.h)
+    # split step and face-speed maxima (slab decomposition, paper_2205_02484_b200/slab.py)
+    def set_dt(self, dt): cuharm_set_dt(self.h, dt)
+    def substep(self, which): cuharm_substep(self.h, which)
+    def substep_update(self, which): cuharm_substep_update(self.h, which)
+    def repair_pass(self, which, npass): return cuharm_repair_pass(self.h, which, npass)
+    def substep_finish(self, which): cuharm_substep_finish(self.h, which)
+    def work(self, which): return self.half if which == 0 else self.prim   # the array substep `which` produces
+    def end_step(self): pass
+
+    @property
+    def max_passes(self): return int(self.params["fixup_max_passes"])
+
+    @property
+    def flags(self):
+        """The fail flags of the last substep (a view of the workspace; int32 [n1g, n2g, n3g])."""
+        import torch
+        off, n = cuharm_flag_offset(self.h), self.shape[1] * self.shape[2] * self.shape[3] * 4
+        return self.workspace[off:off + n].view(torch.int32).view(self.shape[1:])
+    def last_cw(self): return cuharm_last_cw(self.h)
+    def cfl_cw(self): return cuharm_cfl_cw(self.h)
+    def dt_of_cw(self, xi, cw): return cuharm_dt_of_cw(self.h, xi, cw)
+
+    @property
+    def half(self):
+        """The half-step primitives (a view of the workspace; layout of `prim`)."""
+        import torch
+        off, n = cuharm_half_offset(self.h), 8 * self.shape[1] * self.shape[2] * self.shape[3] * 8
+        return self.workspace[off:off + n].view(torch.float64).view(self.shape)
     def repair(self, prim, flag): cuharm_repair(self.h, prim, flag)
     def use_graph(self, on=True): cuharm_use_graph(self.h, on)
     def launch_count(self): return cuharm_launch_count(self.h)

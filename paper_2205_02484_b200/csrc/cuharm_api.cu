@@ -60,6 +60,7 @@ struct cuharm_ctx {
   int *flag = nullptr, *list = nullptr;
   unsigned long long* cnt = nullptr;
   bool bound = false, have_geom = false, stepped = false;
+  bool dt_set = false, half_done = false;  // cuharm_set_dt / cuharm_substep sequencing
   int64_t launches = 0;
   // optional per-kernel-class timing with CUDA events on the library's stream (cuharm_set_timing)
   bool timing = false, capturing = false;
@@ -207,7 +208,9 @@ int launch_bc(cuharm_ctx* h, double* P, const unsigned long long* gate) {
   const int kchunks = (d.n3g + 127) / 128;
   const int per = 128 / (2 * d.ng);
   const long long nb = (long long)nrows_a * kchunks + ((long long)d.n1 * d.n2 + per - 1) / per;
-  BcAllArgs b{d, P, h->gC, h->p.bc_x1, h->p.bc_x2, h->p.bc_x3, h->p.coords, h->p.gamma_max, gate, nrows_a};
+  const bool slab = h->p.n1_global > 0;
+  BcAllArgs b{d, P, h->gC, h->p.bc_x1, h->p.bc_x2, h->p.bc_x3, h->p.coords, (slab && h->p.slab_lo) ? 3 : h->p.bc_x1,
+              (slab && h->p.slab_hi) ? 3 : h->p.bc_x1, h->p.gamma_max, gate, nrows_a};
   bc_all_kernel<<<(unsigned)nb, 128, 0, h->stream>>>(b);
   h->launches++;
   CK(cudaGetLastError());
@@ -301,7 +304,8 @@ int launch_flux(cuharm_ctx* h, const double* P, int dir, double* F, double* cw, 
 }
 
 // one RK2 substep (A34 order): fluxes -> EMFs -> update+inversion+floors -> ghost fill -> repair -> ghost fill
-int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pout, double dtfac, int which) {
+// `with_repair` = false: stop after the first ghost fill (the caller drives the repair pass by pass: cuharm_repair_pass)
+int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pout, double dtfac, int which, bool with_repair = true) {
   const Dims& d = h->d;
   unsigned long long* cwmax = h->cnt + (which == 0 ? CNT_CWPRED : CNT_CWSCR);
   // The three flux kernels are independent of one another.  While a graph is being recorded they go on three
@@ -433,7 +437,7 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
     CK(cudaGetLastError());
   }
   int rc = launch_bc(h, Pout, nullptr);
-  if (rc) return rc;
+  if (rc || !with_repair) return rc;
   {
     Timed t_(h, CUHARM_K_FIXUP);
     unsigned long long* fixw = h->cnt + CNT_FIX + which * CNT_FIXW;
@@ -507,6 +511,10 @@ int check_params(const cuharm_params* p) {
       if (!(p->xmax[c] > p->xmin[c])) return CUHARM_EINVAL;
   }
   if (p->polar_damp < 0 || p->polar_damp > 1 || p->reserved != 0) return CUHARM_EINVAL;
+  if (p->n1_global < 0 || (p->n1_global > 0 && (p->i_offset < 0 || p->i_offset + p->n1 > p->n1_global || p->slab_lo < 0 ||
+                                                p->slab_lo > 1 || p->slab_hi < 0 || p->slab_hi > 1)))
+    return CUHARM_EINVAL;
+  if (p->n1_global > 0 && (p->slab_lo || p->slab_hi) && p->n1 < p->ng) return CUHARM_EINVAL;  // a halo is ng interior planes
   if (p->polar_damp && (p->bc_x2 != 2 || p->n2 < 6)) return CUHARM_EINVAL;
   if (p->inv_chain < 0 || p->inv_chain > 1) return CUHARM_EINVAL;
   if (p->inv_chain && (p->brent_maxit < 1 || !(p->brent_tol >= 0.0) || !std::isfinite(p->beta_min))) return CUHARM_EINVAL;
@@ -562,11 +570,11 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
         x_out = x;
       }
     }
-    h->dx[0] = (x_out - h->x0[0]) / p->n1;
+    h->dx[0] = (x_out - h->x0[0]) / (p->n1_global > 0 ? p->n1_global : p->n1);
     h->x0[1] = -1.0; h->dx[1] = 2.0 / p->n2;
     h->x0[2] = 0.0;  h->dx[2] = 2.0 * PI / p->n3;
   } else {
-    const int n[3] = {p->n1, p->n2, p->n3};
+    const int n[3] = {p->n1_global > 0 ? p->n1_global : p->n1, p->n2, p->n3};
     for (int c = 0; c < 3; c++) { h->x0[c] = p->xmin[c]; h->dx[c] = (p->xmax[c] - p->xmin[c]) / n[c]; }
   }
   {  // opt in to the dynamic shared memory of the bulk-copy update kernel (67.5 KB per block)
@@ -631,6 +639,7 @@ int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_by
   h->maps_ok = h->upd_tmap && h->tmap_enable && encode_update_maps(h);
   h->bound = true;
   h->stepped = false;
+  h->dt_set = h->half_done = false;
   CK(cudaMemsetAsync(h->flag, 0, (size_t)h->d.nz * sizeof(int), h->stream));  // ghost zones always count as good
   CK(cudaMemsetAsync(h->cnt, 0, CNT_TOTAL * sizeof(unsigned long long), h->stream));
   if (h->have_geom) {
@@ -648,7 +657,7 @@ int cuharm_metric_precompute(cuharm_handle h) {
   DevGuard dg_(h);
   const cuharm_params& p = h->p;
   const Dims& d = h->d;
-  GeomArgs a{d.n1g, d.n2g, d.ng, d.n2, p.coords, (p.coords == 0 && p.bc_x2 == 2) ? 1 : 0, p.a, p.R0, p.hslope,
+  GeomArgs a{d.n1g, d.n2g, d.ng, d.n2, p.n1_global > 0 ? p.i_offset : 0, p.coords, (p.coords == 0 && p.bc_x2 == 2) ? 1 : 0, p.a, p.R0, p.hslope,
              h->xb, h->nx, h->x0[0], h->x0[1], h->dx[0], h->dx[1], p.rho_fl_coef, p.rho_fl_pow, p.rho_fl_abs, p.u_fl_coef,
              p.u_fl_pow, p.u_fl_abs, h->gC, h->gF1, h->gF2, h->conn, h->srcw, h->floors, h->rec};
   const int n = d.n1g * d.n2g;
@@ -672,6 +681,81 @@ int cuharm_step(cuharm_handle h, double dt) {
   CK(cudaGetLastError());
   return run_step(h);
 }
+
+int cuharm_set_dt(cuharm_handle h, double dt) {
+  if (!h) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  if (!(dt > 0.0) || !std::isfinite(dt)) return CUHARM_EINVAL;
+  DevGuard dg_(h);
+  set_dt_kernel<<<1, 1, 0, h->stream>>>(reinterpret_cast<double*>(h->cnt + CNT_CLOCK), dt);
+  h->launches++;
+  CK(cudaGetLastError());
+  h->dt_set = true;
+  return CUHARM_OK;
+}
+
+int cuharm_substep(cuharm_handle h, int32_t which) {
+  if (!h || which < 0 || which > 1) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom || !h->dt_set || (which == 1 && !h->half_done)) return CUHARM_ESTATE;
+  DevGuard dg_(h);
+  if (which == 0) {
+    CK(cudaMemsetAsync(h->cnt + CNT_NFAIL, 0, (CNT_STEP_END - CNT_NFAIL) * sizeof(unsigned long long), h->stream));
+    const int rc = substep(h, h->prim, h->prim, h->Phalf, 0.5, 0);
+    if (rc) return rc;
+    h->half_done = true;
+    h->stepped = true;
+    return CUHARM_OK;
+  }
+  h->half_done = false;
+  h->dt_set = false;
+  return substep(h, h->Phalf, h->prim, h->prim, 1.0, 1);
+}
+
+int cuharm_substep_update(cuharm_handle h, int32_t which) {
+  if (!h || which < 0 || which > 1) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom || !h->dt_set || (which == 1 && !h->half_done)) return CUHARM_ESTATE;
+  DevGuard dg_(h);
+  if (which == 0) {
+    CK(cudaMemsetAsync(h->cnt + CNT_NFAIL, 0, (CNT_STEP_END - CNT_NFAIL) * sizeof(unsigned long long), h->stream));
+    const int rc = substep(h, h->prim, h->prim, h->Phalf, 0.5, 0, false);
+    if (rc) return rc;
+    h->half_done = true;
+    h->stepped = true;
+    return CUHARM_OK;
+  }
+  h->half_done = false;
+  h->dt_set = false;
+  return substep(h, h->Phalf, h->prim, h->prim, 1.0, 1, false);
+}
+
+int cuharm_repair_pass(cuharm_handle h, int32_t which, int32_t pass, int64_t out[2]) {
+  if (!h || !out || which < 0 || which > 1 || pass < 0 || pass > h->p.fixup_max_passes) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom || !h->stepped) return CUHARM_ESTATE;
+  DevGuard dg_(h);
+  const Dims& d = h->d;
+  unsigned long long* fixw = h->cnt + CNT_FIX + which * CNT_FIXW;
+  unsigned long long* nfail = h->cnt + CNT_NFAIL + which;
+  CK(cudaMemsetAsync(fixw + 1, 0, 2 * sizeof(unsigned long long), h->stream));
+  FixArgs a{d, which == 0 ? h->Phalf : h->prim, h->flag, h->list, nfail, h->p.inv_chain ? fixw + CNT_FIXW - 1 : nullptr,
+            h->cnt + CNT_STATS, fixw, h->gC, h->floors, h->p.fixup_max_passes, h->p.gam, newton_cfg(h->p), floor_cfg(h->p)};
+  fixup_pass_kernel<<<2 * h->sms, 256, 0, h->stream>>>(a, pass, fixw + 1);
+  h->launches++;
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(out, fixw + 1, 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return CUHARM_OK;
+}
+
+int cuharm_substep_finish(cuharm_handle h, int32_t which) {
+  if (!h || which < 0 || which > 1) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom || !h->stepped) return CUHARM_ESTATE;
+  DevGuard dg_(h);
+  return launch_bc(h, which == 0 ? h->Phalf : h->prim, nullptr);
+}
+
+size_t cuharm_flag_offset(cuharm_handle h) { return h ? layout(h->d, h->p.inv_chain != 0).flag : 0; }
+
+size_t cuharm_half_offset(cuharm_handle h) { return h ? layout(h->d, h->p.inv_chain != 0).Phalf : 0; }
 
 int cuharm_step_cfl(cuharm_handle h, double xi, double dt_max) {
   if (!h || !(xi > 0.0) || !std::isfinite(xi) || dt_max != dt_max) return CUHARM_EINVAL;
@@ -775,20 +859,56 @@ int cuharm_prim_to_cons(cuharm_handle h, const double* d_prim, double* d_U) {
   return CUHARM_OK;
 }
 
-static int dt_from_cw(cuharm_handle h, const unsigned long long* d_cw, double xi, double* dt_out) {
+static int read_cw(cuharm_handle h, const unsigned long long* d_cw, double cw[3]) {
   unsigned long long m[3];
   CK(cudaMemcpyAsync(m, d_cw, sizeof(m), cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
+  for (int c = 0; c < 3; c++) std::memcpy(&cw[c], &m[c], sizeof(double));
+  return CUHARM_OK;
+}
+
+static double dt_of_cw(const cuharm_ctx* h, double xi, const double cw[3]) {
   double inv = 0.0;
   for (int c = 0; c < 3; c++) {
-    double cw;
-    std::memcpy(&cw, &m[c], sizeof(double));
-    const double dtl = xi * h->dx[c] / cw;  // dt^l = xi dx^l / max c_w
-    inv += 1.0 / dtl;                       // eq. 26
+    const double dtl = xi * h->dx[c] / cw[c];  // dt^l = xi dx^l / max c_w
+    inv += 1.0 / dtl;                          // eq. 26
   }
   const double dt = 1.0 / inv;
-  *dt_out = std::isfinite(dt) && dt > 0.0 ? dt : 0.0;  // a non-finite wave speed anywhere (a NaN enters as +inf): 0
+  return std::isfinite(dt) && dt > 0.0 ? dt : 0.0;  // a non-finite wave speed anywhere (a NaN enters as +inf): 0
+}
+
+static int dt_from_cw(cuharm_handle h, const unsigned long long* d_cw, double xi, double* dt_out) {
+  double cw[3];
+  const int rc = read_cw(h, d_cw, cw);
+  if (rc) return rc;
+  *dt_out = dt_of_cw(h, xi, cw);
   return CUHARM_OK;
+}
+
+int cuharm_dt_of_cw(cuharm_handle h, double xi, const double cw[3], double* dt_out) {
+  if (!h || !cw || !dt_out || !(xi > 0.0)) return CUHARM_EINVAL;
+  *dt_out = dt_of_cw(h, xi, cw);
+  return CUHARM_OK;
+}
+
+int cuharm_last_cw(cuharm_handle h, double cw[3]) {
+  if (!h || !cw) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom || !h->stepped) return CUHARM_ESTATE;
+  DevGuard dg_(h);
+  return read_cw(h, h->cnt + CNT_CWPRED, cw);
+}
+
+int cuharm_cfl_cw(cuharm_handle h, double cw[3]) {
+  if (!h || !cw) return CUHARM_EINVAL;
+  if (!h->bound || !h->have_geom) return CUHARM_ESTATE;
+  DevGuard dg_(h);
+  unsigned long long* d_cw = h->cnt + CNT_CWSCR;
+  CK(cudaMemsetAsync(d_cw, 0, 3 * sizeof(unsigned long long), h->stream));
+  for (int dir = 1; dir <= 3; dir++) {
+    int rc = launch_flux<false>(h, h->prim, dir, h->F[dir - 1], nullptr, d_cw + (dir - 1));
+    if (rc) return rc;
+  }
+  return read_cw(h, d_cw, cw);
 }
 
 int cuharm_cfl_dt(cuharm_handle h, double xi, double* dt_out) {

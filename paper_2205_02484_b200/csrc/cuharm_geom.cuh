@@ -9,6 +9,7 @@ namespace cuharm {
 
 struct GeomArgs {
   int n1g, n2g, ng, n2;
+  int i_off;       // global X1 index of this grid's first interior zone (slab decomposition; 0 for the whole grid)
   int coords, polar_bc;  // polar_bc: X2 boundary is the polar reflection -> the 2-faces J = 0, n2 lie on the axis (A32)
   double a, R0, hslope;
   double xb;       // X1 of the exponential -> hyper-exponential transition (eq. 39); used when nx >= 2
@@ -166,7 +167,7 @@ __global__ void geom_kernel(GeomArgs A) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= A.n1g * A.n2g) return;
   const int i = t / A.n2g, j = t % A.n2g;
-  const int I = i - A.ng, Jz = j - A.ng;
+  const int I = i - A.ng + A.i_off, Jz = j - A.ng;
   Geom C, F1, F2;
   double cn[40], sw[14];
   double rc = 1.0;

@@ -45,6 +45,7 @@ struct BcAllArgs {
   double* P;
   const Geom* C;
   int kind1, kind2, kind3, coords;
+  int kind1_lo, kind1_hi;  // the X1 rule per side: kind1, or 3 (never written) on an internal slab boundary
   double gamma_max;
   const unsigned long long* gate;
   int nrows_a;  // (i, j) rows with a ghost index in X1 or X2
@@ -63,7 +64,7 @@ __device__ __forceinline__ int bc_source(int x, int n, int ng, int kind, bool re
 
 __device__ __forceinline__ void bc_zone(const BcAllArgs& a, int i, int j, int k) {
   const Dims& d = a.d;
-  const bool gi = (i < d.ng || i >= d.ng + d.n1) && a.kind1 != 3;
+  const bool gi = (i < d.ng && a.kind1_lo != 3) || (i >= d.ng + d.n1 && a.kind1_hi != 3);
   const bool gj = (j < d.ng || j >= d.ng + d.n2) && a.kind2 != 3;
   const bool gk = (k < d.ng || k >= d.ng + d.n3) && a.kind3 != 3;
   if (!(gi || gj || gk)) return;
@@ -583,68 +584,76 @@ __device__ __forceinline__ void fix_grid_barrier(unsigned long long* bar, unsign
   __syncthreads();
 }
 
-__global__ void __launch_bounds__(FIX_THREADS) fixup_kernel(FixArgs a) {
+// One zone of the list in one pass: 0 nothing to do (already repaired), 1 repaired, 2 repaired by the last-resort rule,
+// 3 left waiting.
+__device__ __forceinline__ int fix_one(const FixArgs& a, long long idx, int pass, bool last) {
   const Dims& d = a.d;
+  if (__ldcg(a.flag + idx) <= 0) return 0;
+  const long long fo[4] = {d.s1, -d.s1, d.s2, -d.s2};
+  const long long dg[4] = {d.s1 + d.s2, d.s1 - d.s2, -d.s1 + d.s2, -d.s1 - d.s2};
+  bool fg = true, dgood = true;
+#pragma unroll
+  for (int m = 0; m < 4; m++) {
+    fg = fg && zone_good(__ldcg(a.flag + idx + fo[m]), pass);
+    dgood = dgood && zone_good(__ldcg(a.flag + idx + dg[m]), pass);
+  }
+  double q[8];
+  int what = 1;
+  if (fg || dgood) {
+    const long long* st = fg ? fo : dg;
+#pragma unroll
+    for (int v = 0; v < 5; v++) {
+      double s = 0.0;
+#pragma unroll
+      for (int m = 0; m < 4; m++) s += __ldcg(a.P + v * d.nz + idx + st[m]);
+      q[v] = 0.25 * s;
+    }
+  } else if (last) {
+    int cnt = 0;
+    double s[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    for (int di = -1; di <= 1; di++)
+      for (int dj = -1; dj <= 1; dj++) {
+        if (!di && !dj) continue;
+        const long long n = idx + di * d.s1 + dj * d.s2;
+        if (!zone_good(__ldcg(a.flag + n), pass)) continue;
+        cnt++;
+#pragma unroll
+        for (int v = 0; v < 5; v++) s[v] += __ldcg(a.P + v * d.nz + n);
+      }
+#pragma unroll
+    for (int v = 0; v < 5; v++) q[v] = cnt > 0 ? s[v] / cnt : __ldcg(a.P + v * d.nz + idx);
+    what = 2;
+  } else {
+    return 3;
+  }
+#pragma unroll
+  for (int v = 5; v < 8; v++) q[v] = __ldcg(a.P + v * d.nz + idx);
+  const int q2 = (int)(idx / d.s2);  // = i * n2g + j
+  const Geom G = load_geom(a.C, q2);
+  apply_floors(q, G, a.C + q2, a.floors[2 * q2], a.floors[2 * q2 + 1], a.fc, a.gam, a.nc);
+#pragma unroll
+  for (int v = 0; v < 5; v++) a.P[v * d.nz + idx] = q[v];
+  a.flag[idx] = -(pass + 1);
+  return what;
+}
+
+__global__ void __launch_bounds__(FIX_THREADS) fixup_kernel(FixArgs a) {
   const unsigned long long nf = *a.nfail;
   if (nf == 0ull) return;
   const unsigned long long want = (nf + FIX_THREADS - 1) / FIX_THREADS;
   const unsigned nb = (unsigned)(want < gridDim.x ? want : gridDim.x);  // participating blocks
   if (blockIdx.x >= nb) return;
   if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(a.stats + 0, a.nbad ? *a.nbad : nf);
-  const long long fo[4] = {d.s1, -d.s1, d.s2, -d.s2};
-  const long long dg[4] = {d.s1 + d.s2, d.s1 - d.s2, -d.s1 + d.s2, -d.s1 - d.s2};
   unsigned long long repaired = 0ull, lastres = 0ull;
   const unsigned long long stride = (unsigned long long)nb * FIX_THREADS;
   for (int pass = 0; pass <= a.max_passes; pass++) {
     const bool last = pass == a.max_passes;
     int left = 0;
     for (unsigned long long e = (unsigned long long)blockIdx.x * FIX_THREADS + threadIdx.x; e < nf; e += stride) {
-      const long long idx = a.list[e];
-      if (__ldcg(a.flag + idx) <= 0) continue;
-      bool fg = true, dgood = true;
-#pragma unroll
-      for (int m = 0; m < 4; m++) {
-        fg = fg && zone_good(__ldcg(a.flag + idx + fo[m]), pass);
-        dgood = dgood && zone_good(__ldcg(a.flag + idx + dg[m]), pass);
-      }
-      double q[8];
-      if (fg || dgood) {
-        const long long* st = fg ? fo : dg;
-#pragma unroll
-        for (int v = 0; v < 5; v++) {
-          double s = 0.0;
-#pragma unroll
-          for (int m = 0; m < 4; m++) s += __ldcg(a.P + v * d.nz + idx + st[m]);
-          q[v] = 0.25 * s;
-        }
-      } else if (last) {
-        int cnt = 0;
-        double s[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-        for (int di = -1; di <= 1; di++)
-          for (int dj = -1; dj <= 1; dj++) {
-            if (!di && !dj) continue;
-            const long long n = idx + di * d.s1 + dj * d.s2;
-            if (!zone_good(__ldcg(a.flag + n), pass)) continue;
-            cnt++;
-#pragma unroll
-            for (int v = 0; v < 5; v++) s[v] += __ldcg(a.P + v * d.nz + n);
-          }
-#pragma unroll
-        for (int v = 0; v < 5; v++) q[v] = cnt > 0 ? s[v] / cnt : __ldcg(a.P + v * d.nz + idx);
-        lastres++;
-      } else {
-        left = 1;
-        continue;
-      }
-#pragma unroll
-      for (int v = 5; v < 8; v++) q[v] = __ldcg(a.P + v * d.nz + idx);
-      const int q2 = (int)(idx / d.s2);  // = i * n2g + j
-      const Geom G = load_geom(a.C, q2);
-      apply_floors(q, G, a.C + q2, a.floors[2 * q2], a.floors[2 * q2 + 1], a.fc, a.gam, a.nc);
-#pragma unroll
-      for (int v = 0; v < 5; v++) a.P[v * d.nz + idx] = q[v];
-      a.flag[idx] = -(pass + 1);
-      repaired++;
+      const int w = fix_one(a, a.list[e], pass, last);
+      repaired += w == 1 || w == 2;
+      lastres += w == 2;
+      left |= w == 3;
     }
     if (last) break;
     // anything left waiting anywhere?  (one atomic per block that has some; read after the barrier)
@@ -660,6 +669,28 @@ __global__ void __launch_bounds__(FIX_THREADS) fixup_kernel(FixArgs a) {
   }
   if (repaired) atomicAdd(a.stats + 1, repaired);
   if (lastres) atomicAdd(a.stats + 7, lastres);
+}
+
+// One Jacobi pass as a launch of its own (cuharm_repair_pass): for a caller that refreshes the halo planes of the
+// primitives and of the flags between the passes (slab decomposition), so that a repair next to an internal boundary sees
+// its neighbours exactly as the single-domain repair does.  out[0] = entries of the list, out[1] = zones left waiting.
+__global__ void __launch_bounds__(256) fixup_pass_kernel(FixArgs a, int pass, unsigned long long* out) {
+  const unsigned long long nf = *a.nfail;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    out[0] = nf;
+    if (pass == 0 && nf) atomicAdd(a.stats + 0, a.nbad ? *a.nbad : nf);
+  }
+  unsigned long long repaired = 0ull, lastres = 0ull, left = 0ull;
+  for (unsigned long long e = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; e < nf;
+       e += (unsigned long long)gridDim.x * blockDim.x) {
+    const int w = fix_one(a, a.list[e], pass, pass == a.max_passes);
+    repaired += w == 1 || w == 2;
+    lastres += w == 2;
+    left += w == 3;
+  }
+  if (repaired) atomicAdd(a.stats + 1, repaired);
+  if (lastres) atomicAdd(a.stats + 7, lastres);
+  if (left) atomicAdd(out + 1, left);
 }
 
 // P:L311 (A16): utilde^2 of the two zones nearest each pole <- the straight line in X^2 through zero at the pole and

@@ -1,0 +1,228 @@
+"""Slab decomposition of the grid along X1 over several GPUs (paper: P:L271-273, one slab per GPU with neighbour
+copies over NVLink): host-side sequencing only.  Every step of the update still runs in the
+library's kernels on each rank's own slab; this module cuts the grid, moves the halo planes between neighbours after
+each substep and takes the maximum of the face speeds over the slabs for eq. 26.
+
+    per substep (predictor into the half-step array, corrector into the primitives):
+        substep_update (fluxes, update, inversion, floors, ghost fill)  ->  halo exchange of the array and of the fail flags
+        -> repair pass 0 on every slab; sum over the slabs of (failed zones, zones left waiting)
+        -> only if any zone failed anywhere: [halo exchange of array + flags; next pass while zones are waiting] ...,
+           second ghost fill, halo exchange of the array
+    halo = the outermost ng interior (i) planes of a slab, whole (j, k) extent incl. ghosts  ->  the neighbour's ng
+           ghost planes on that side (C4, ng = 3: 3 x 262 x 262 x 8 doubles = 13 MB per side and substep; flags 0.8 MB)
+    With these exchanges every Jacobi pass of the eq. 34 repair sees across an internal boundary exactly what the
+    single-domain repair sees: the decomposition does not change the answer even when zones fail next to a cut.
+
+The objects below work on any `engine` with the split-step interface of `binding.Solver` (set_dt, substep_update, repair_pass,
+substep_finish, work, flags, end_step, max_passes, cfl_cw, last_cw, dt_of_cw): the library on GPUs, or a CPU stand-in in the host-logic tests.
+
+* `slab_params(p, nslabs, r)`      parameter block of slab r of nslabs
+* `slab_slice(p, nslabs, r)`       the i-range of the full (ghost-padded) array that slab r starts from
+* `SlabRank(engine, ...)`          one rank of a torch.distributed job (NCCL on GPUs, gloo on CPUs): isend / irecv with
+                                   rank - 1 and rank + 1, all_reduce(MAX) of three doubles
+* `SlabGroup(engines, p)`          all slabs in one process (one device), halos moved by plain copies: the reference for
+                                   the sequencing, and what the single-GPU parity test runs
+
+Not measured on more than one GPU in this build (the run's boxes have one); `bench.py --gpus N` keeps running N
+replicas.
+"""
+from typing import List, Sequence, Tuple
+
+
+def slab_ranges(n1: int, nslabs: int) -> List[Tuple[int, int]]:
+    """(first zone, zone count) of every slab: as equal as possible, the first n1 % nslabs slabs one zone longer."""
+    if nslabs < 1 or nslabs > n1:
+        raise ValueError("need 1 <= nslabs <= n1")
+    base, extra = divmod(n1, nslabs)
+    out, i0 = [], 0
+    for r in range(nslabs):
+        n = base + (1 if r < extra else 0)
+        out.append((i0, n))
+        i0 += n
+    return out
+
+
+def slab_params(p: dict, nslabs: int, r: int) -> dict:
+    """Parameter block of slab r: n1 local, coordinates of the full grid, internal sides marked."""
+    if nslabs == 1:
+        return dict(p)
+    i0, n = slab_ranges(p["n1"], nslabs)[r]
+    if n < p["ng"]:
+        raise ValueError("a slab needs at least ng zones along X1")
+    periodic = p["bc_x1"] == 1
+    return dict(p, n1=n, n1_global=p["n1"], i_offset=i0, slab_lo=1 if (r > 0 or periodic) else 0,
+                slab_hi=1 if (r < nslabs - 1 or periodic) else 0)
+
+
+def slab_slice(p: dict, nslabs: int, r: int) -> slice:
+    """i-range of the full array [8, n1 + 2 ng, ...] that holds slab r with its ghost / halo planes."""
+    i0, n = slab_ranges(p["n1"], nslabs)[r]
+    return slice(i0, i0 + n + 2 * p["ng"])
+
+
+def neighbours(p: dict, nslabs: int, r: int) -> Tuple[int, int]:
+    """Ranks of the lower and upper X1 neighbour (-1: a physical boundary)."""
+    if nslabs == 1:
+        return -1, -1
+    if p["bc_x1"] == 1:
+        return (r - 1) % nslabs, (r + 1) % nslabs
+    return (r - 1 if r > 0 else -1), (r + 1 if r < nslabs - 1 else -1)
+
+
+def _planes(arr, ng: int, n1: int):
+    """(lowest ng interior planes, highest ng interior planes, lower ghost planes, upper ghost planes) as views."""
+    return arr[:, ng:2 * ng], arr[:, n1:n1 + ng], arr[:, 0:ng], arr[:, n1 + ng:n1 + 2 * ng]
+
+
+class SlabGroup:
+    """All slabs of a grid in one process; halos move by copies between the engines' arrays."""
+
+    def __init__(self, engines: Sequence, p: dict):
+        self.engines, self.p, self.n = list(engines), p, len(engines)
+        self.ranges = slab_ranges(p["n1"], self.n)
+
+    def _exchange_arrays(self, arrs):
+        ng = self.p["ng"]
+        # snapshot of what every slab sends before anything is written: the copies must not depend on their order
+        sends = []
+        for r, a in enumerate(arrs):
+            lo, hi, _, _ = _planes(a, ng, self.ranges[r][1])
+            sends.append((lo.clone() if hasattr(lo, "clone") else lo.copy(), hi.clone() if hasattr(hi, "clone") else hi.copy()))
+        for r, a in enumerate(arrs):
+            rl, rh = neighbours(self.p, self.n, r)
+            _, _, glo, ghi = _planes(a, ng, self.ranges[r][1])
+            if rl >= 0:
+                glo[...] = sends[rl][1]   # the lower neighbour's highest interior planes
+            if rh >= 0:
+                ghi[...] = sends[rh][0]   # the upper neighbour's lowest interior planes
+
+    def _exchange(self, which: int, flags: bool):
+        self._exchange_arrays([e.work(which) for e in self.engines])
+        if flags:
+            # the flag array has no leading component axis: give it one so that the same plane arithmetic applies
+            self._exchange_arrays([e.flags[None] for e in self.engines])
+
+    def _substep(self, which: int):
+        for e in self.engines:
+            e.substep_update(which)
+        self._exchange(which, flags=True)
+        res = [e.repair_pass(which, 0) for e in self.engines]
+        if sum(r[0] for r in res) == 0:
+            return
+        npass, left = 0, sum(r[1] for r in res)
+        self._exchange(which, flags=True)
+        while left > 0 and npass < self.engines[0].max_passes:
+            npass += 1
+            left = sum(e.repair_pass(which, npass)[1] for e in self.engines)
+            self._exchange(which, flags=True)
+        for e in self.engines:
+            e.substep_finish(which)
+        self._exchange(which, flags=False)
+
+    def step(self, dt: float):
+        for e in self.engines:
+            e.set_dt(dt)
+        self._substep(0)
+        self._substep(1)
+        for e in self.engines:
+            e.end_step()
+
+    def _max_cw(self, cws):
+        return [max(c[d] for c in cws) for d in range(3)]
+
+    def cfl_dt(self, xi: float) -> float:
+        return self.engines[0].dt_of_cw(xi, self._max_cw([e.cfl_cw() for e in self.engines]))
+
+    def last_cfl_dt(self, xi: float) -> float:
+        return self.engines[0].dt_of_cw(xi, self._max_cw([e.last_cw() for e in self.engines]))
+
+    def gather(self, which: str = "prim"):
+        """The full array (ghosts of the physical sides included) assembled from the slabs; numpy."""
+        import numpy as np
+        ng = self.p["ng"]
+        parts = []
+        for r, e in enumerate(self.engines):
+            a = getattr(e, which)
+            a = a.detach().cpu().numpy() if hasattr(a, "detach") else np.asarray(a)
+            n = self.ranges[r][1]
+            lo = 0 if r == 0 else ng
+            hi = n + 2 * ng if r == self.n - 1 else n + ng
+            parts.append(a[:, lo:hi])
+        return np.concatenate(parts, axis=1)
+
+
+class SlabRank:
+    """One rank of a torch.distributed job: the same sequence with isend / irecv to the neighbouring ranks.
+
+    `engine.prim` / `engine.half` must be torch tensors (CUDA with the NCCL backend, CPU with gloo)."""
+
+    def __init__(self, engine, p: dict, rank: int, world: int, group=None):
+        import torch.distributed as dist
+        self.dist, self.group = dist, group
+        self.engine, self.p, self.rank, self.world = engine, p, rank, world
+        self.n1 = slab_ranges(p["n1"], world)[rank][1]
+        self.lo, self.hi = neighbours(p, world, rank)
+
+    def _exchange(self, arr):
+        import torch
+        ng = self.p["ng"]
+        lo, hi, glo, ghi = _planes(arr, ng, self.n1)
+        ops, recv = [], []
+        if self.lo >= 0:
+            s, r = lo.contiguous(), torch.empty_like(glo.contiguous())
+            ops += [self.dist.P2POp(self.dist.isend, s, self.lo, self.group), self.dist.P2POp(self.dist.irecv, r, self.lo, self.group)]
+            recv.append((glo, r))
+        if self.hi >= 0:
+            s, r = hi.contiguous(), torch.empty_like(ghi.contiguous())
+            ops += [self.dist.P2POp(self.dist.isend, s, self.hi, self.group), self.dist.P2POp(self.dist.irecv, r, self.hi, self.group)]
+            recv.append((ghi, r))
+        if ops:
+            for w in self.dist.batch_isend_irecv(ops):
+                w.wait()
+        for dst, buf in recv:
+            dst.copy_(buf)
+
+    def _allsum(self, a, b):
+        import torch
+        t = torch.tensor([a, b], dtype=torch.int64, device=self.engine.prim.device)
+        if self.world > 1:
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM, group=self.group)
+        return int(t[0]), int(t[1])
+
+    def _substep(self, which: int):
+        e = self.engine
+        e.substep_update(which)
+        self._exchange(e.work(which))
+        self._exchange(e.flags[None])
+        nf, left = self._allsum(*e.repair_pass(which, 0))
+        if nf == 0:
+            return
+        npass = 0
+        self._exchange(e.work(which))
+        self._exchange(e.flags[None])
+        while left > 0 and npass < e.max_passes:
+            npass += 1
+            _, left = self._allsum(*e.repair_pass(which, npass))
+            self._exchange(e.work(which))
+            self._exchange(e.flags[None])
+        e.substep_finish(which)
+        self._exchange(e.work(which))
+
+    def step(self, dt: float):
+        self.engine.set_dt(dt)
+        self._substep(0)
+        self._substep(1)
+        self.engine.end_step()
+
+    def _allmax(self, cw):
+        import torch
+        t = torch.tensor(list(cw), dtype=torch.float64, device=self.engine.prim.device)
+        if self.world > 1:
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX, group=self.group)
+        return [float(x) for x in t.cpu()]
+
+    def cfl_dt(self, xi: float) -> float:
+        return self.engine.dt_of_cw(xi, self._allmax(self.engine.cfl_cw()))
+
+    def last_cfl_dt(self, xi: float) -> float:
+        return self.engine.dt_of_cw(xi, self._allmax(self.engine.last_cw()))

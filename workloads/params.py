@@ -30,6 +30,7 @@ def default_params(**kw) -> dict:
         n_x=0, r_break=0.0,            # hyper-exponential radial branch of eq. 39: off; the paper: 4, 400
         inv_chain=0, brent_maxit=200,  # inversion fallback chain: off on the hot path (A33)
         beta_min=1e-2, brent_tol=1e-14,   # eq. 33; Brent's relative tolerance (A40)
+        n1_global=0, i_offset=0, slab_lo=0, slab_hi=0,   # slab of a larger grid; 0: the whole grid
         polar_damp=0,                  # P:L311 (A16): polar velocity of the two zones nearest each pole -> 0 at the pole; off
     )
     d.update(kw)
