@@ -396,5 +396,20 @@ def test_error_codes():
     assert L.cuharm_metric_precompute(h) == 0
     assert L.cuharm_step(h, -1.0) == -1
     assert L.cuharm_step(h, float("nan")) == -1
+    # split step: order is enforced; options are validated
+    assert L.cuharm_substep(h, 0) == -2                     # no cuharm_set_dt yet
+    assert L.cuharm_set_dt(h, 0.0) == -1
+    assert L.cuharm_set_dt(h, 1e-3) == 0
+    assert L.cuharm_substep(h, 1) == -2                     # corrector before predictor
+    assert L.cuharm_substep(h, 2) == -1
+    assert L.cuharm_substep(h, 0) == 0 and L.cuharm_substep(h, 1) == 0
+    out2 = (C.c_int64 * 2)()
+    assert L.cuharm_repair_pass(h, 0, 99, out2) == -1       # pass beyond fixup_max_passes
+    assert L.cuharm_invert_fallback(h, 3, C.c_void_p(prim.data_ptr()), None, C.c_void_p(prim.data_ptr()), None) == -1
+    assert L.cuharm_shell_fluxes(h, 99, (C.c_double * 4)()) == -1
     torch.cuda.synchronize()
     L.cuharm_destroy(h)
+    for kw in (dict(polar_damp=1, bc_x2=1), dict(n1_global=8, i_offset=4, n1=8), dict(inv_chain=1, brent_maxit=0),
+               dict(fixup_max_passes=99), dict(reserved=1)):
+        bad = cu.make_params(default_params(**kw))
+        assert L.cuharm_grid_init(C.byref(h), C.byref(bad), None) == -1, kw
