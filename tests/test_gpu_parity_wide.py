@@ -263,3 +263,31 @@ def test_tensor_map_update_kernel_is_bitwise_the_row_copy_kernel(monkeypatch):
             s.close()
         monkeypatch.delenv("CUHARM_NO_TMAP", raising=False)
         assert np.array_equal(res[0][0], res[1][0]) and res[0][1] == res[1][1] and res[0][2] == res[1][2]
+
+
+# ------------------------------------------------------------------ the headline workload itself, every zone
+def test_full_size_c4_workload_two_steps_every_zone_against_the_oracle():
+    """BASELINE.json's headline config as bench.py runs it -- C4, 256 x 256 x 256, the seeded 3D-perturbed magnetised
+    torus, PPM + LLF, graph replay, tensor-map update kernel with two 128-zone tiles per row -- against the oracle on ALL
+    16.8 million zones (the oracle needs ~6 s per full step on 16 cores): <= 1e-11 per primitive after one RK2 step,
+    <= 1e-10 after two, div B at round-off, counters equal."""
+    p = config("C4")
+    assert (p["n1"], p["n2"], p["n3"]) == (256, 256, 256)
+    prim0, _ = fm_torus(p)
+    ref = prim0.copy()
+    g = oracle.Grid(p)
+    g.bind(ref)
+    dt = g.cfl_dt(0.45)
+    s = cu.Solver(p, torch.from_numpy(prim0))
+    assert abs(s.cfl_dt(0.45) / dt - 1.0) < 1e-13
+    s.use_graph(True)
+    for n, tol in ((1, 1e-11), (2, 1e-10)):
+        g.step(dt)
+        s.step(dt)
+        got = s.prim.cpu().numpy()
+        err = prim_errors(p, got, ref, whole=True, tol=tol)
+        assert (err < tol).all(), (n, err)
+        assert list(s.stats()) == [int(x) for x in g.get_stats()]
+    assert s.divb()[1] < 1e-12 and g.divb()[1] < 1e-12
+    assert abs(s.last_cfl_dt(0.45) / g.last_cfl_dt(0.45) - 1.0) < 1e-13
+    s.close()
