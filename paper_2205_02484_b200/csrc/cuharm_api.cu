@@ -78,6 +78,7 @@ struct cuharm_ctx {
   UpdMaps maps;
   int upd_blocks = 0, upd_blocks64 = 0;  // its persistent grid sizes (128- and 64-zone tiles)
   int sms = 148;         // multiprocessors of the device
+  bool coop = false;     // cooperative launches available (device attribute; decided at grid_init)
   double xb = 0.0;       // eq. 39: X1 of the exponential -> hyper-exponential transition
   int nx = 0;            // its exponent (0: plain exponential)
   bool fluxk_row = true; // prefer the whole-row pipeline (flux_k_row_kernel)
@@ -198,6 +199,34 @@ struct Timed {
     h->ev_used += 2;
   }
 };
+
+// The repair kernel separates its Jacobi passes by a grid barrier, so its participating blocks must be resident together.
+// A COOPERATIVE launch makes the driver guarantee that (and keeps two such kernels from different streams from holding
+// multiprocessors against each other); it is also what a recorded graph stores.  Devices / drivers without cooperative
+// launch get a plain launch of at most one block per multiprocessor.
+int launch_fixup(cuharm_ctx* h, const FixArgs& a) {
+  if (h->coop) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)h->sms);
+    cfg.blockDim = dim3(FIX_THREADS);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, fixup_kernel, a);
+    if (e == cudaSuccess) { h->launches++; return CUHARM_OK; }
+    if (h->capturing) return cuda_fail(e, "cudaLaunchKernelEx(fixup_kernel, cooperative)");
+    (void)cudaGetLastError();
+    h->coop = false;  // not supported here after all: plain launches from now on
+  }
+  fixup_kernel<<<h->sms, FIX_THREADS, 0, h->stream>>>(a);
+  h->launches++;
+  CK(cudaGetLastError());
+  return CUHARM_OK;
+}
 
 int launch_bc(cuharm_ctx* h, double* P, const unsigned long long* gate) {
   Timed t_(h, CUHARM_K_BC);
@@ -443,8 +472,8 @@ int substep(cuharm_ctx* h, const double* Pflux, const double* Pbase, double* Pou
     unsigned long long* fixw = h->cnt + CNT_FIX + which * CNT_FIXW;
     FixArgs a{d, Pout, h->flag, h->list, nfail, h->p.inv_chain ? fixw + CNT_FIXW - 1 : nullptr, h->cnt + CNT_STATS, fixw, h->gC,
               h->floors, h->p.fixup_max_passes, h->p.gam, newton_cfg(h->p), floor_cfg(h->p)};
-    fixup_kernel<<<h->sms, FIX_THREADS, 0, h->stream>>>(a);  // at most one block per multiprocessor (grid barrier)
-    h->launches++;
+    const int rf = launch_fixup(h, a);
+    if (rf) return rf;
   }
   CK(cudaGetLastError());
   return launch_bc(h, Pout, nfail);
@@ -608,6 +637,10 @@ int cuharm_grid_init(cuharm_handle* out, const cuharm_params* p, void* cuda_stre
       cudaGetDevice(&dev);
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
       if (sms > 0) h->sms = sms;
+      int coop = 0, per = 0;
+      if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop &&
+          cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, fixup_kernel, FIX_THREADS, 0) == cudaSuccess && per >= 1)
+        h->coop = true;
     }
   }
   *out = h;
@@ -1015,9 +1048,10 @@ int cuharm_repair(cuharm_handle h, double* d_prim, const int32_t* d_flag) {
   repair_list_kernel<<<dim3((d.n3g + 127) / 128, d.n2g, d.n1g), 128, 0, h->stream>>>(d, d_flag, h->flag, h->list, nfail);
   FixArgs a{d, d_prim, h->flag, h->list, nfail, nullptr, h->cnt + CNT_STATS, fixw, h->gC, h->floors, h->p.fixup_max_passes,
             h->p.gam, newton_cfg(h->p), floor_cfg(h->p)};
-  fixup_kernel<<<h->sms, FIX_THREADS, 0, h->stream>>>(a);
-  h->launches += 2;
+  h->launches++;
   CK(cudaGetLastError());
+  const int rf = launch_fixup(h, a);
+  if (rf) return rf;
   // the library's flag array goes back to "all good" (its state between steps)
   CK(cudaMemsetAsync(h->flag, 0, (size_t)d.nz * sizeof(int), h->stream));
   return CUHARM_OK;

@@ -545,9 +545,10 @@ __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kern
 // zones that are not written in the current pass.
 //
 // Grid-wide: the list is dealt to min(gridDim.x, ceil(nf / 512)) blocks (the others leave at once), and the passes
-// are separated by a grid barrier on a device counter (monotonic, zeroed with the per-step counters).  The grid has
-// at most one block per multiprocessor, so every participating block is resident as soon as whatever else shares
-// the device drains: the barrier cannot deadlock.  With nothing failed (every step of the torus workloads' first
+// are separated by a grid barrier on a device counter (monotonic, zeroed with the per-step counters).  The kernel is
+// launched COOPERATIVELY (cuharm_api.cu: launch_fixup), with at most one block per multiprocessor, so the driver
+// guarantees that the participating blocks are resident together -- also when several contexts repair on several
+// streams at once.  With nothing failed (every step of the torus workloads' first
 // 1000) the kernel is one read and an exit; with a handful of failures one block does the work without touching the
 // barrier; a step with 1e6 failures is spread over the whole device.  Reads of flags and donors bypass L1 (other
 // blocks write them between passes).
