@@ -283,35 +283,40 @@ def run_ours(args):
                      "divb_norm": s.divb()[1], "failed_inversions": int(s.stats()[0])}
 
     # ---- e2e: the same step through the public API with HOST buffers: H2D of the primitives from pinned memory,
-    # one step, D2H of the result into pinned memory, every step inside the timed region.  Two solver objects on two
-    # streams take alternate steps (each step is an independent problem: fresh input, own output), so the H2D copy of
+    # one step, D2H of the result into pinned memory, every step inside the timed region.  Three solver objects on three
+    # streams take the steps in turn (each step is an independent problem: fresh input, own output), so the H2D copy of
     # one step overlaps the D2H copy and the kernels of the other (PCIe is full duplex; 1.15 GB each way per step).
     e2e_steps = max(2, min(args.e2e_steps, args.steps))
-    side = torch.cuda.Stream(device=local)
-    with torch.cuda.stream(side):
-        s2 = cu.Solver(p, prim_pinned, device=f"cuda:{local}", stream=side)
-        if args.graph:
-            s2.use_graph(True)
-        s2.step(dt)                      # records its graph outside the timed region
-    side.synchronize()
-    lanes = [(s, torch.cuda.current_stream(), torch.empty_like(prim_pinned).pin_memory()),
-             (s2, side, torch.empty_like(prim_pinned).pin_memory())]
-    e_side = torch.cuda.Event()
+    NLANE = 3                            # H2D 22 ms + kernels 6 ms + D2H 22 ms per step: three steps in flight keep both copy
+    lanes = [(s, torch.cuda.current_stream(), torch.empty_like(prim_pinned).pin_memory())]   # engines busy (PCIe is full duplex)
+    for _ in range(NLANE - 1):
+        side = torch.cuda.Stream(device=local)
+        with torch.cuda.stream(side):
+            sx = cu.Solver(p, prim_pinned, device=f"cuda:{local}", stream=side)
+            if args.graph:
+                sx.use_graph(True)
+            sx.step(dt)                  # records its graph outside the timed region
+        side.synchronize()
+        lanes.append((sx, side, torch.empty_like(prim_pinned).pin_memory()))
     barrier()
     e0.record()
-    side.wait_event(e0)
+    for _, st, _ in lanes[1:]:
+        st.wait_event(e0)
     for n in range(e2e_steps):
-        sol, st, out_pinned = lanes[n & 1]
+        sol, st, out_pinned = lanes[n % NLANE]
         with torch.cuda.stream(st):
             sol.load(prim_pinned)          # H2D + ghost fill
             sol.step(dt)
             out_pinned.copy_(sol.prim, non_blocking=True)
-    e_side.record(side)
-    torch.cuda.current_stream().wait_event(e_side)
+    for _, st, _ in lanes[1:]:
+        ev = torch.cuda.Event()
+        ev.record(st)
+        torch.cuda.current_stream().wait_event(ev)
     e1.record()
     barrier()
     ms_e2e = e0.elapsed_time(e1)
-    s2.close()
+    for sx, _, _ in lanes[1:]:
+        sx.close()
     ms_e2e, e2e_val = aggregate(ms_e2e, zones, e2e_steps, world, dist, "cuda")
     nbytes = prim_pinned.numel() * 8
     if rank == 0:
@@ -374,7 +379,7 @@ def run_ours(args):
                           "dt": dt},
                "clocks": clocks, "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": nbytes,
                                          "d2h_bytes_per_step": nbytes, "steps": e2e_steps,
-                                         "pipeline": "2 solver objects on 2 streams, alternate steps"},
+                                         "pipeline": "3 solver objects on 3 streams, steps dealt round-robin"},
                "gpu_launches": int(launches), "roofline": roof, "roofline_alu": roof_alu, "sustained": sustained,
                "cpu_baseline": cpu,
                "checks": {"divb_norm": divb, "stats": stats}}
@@ -501,7 +506,7 @@ def main():
     ap.add_argument("--config", default="C4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--graph", type=int, default=1)
-    ap.add_argument("--e2e-steps", type=int, default=6)
+    ap.add_argument("--e2e-steps", type=int, default=18)
     ap.add_argument("--cpu-steps", type=int, default=2, help="cpu_baseline: RK2 steps of the oracle on all host cores")
     ap.add_argument("--cpu-n3", type=int, default=0, help="cpu_baseline: phi zones of the sample (0 = the full grid)")
     ap.add_argument("--ref-n3", type=int, default=32, help="--impl reference: phi zones of the per-step sample")
