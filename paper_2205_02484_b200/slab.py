@@ -167,15 +167,22 @@ class SlabRank:
         import torch
         ng = self.p["ng"]
         lo, hi, glo, ghi = _planes(arr, ng, self.n1)
+        # Order of the operations: [send lowest planes down, receive upper ghosts from above, send highest planes up,
+        # receive lower ghosts from below].  NCCL pairs point-to-point operations between two ranks by ORDER, and with two
+        # ranks and a periodic direction the lower and the upper neighbour are the same rank: in this order its first send
+        # (its lowest planes) meets my first receive (my upper ghosts), as it must.
         ops, recv = [], []
         if self.lo >= 0:
-            s, r = lo.contiguous(), torch.empty_like(glo.contiguous())
-            ops += [self.dist.P2POp(self.dist.isend, s, self.lo, self.group), self.dist.P2POp(self.dist.irecv, r, self.lo, self.group)]
-            recv.append((glo, r))
+            ops.append(self.dist.P2POp(self.dist.isend, lo.contiguous(), self.lo, self.group))
         if self.hi >= 0:
-            s, r = hi.contiguous(), torch.empty_like(ghi.contiguous())
-            ops += [self.dist.P2POp(self.dist.isend, s, self.hi, self.group), self.dist.P2POp(self.dist.irecv, r, self.hi, self.group)]
+            r = torch.empty(ghi.shape, dtype=arr.dtype, device=arr.device)
+            ops.append(self.dist.P2POp(self.dist.irecv, r, self.hi, self.group))
             recv.append((ghi, r))
+            ops.append(self.dist.P2POp(self.dist.isend, hi.contiguous(), self.hi, self.group))
+        if self.lo >= 0:
+            r = torch.empty(glo.shape, dtype=arr.dtype, device=arr.device)
+            ops.append(self.dist.P2POp(self.dist.irecv, r, self.lo, self.group))
+            recv.append((glo, r))
         if ops:
             for w in self.dist.batch_isend_irecv(ops):
                 w.wait()

@@ -159,13 +159,20 @@ def test_oracle_slabs_with_a_periodic_x1_direction():
 
 
 # ------------------------------------------------------------------ two gloo ranks, torch.distributed sequencing
-def _rank_main(rank, world, port, q):
+def periodic_case():
+    p = minkowski_params(24, 4, 4)
+    prim0, _ = sound_wave(p, direction=0, amp=1e-3)
+    oracle.Grid(p).apply_bc(prim0)
+    return p, prim0
+
+
+def _rank_main(rank, world, port, q, periodic=False):
     sys.path.insert(0, ROOT)
     sys.path.insert(0, os.path.join(ROOT, "tests"))
     import torch.distributed as dist
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
-    p, prim0 = torus_case("C4", n1=20, n2=12, n3=6)
+    p, prim0 = periodic_case() if periodic else torus_case("C4", n1=20, n2=12, n3=6)
     eng = OracleEngine(slab.slab_params(p, world, rank), prim0[:, slab.slab_slice(p, world, rank)].copy(), as_torch=True)
     me = slab.SlabRank(eng, p, rank, world)
     dt = me.cfl_dt(0.45)
@@ -197,6 +204,27 @@ def test_two_gloo_ranks_reproduce_the_single_domain():
     # and the halo planes each rank holds are its neighbour's interior planes
     assert np.array_equal(res[0][3][:, ng + 10:], ref[:, ng + 10:2 * ng + 10])
     assert np.array_equal(res[1][3][:, :ng], ref[:, 10:10 + ng])
+
+
+def test_two_gloo_ranks_with_a_periodic_x1_direction():
+    """Two ranks, periodic X1: each rank's lower AND upper neighbour is the other rank -- the pairing of the four
+    point-to-point operations must still put the right planes into the right ghosts."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 33500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_rank_main, args=(r, 2, port, q, True)) for r in range(2)]
+    for pr in procs:
+        pr.start()
+    res = sorted((q.get(timeout=300) for _ in procs), key=lambda t: t[0])
+    for pr in procs:
+        pr.join(timeout=60)
+        assert pr.exitcode == 0
+    p, prim0 = periodic_case()
+    ref, dt, _ = single_domain(p, prim0, 3)
+    ng = p["ng"]
+    got = np.concatenate([res[0][3][:, :ng + 12], res[1][3][:, ng:]], axis=1)
+    assert np.array_equal(got, ref)
 
 
 # ------------------------------------------------------------------ GPU: the library's slabs on one device
