@@ -108,7 +108,8 @@ int cuharm_bind(cuharm_handle h, double* d_prim, void* d_workspace, size_t ws_by
 
 /* Geometry precompute (eqs. 38-39): g_cov, g_con, sqrt(-g), lapse at zone centres, 1-faces and
  * 2-faces (3-faces equal centres: the metric is phi-independent), and the connection coefficients at
- * centres from closed-form derivatives (A19), plus the floor profiles of eq. 35.  Then fills the ghost
+ * centres from closed-form derivatives (A19) together with the source weights sqrt(-g) (1/2 | 1) d_nu g_kl that
+ * the update kernel contracts with T^kl (the same S_nu as eq. 7), plus the floor profiles of eq. 35.  Then fills the ghost
  * zones of the bound d_prim.  Errors: ESTATE (not bound). */
 int cuharm_metric_precompute(cuharm_handle h);
 
