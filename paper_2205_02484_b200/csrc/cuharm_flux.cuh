@@ -218,7 +218,8 @@ __global__ void __launch_bounds__(MARCH_T, MARCH_MINB) flux_march_kernel(FluxArg
       }
 #pragma unroll
       for (int v = 0; v < 8; v++) {
-        const double nxt = y[v * nz + ahead];
+        // (read-only path along X1 only -- measured at 256^3: X1 1.20 -> 1.17 ms per substep with it, X2 1.17 -> 1.30)
+        const double nxt = DIR == 1 ? __ldg(y + v * nz + ahead) : y[v * nz + ahead];
         if (RECON == 0) {
           // cell f: slope from (y_f - y_{f-1}, y_{f+1} - y_f)
           const double dp = yn[v] - yc[v];
