@@ -13,7 +13,8 @@ CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libcuharm.so")
 SOURCES = ["cuharm_api.cu"]
-DEPS = ["cuharm_api.cu", "cuharm_phys.cuh", "cuharm_geom.cuh", "cuharm_flux.cuh", "cuharm_kernels.cuh"]
+DEPS = ["cuharm_api.cu", "cuharm_phys.cuh", "cuharm_geom.cuh", "cuharm_flux.cuh", "cuharm_kernels.cuh", "cuharm_chain.cuh",
+        "cuharm_update_tmap.cuh"]
 
 
 def nvcc_path() -> str:
