@@ -202,6 +202,35 @@ int cuharm_last_cfl_dt(cuharm_handle h, double xi, double* dt_out);
  * the corners where that sum exceeds 1e-290 (below it the terms are in the subnormal range).  Synchronises. */
 int cuharm_divb(cuharm_handle h, double* max_abs, double* max_norm);
 
+/* The same two numbers for a caller that cannot allocate device memory and so has no context (a context needs a
+ * workspace of cuharm_workspace_bytes): an in-situ monitor, analysis or I/O plug-in running inside another code's time
+ * loop, where the host application has given the whole device to its own memory pool, hands the plug-in its arrays and
+ * nothing else, and where cudaMalloc / cudaFree may fail on the full device and would stall every stream of the process.
+ * Needs no handle and no workspace, and calls no cudaMalloc, cudaFree or allocating library routine.
+ *   d_prim       DEVICE, prim[8][n1+2ng][n2+2ng][n3+2ng] (layout above); only B^1..3 are read.  With periodic_x3 != 0 the
+ *                first X3 ghost layer must hold the periodic image (as after cuharm_bind / cuharm_step / cuharm_apply_bc)
+ *   d_sqrtg      DEVICE, sqrt(-g) at zone centres, [n1+2ng][n2+2ng] (component 20 of cuharm_get_geom(h, 0, .), or the
+ *                caller's own table); only interior entries are read
+ *   dx           HOST, the three coordinate spacings; periodic_x3: bc_x3 == 1; 1 <= ng <= 8
+ *   cuda_stream  cudaStream_t (NULL = default stream) of the device that is CURRENT at the call
+ *   d_out        DEVICE, 2 doubles: max |D|, max |D| / (sum of the magnitudes of D's own terms) as cuharm_divb defines
+ *                them; written by a kernel on cuda_stream.  Asynchronous: nothing is synchronised or copied to the host
+ * The reduction's scratch (one pair of partial maxima per (i, j) corner row) is a fixed static device array of
+ * CUHARM_DIVB_NOALLOC_MAX_ROWS rows (2 MiB), present on every GPU that loads the library until the process exits.
+ * Limit: (n1 - 1) * (n2 - 1) <= CUHARM_DIVB_NOALLOC_MAX_ROWS (n3 is unlimited; 362 x 362 and 512 x 257 both fit);
+ * beyond it the call returns CUHARM_ENOMEM, launches nothing and leaves d_out alone.
+ * All calls on one device share that array: two calls whose kernels can overlap on the GPU (different streams with no
+ * ordering between them) race and both results are void -- keep the calls on one stream or order them with events.  The
+ * array keeps the previous call's contents; no call depends on them (each overwrites every slot it later reads).
+ * The FIRST call on each device also looks up the array's device address (cudaGetSymbolAddress); make that first call
+ * outside any stream capture.  Thread-safe on the host side.
+ * Errors: EINVAL (null pointer, bad shape, dx not finite and positive), ENOMEM (grid beyond the limit), ECUDA; the text
+ * of the last failure of this call on the calling thread: cuharm_divb_noalloc_errtext(). */
+#define CUHARM_DIVB_NOALLOC_MAX_ROWS 131072
+int cuharm_divb_noalloc(const double* d_prim, const double* d_sqrtg, int32_t n1, int32_t n2, int32_t n3, int32_t ng,
+                        const double dx[3], int32_t periodic_x3, void* cuda_stream, double* d_out);
+const char* cuharm_divb_noalloc_errtext(void);
+
 /* Fluxes through the coordinate shell of zone centres of radial index i (0 <= i < n1), the paper's horizon
  * diagnostics when i is the shell nearest r_h (eqs. 43-46): out[0] = Mdot = sum sqrt(-g) rho u^1,
  * out[1] = phi_B = 1/2 sum sqrt(-g) |B^1| (*F^{rt} = B^r), out[2] = Ldot = sum sqrt(-g) T^1_phi,

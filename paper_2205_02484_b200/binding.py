@@ -94,6 +94,10 @@ def lib():
         L.cuharm_cfl_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
         L.cuharm_last_cfl_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
         L.cuharm_divb.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.cuharm_divb_noalloc.argtypes = [dp, dp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double),
+                                          C.c_int32, vp, dp]
+        L.cuharm_divb_noalloc_errtext.argtypes = []
+        L.cuharm_divb_noalloc_errtext.restype = C.c_char_p
         L.cuharm_shell_fluxes.argtypes = [vp, C.c_int32, C.POINTER(C.c_double)]
         L.cuharm_get_geom.argtypes = [vp, C.c_int32, dp]
         L.cuharm_apply_bc.argtypes = [vp, dp]
@@ -210,6 +214,20 @@ def cuharm_divb(h):
     a, n = C.c_double(), C.c_double()
     _check(lib().cuharm_divb(h, C.byref(a), C.byref(n)), "cuharm_divb")
     return a.value, n.value
+
+
+def cuharm_divb_noalloc(prim, sqrtg, n1, n2, n3, ng, dx, periodic_x3, out, stream=None):
+    """Eq. 23 maxima without a context, a workspace or any allocation (include/cuharm.h): for code that sits inside
+    another program's time loop and may not touch the device allocator.  `prim`, `sqrtg` ([n1g, n2g]) and `out` (2
+    doubles) are CUDA tensors of the current device; the result lands in `out` asynchronously on `stream`.  The scratch
+    is one static array per device shared by all calls: do not let two calls overlap on the GPU; grids with more than
+    CUHARM_DIVB_NOALLOC_MAX_ROWS corner rows are refused."""
+    arr = (C.c_double * 3)(*[float(x) for x in dx])
+    s = C.c_void_p(stream.cuda_stream if stream is not None else 0)
+    rc = lib().cuharm_divb_noalloc(_dptr(prim), _dptr(sqrtg), int(n1), int(n2), int(n3), int(ng), arr,
+                                   1 if periodic_x3 else 0, s, _dptr(out))
+    if rc != 0:
+        raise CuharmError(f"cuharm_divb_noalloc failed ({rc}): {lib().cuharm_divb_noalloc_errtext().decode()}")
 
 
 def cuharm_get_geom(h, loc: int, out):

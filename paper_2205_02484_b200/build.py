@@ -12,8 +12,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libcuharm.so")
-SOURCES = ["cuharm_api.cu"]
-DEPS = ["cuharm_api.cu", "cuharm_phys.cuh", "cuharm_geom.cuh", "cuharm_flux.cuh", "cuharm_kernels.cuh", "cuharm_chain.cuh",
+SOURCES = ["cuharm_api.cu", "cuharm_noalloc.cu"]
+DEPS = ["cuharm_api.cu", "cuharm_noalloc.cu", "cuharm_phys.cuh", "cuharm_geom.cuh", "cuharm_flux.cuh", "cuharm_kernels.cuh", "cuharm_chain.cuh",
         "cuharm_update_tmap.cuh"]
 
 
