@@ -126,7 +126,9 @@ int cuharm_step(cuharm_handle h, double dt);
 /* The same step with dt taken ON THE DEVICE from eq. 26 (A17) applied to the face speeds the predictor
  * of the previous step saw ("the next time step"): dt = min(dt_max, 1 / sum_l max c_w^l / (xi dx^l))
  * (dt_max <= 0: no cap) -- the value cuharm_last_cfl_dt would return, bit for bit, without the read-back and the
- * synchronisation.  Asynchronous.  Errors: ESTATE (no previous step since bind), EINVAL (xi not finite or <= 0). */
+ * synchronisation, including its guard: where that value is not finite and positive (a non-finite face speed; no
+ * speed at all and no cap) dt = 0, the step leaves the state unchanged and cuharm_get_time reports dt_last = 0.
+ * Asynchronous.  Errors: ESTATE (no previous step since bind), EINVAL (xi not finite or <= 0). */
 int cuharm_step_cfl(cuharm_handle h, double xi, double dt_max);
 
 /* The same step in two calls, for a caller that exchanges halo planes between slabs (n1_global > 0): cuharm_set_dt
@@ -149,7 +151,10 @@ int cuharm_step_cfl(cuharm_handle h, double xi, double dt_max);
  *                                          after every pass in which any slab had failed zones; stop when the sum of
  *                                          out[1] over the slabs is 0 (or after pass fixup_max_passes, the last-resort one)
  *   cuharm_substep_finish(h, which)        second ghost fill (needed only if any slab had failed zones); [exchange array]
- * With the exchanges in place every pass sees exactly what the single-domain repair sees. */
+ * With the exchanges in place every pass sees across an internal boundary what the single-domain repair sees there.
+ * Exception: a periodic X1 wrap that coincides with a cut.  The single-domain repair counts ghost zones as good donors
+ * (their flags are 0), so the periodic image of a failed zone donates its unrepaired value; slabs exchange the real flags
+ * and skip it.  With failed zones on both sides of such a wrap the results differ in the repaired zones. */
 int cuharm_set_dt(cuharm_handle h, double dt);
 int cuharm_substep(cuharm_handle h, int32_t which);
 int cuharm_substep_update(cuharm_handle h, int32_t which);

@@ -203,7 +203,7 @@ struct Timed {
 // The repair kernel separates its Jacobi passes by a grid barrier, so its participating blocks must be resident together.
 // A COOPERATIVE launch makes the driver guarantee that (and keeps two such kernels from different streams from holding
 // multiprocessors against each other); it is also what a recorded graph stores.  Devices / drivers without cooperative
-// launch get a plain launch of at most one block per multiprocessor.
+// launch get a plain launch of one block (no barrier needed).
 int launch_fixup(cuharm_ctx* h, const FixArgs& a) {
   if (h->coop) {
     cudaLaunchConfig_t cfg = {};
@@ -222,7 +222,10 @@ int launch_fixup(cuharm_ctx* h, const FixArgs& a) {
     (void)cudaGetLastError();
     h->coop = false;  // not supported here after all: plain launches from now on
   }
-  fixup_kernel<<<h->sms, FIX_THREADS, 0, h->stream>>>(a);
+  // without the cooperative attribute nothing makes several blocks co-resident, and blocks spinning at the kernel's
+  // grid barrier could wait for one that never starts (other streams may hold the multiprocessors): ONE block, which
+  // takes the barrier-free path of the kernel -- slow for many failed zones, never a deadlock
+  fixup_kernel<<<1, FIX_THREADS, 0, h->stream>>>(a);
   h->launches++;
   CK(cudaGetLastError());
   return CUHARM_OK;
@@ -1044,7 +1047,10 @@ int cuharm_repair(cuharm_handle h, double* d_prim, const int32_t* d_flag) {
   const Dims& d = h->d;
   unsigned long long* nfail = h->cnt + CNT_NFAIL;
   unsigned long long* fixw = h->cnt + CNT_FIX;
-  CK(cudaMemsetAsync(h->cnt + CNT_NFAIL, 0, (CNT_STEP_END - CNT_NFAIL) * sizeof(unsigned long long), h->stream));
+  // only the failure counts and the repair scratch: the c_w maxima of the last predictor (CNT_CWPRED) stay, so that a
+  // cuharm_step_cfl / cuharm_last_cfl_dt after this call still sees them
+  CK(cudaMemsetAsync(h->cnt + CNT_NFAIL, 0, (CNT_CWPRED - CNT_NFAIL) * sizeof(unsigned long long), h->stream));
+  CK(cudaMemsetAsync(h->cnt + CNT_FIX, 0, (CNT_STEP_END - CNT_FIX) * sizeof(unsigned long long), h->stream));
   repair_list_kernel<<<dim3((d.n3g + 127) / 128, d.n2g, d.n1g), 128, 0, h->stream>>>(d, d_flag, h->flag, h->list, nfail);
   FixArgs a{d, d_prim, h->flag, h->list, nfail, nullptr, h->cnt + CNT_STATS, fixw, h->gC, h->floors, h->p.fixup_max_passes,
             h->p.gam, newton_cfg(h->p), floor_cfg(h->p)};

@@ -729,7 +729,7 @@ __global__ void __launch_bounds__(128) repair_list_kernel(Dims d, const int* fla
 // one every step).  clock[0] = dt of the current step, clock[1] = time integrated so far.
 // set_dt_kernel: dt chosen by the caller.  dt_from_cw_kernel: eq. 26 from the c_w maxima the predictor of the
 // previous step recorded ("the next time step"), with the host formula of cuharm_last_cfl_dt written out in
-// the same order (IEEE divisions, no contraction possible), so host and device agree bit for bit.
+// the same order (IEEE divisions, no contraction possible) and with the same guard, so host and device agree bit for bit.
 // ---------------------------------------------------------------------------------------------------------
 __global__ void set_dt_kernel(double* clock, double dt) {
   clock[0] = dt;
@@ -747,6 +747,10 @@ __global__ void dt_from_cw_kernel(double* clock, const unsigned long long* cw, d
   }
   double dt = 1.0 / inv;
   if (dt_max > 0.0 && dt > dt_max) dt = dt_max;
+  // the host's guard (dt_of_cw): a non-finite speed (a NaN enters the maxima as +inf) or no speed at all with no cap
+  // gives dt = 0 -- the step that follows leaves the state where it is and the clock does not advance, which
+  // cuharm_get_time shows as dt_last = 0
+  if (!(dt > 0.0) || isinf(dt)) dt = 0.0;
   clock[0] = dt;
   clock[1] += dt;
 }

@@ -10,8 +10,13 @@ each substep and takes the maximum of the face speeds over the slabs for eq. 26.
            second ghost fill, halo exchange of the array
     halo = the outermost ng interior (i) planes of a slab, whole (j, k) extent incl. ghosts  ->  the neighbour's ng
            ghost planes on that side (C4, ng = 3: 3 x 262 x 262 x 8 doubles = 13 MB per side and substep; flags 0.8 MB)
-    With these exchanges every Jacobi pass of the eq. 34 repair sees across an internal boundary exactly what the
-    single-domain repair sees: the decomposition does not change the answer even when zones fail next to a cut.
+    With these exchanges every Jacobi pass of the eq. 34 repair sees across an INTERNAL boundary what the single-domain
+    repair sees there: the decomposition does not change the answer when zones fail next to a cut (pinned bit for bit).
+    One known exception, at a PERIODIC X1 wrap that falls on a cut: the single-domain repair (oracle and library alike)
+    counts every ghost zone as a good donor (ghost flags stay 0; reading A13), so the periodic image of a failed zone
+    donates its unrepaired value, whereas the slabs exchange the real flags and skip it -- the stricter reading of P:L248.
+    With failed zones on BOTH sides of such a wrap the two answers differ (O(1) in the repaired zones); one failed zone
+    alone is bit-equal.  The benchmark configurations have outflow in X1 and are not affected.
 
 The objects below work on any `engine` with the split-step interface of `binding.Solver` (set_dt, substep_update, repair_pass,
 substep_finish, work, flags, end_step, max_passes, cfl_cw, last_cw, dt_of_cw): the library on GPUs, or a CPU stand-in in the host-logic tests.
