@@ -25,10 +25,12 @@ if ROOT not in sys.path:
 METRIC = "zone-cycles/s per full RK2 step at 256^3 fp64 (1 B200); % of HBM roofline"
 UNIT = "zone-cycles/s"
 B_ALG = 1218.0          # algorithmic bytes per zone-cycle
-# algorithmic bytes per zone and launch of each kernel class: flux: read P 64, write 7 comps 56;
-# emf: read 6 B-fluxes 48, write 3 EMFs 24; update: P^n 64 + hydro fluxes 120 + EMFs 24 (+ P-half 64 in the
-# corrector, averaged: +32) in, 64 + 4 (flag) out
-KERNEL_BYTES = {"flux1": 120.0, "flux2": 120.0, "flux3": 120.0, "emf": 72.0, "update": 332.0}
+# algorithmic bytes per zone and launch of each kernel class (SURVEY 8(d) accounting): flux: read P 64, write 7
+# components 56; emf (generic path only): read 6 induction fluxes 48, write 3 EMFs 24; update (the fused kernel evaluates
+# eq. 21 in place, so it reads the six induction-flux components instead of three EMFs): P^n 64 + hydro fluxes 5 x 3 x 8 =
+# 120 + induction fluxes 6 x 8 = 48 + P-half 64 in the corrector only (mean of the two launches: 32) in, P 64 + flag 1 out
+# = 64 + 120 + 48 + 32 + 65 = 329
+KERNEL_BYTES = {"flux1": 120.0, "flux2": 120.0, "flux3": 120.0, "emf": 72.0, "update": 329.0}
 # ncu --set full counters of this command at C4, per launch and averaged over the predictor and corrector launches
 # (DRAM bytes read + written; fp64 DFMA/DMUL/DADD/DSETP warp instructions executed), are READ from the committed
 # summary of the capture, never typed in here.  Only quoted for the workload they were captured on.
@@ -220,31 +222,62 @@ def run_ours(args):
         s.step(dt)
     barrier()
 
-    # ---- timed region: K steps, device-resident inputs, CUDA events on the library's stream -----------------
-    if not args.graph:
-        s.set_timing(True)
-    l0 = s.launch_count()
+    # ---- timed regions: device-resident inputs, CUDA events on the library's stream (= torch's current stream) ----
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    w0 = time.perf_counter()
-    e0.record()
-    for _ in range(args.steps):
+
+    def one_step():
         if args.cfl_each_step:           # second protocol -- a new dt every step from eq. 26, taken on the
             s.step_cfl(0.45)             # device from the previous predictor's face speeds (same graph, no host sync)
         else:
             s.step(dt)
-    e1.record()
-    barrier()
-    w1 = time.perf_counter()
-    ms = e0.elapsed_time(e1)
-    launches = s.launch_count() - l0
-    clocks = sampler.window(w0, w1) if rank == 0 else None
+
+    def timed(n):
+        """n steps between two events, barrier + synchronize on both sides: (max-over-ranks ms, zone-cycles/s of the whole
+        job, clock summary of the window, launches)."""
+        l0 = s.launch_count()
+        barrier()
+        w0 = time.perf_counter()
+        e0.record()
+        for _ in range(n):
+            one_step()
+        e1.record()
+        barrier()
+        w1 = time.perf_counter()
+        ms_, val_ = aggregate(e0.elapsed_time(e1), zones, n, world, dist, "cuda")
+        return ms_, val_, (sampler.window(w0, w1) if rank == 0 else None), s.launch_count() - l0
+
+    # (1) burst: the first K steps after the W warm-up steps -- a fraction of a second, before the board has ramped to its
+    # power cap.  Reported as `burst`; NOT the headline (the metric's workload is hundreds of steps: 500 at C4).
+    if not args.graph:
+        s.set_timing(True)
+    ms_b, val_b, clk_b, _ = timed(args.steps)
     timing = s.get_timing() if not args.graph else {}
     s.set_timing(False)
+    burst = {"steps": args.steps, "ms_per_step": ms_b / args.steps, "value": val_b, "unit": UNIT, "clocks": clk_b,
+             "note": "first K steps after the warm-up, board not yet at its power cap"}
+
+    # (2) sustained: after >= sustain_warm_s seconds of the same load, >= 300 steps (and >= sustain_s seconds) timed the
+    # same way; clocks, power and throttle reasons over that window ride along.
+    sustained = None
+    if args.sustain_s > 0:
+        est = ms_b / args.steps
+        n_warm = max(1, int(args.sustain_warm_s * 1e3 / est))
+        n_sus = max(300, int(args.sustain_s * 1e3 / est))
+        barrier()
+        for _ in range(n_warm):
+            one_step()
+        ms_s, val_s, clk_s, _ = timed(n_sus)
+        sustained = {"steps": n_sus, "warm_steps": n_warm, "ms_per_step": ms_s / n_sus, "value": val_s, "unit": UNIT,
+                     "seconds": ms_s * 1e-3, "clocks": clk_s,
+                     "divb_norm": s.divb()[1], "failed_inversions": int(s.stats()[0])}
+
+    # (3) headline: EXACTLY K steps, timed straight after the sustained leg, i.e. with the board in the state the metric's
+    # own run (BASELINE.json: 500 steps at C4) spends nearly all of its time in.  With --sustain-s 0 this region follows
+    # the burst directly (use --steps 500 --sustain-s 0 to time the config's own step count as one region).
+    ms, value, clocks, launches = timed(args.steps)
     if args.graph:
-        # per-kernel durations for the roofline object: a second, short pass of the same steps launched kernel by
-        # kernel with CUDA events around each launch (the graph replay above has no place for them); its events sit
-        # on the library's stream inside the loop below, after the headline region has been timed
+        # per-kernel durations for the roofline objects: a short pass of the same steps launched kernel by kernel with
+        # CUDA events around each launch (a graph replay has no place for them), after the headline region
         s.use_graph(False)
         s.set_timing(True)
         barrier()
@@ -254,33 +287,8 @@ def run_ours(args):
         timing = s.get_timing()
         s.set_timing(False)
         s.use_graph(True)
-    ms, value = aggregate(ms, zones, args.steps, world, dist, "cuda")
     divb = s.divb()[1]
     stats = s.stats()
-
-    # ---- sustained: the metric's own workload is hundreds of steps (BASELINE.json: 500 at C4), long enough for the
-    # board to reach its power cap.  After >= sustain_warm_s seconds of the same load, time >= 300 steps (and >=
-    # sustain_s seconds) the same way; clocks, power and throttle reasons over that window ride along.
-    sustained = None
-    if args.sustain_s > 0:
-        est = ms / args.steps
-        n_warm = max(1, int(args.sustain_warm_s * 1e3 / est))
-        n_sus = max(300, int(args.sustain_s * 1e3 / est))
-        barrier()
-        for _ in range(n_warm):
-            s.step(dt)
-        barrier()
-        ws0 = time.perf_counter()
-        e0.record()
-        for _ in range(n_sus):
-            s.step(dt)
-        e1.record()
-        barrier()
-        ws1 = time.perf_counter()
-        ms_s, val_s = aggregate(e0.elapsed_time(e1), zones, n_sus, world, dist, "cuda")
-        sustained = {"steps": n_sus, "warm_steps": n_warm, "ms_per_step": ms_s / n_sus, "value": val_s, "unit": UNIT,
-                     "seconds": ms_s * 1e-3, "clocks": sampler.window(ws0, ws1) if rank == 0 else None,
-                     "divb_norm": s.divb()[1], "failed_inversions": int(s.stats()[0])}
 
     # ---- e2e: the same step through the public API with HOST buffers: H2D of the primitives from pinned memory,
     # one step, D2H of the result into pinned memory, every step inside the timed region.  Three solver objects on three
@@ -318,6 +326,20 @@ def run_ours(args):
     for sx, _, _ in lanes[1:]:
         sx.close()
     ms_e2e, e2e_val = aggregate(ms_e2e, zones, e2e_steps, world, dist, "cuda")
+    # the same through ONE solver as a time-dependent run: step n+1 loads the host array step n wrote, so nothing overlaps
+    # (H2D -> ghost fill -> step -> D2H, one after the other on one stream)
+    ser_steps = max(2, min(6, e2e_steps))
+    host_state = lanes[0][2]
+    host_state.copy_(prim_pinned)
+    barrier()
+    e0.record()
+    for n in range(ser_steps):
+        s.load(host_state)
+        s.step(dt)
+        host_state.copy_(s.prim, non_blocking=True)
+    e1.record()
+    barrier()
+    _, e2e_serial = aggregate(e0.elapsed_time(e1), zones, ser_steps, world, dist, "cuda")
     nbytes = prim_pinned.numel() * 8
     if rank == 0:
         sampler.stop()
@@ -329,6 +351,7 @@ def run_ours(args):
         roof = None
         roof_alu = None
         shares = {}
+        per_kernel = []      # every kernel class: algorithmic GB/s against the HBM peak, ncu DRAM bytes, fp64 pipe fraction
         if timing:
             tot = sum(v[0] for v in timing.values())
             shares = {k: round(v[0] / tot, 4) for k, v in timing.items() if v[1]}
@@ -342,6 +365,20 @@ def run_ours(args):
                             "unit": "fp64 warp-instructions/s", "frac": a_alu / FP64_WARP_INST_PER_S,
                             "peak_source": "148 SMs x 4 sub-partitions x 1.965 GHz / 2 cycles per fp64 warp instruction",
                             "count_source": f"ncu, {ncu_src}"}
+            for k in KERNEL_BYTES:
+                if not timing[k][1]:
+                    continue
+                ms_k = timing[k][0] / timing[k][1]
+                nk = ncu_all.get(k) if (args.config == "C4" and world == 1) else None
+                gbs = KERNEL_BYTES[k] * zones / (ms_k * 1e-3) / 1e9
+                per_kernel.append({
+                    "kernel": k, "launches_per_step": 2, "algorithmic_bytes_per_zone": KERNEL_BYTES[k],
+                    "ms_per_launch": ms_k, "achieved": gbs, "unit": "GB/s", "frac": gbs / peak,
+                    "traffic": nk["traffic"] if nk else None,
+                    "traffic_over_algorithmic": nk["traffic"] / (KERNEL_BYTES[k] * zones) if nk else None,
+                    "dram_frac": nk["traffic"] / (ms_k * 1e-3) / 1e9 / peak if nk else None,
+                    "fp64_frac": nk["fp64_warp_inst"] / (ms_k * 1e-3) / FP64_WARP_INST_PER_S if nk else None,
+                    "time_share": shares.get(k)})
             roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                     "frac": achieved / peak, "traffic": ncu["traffic"] if ncu else None,
                     "traffic_source": f"ncu --set full, {ncu_src}" if ncu else None, "peak_source": peak_src,
@@ -355,6 +392,7 @@ def run_ours(args):
                     "peak_source": peak_src}
         if sustained is not None:
             sustained["step_frac_of_hbm_roofline"] = sustained["value"] / world * B_ALG / (peak * 1e9)
+        burst["step_frac_of_hbm_roofline"] = burst["value"] / world * B_ALG / (peak * 1e9)
         cpu = None
         if not args.no_cpu:
             # SURVEY 8(d) "CPU baseline": (i) all host cores, full steps of this config; (ii) one core at C3
@@ -379,8 +417,15 @@ def run_ours(args):
                           "dt": dt},
                "clocks": clocks, "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": nbytes,
                                          "d2h_bytes_per_step": nbytes, "steps": e2e_steps,
-                                         "pipeline": "3 solver objects on 3 streams, steps dealt round-robin"},
-               "gpu_launches": int(launches), "roofline": roof, "roofline_alu": roof_alu, "sustained": sustained,
+                                         "pipeline": "3 solver objects on 3 streams, steps dealt round-robin (independent "
+                                                     "one-step problems)",
+                                         "serial": {"value": e2e_serial, "unit": UNIT, "steps": ser_steps,
+                                                    "pipeline": "one solver, one stream; step n+1 loads the host array "
+                                                                "step n wrote (a time-dependent run through host buffers)"}},
+               "gpu_launches": int(launches), "roofline": roof, "roofline_alu": roof_alu,
+               "roofline_per_kernel": per_kernel, "burst": burst, "sustained": sustained,
+               "headline_region": ("K steps timed after the sustained leg (board at the steady state of the metric's "
+                                   "500-step run)" if sustained is not None else "K steps after the warm-up and the burst leg"),
                "cpu_baseline": cpu,
                "checks": {"divb_norm": divb, "stats": stats}}
         print(json.dumps(out), flush=True)
