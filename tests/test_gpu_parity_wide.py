@@ -241,6 +241,38 @@ def test_non_finite_wave_speed_gives_zero_dt():
     s.close()
 
 
+def test_device_side_eq26_carries_the_host_guard_and_repair_keeps_the_face_speeds():
+    """(i) cuharm_step_cfl takes dt on the device; where the host formula answers 0 (a non-finite face speed)
+    the device must answer 0 too -- a step that leaves the clock where it is -- not 1/0 or NaN; (ii) cuharm_repair as a
+    stage of its own must not wipe the face-speed maxima of the last predictor, which cuharm_step_cfl reads next."""
+    p = minkowski_params(8, 8, 8)
+    prim = np.zeros((8, 14, 14, 14))
+    prim[0] = 1.0; prim[1] = 1.0
+    prim[1, 6, 6, 6] = np.nan
+    s = cu.Solver(p, prim)
+    s.step(1e-3)                                   # its predictor records a non-finite c_w
+    assert s.last_cfl_dt(0.45) == 0.0
+    t_before = s.time()[0]
+    s.step_cfl(0.45)
+    t_after, dt_last = s.time()
+    assert dt_last == 0.0 and t_after == t_before
+    s.close()
+    p = config("C4", n1=24, n2=20, n3=12)
+    prim0, _ = fm_torus(p)
+    s = cu.Solver(p, prim0)
+    s.step(s.cfl_dt(0.45))
+    cw = s.last_cw()
+    expect = s.last_cfl_dt(0.45)
+    flag = torch.zeros(s.shape[1:], dtype=torch.int32, device=s.device)
+    flag[10, 9, 7] = 2
+    work = s.prim.clone()
+    s.repair(work, flag)
+    assert s.last_cw() == cw and min(cw) > 0.0
+    s.step_cfl(0.45)
+    assert s.time()[1] == expect and expect > 0.0
+    s.close()
+
+
 # ------------------------------------------------------------------ tensor-map vs one-dimensional bulk-copy staging
 def test_tensor_map_update_kernel_is_bitwise_the_row_copy_kernel(monkeypatch):
     """update_tmap_kernel (12 tensor-map boxes per tile) against update_tma_kernel (63 row copies per tile; selected by
