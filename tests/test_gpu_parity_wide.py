@@ -41,11 +41,9 @@ CEIL_CASES = [
     # the torus' own field against tight limits: ceilings fire in ~1e3 zones, few failures
     ("tight limits", dict(sigma_max=1e-4, b2_over_u_max=1e-2, gamma_max=1.5), 1.0, 2.0),
 ]
-# The Lorentz cap is exercised with Gamma_max = 1.5 against a Gamma = 2 patch, not with the paper's 50 against Gamma =
-# 80: a Gamma = 80 patch next to floor-density zones at rest makes the update of those neighbours a difference of
-# terms 1e5 times larger than the result, and the two sides then differ by 1e-9 in rho there for conditioning
-# reasons (measured: 26 zones above 1e-11, unchanged by two extra Newton updates).  The rescale formula (A12) at the
-# paper's Gamma_max = 50 is compared zone by zone in test_floors_stage_matches_the_oracle_zone_by_zone below.
+# Here the Lorentz cap is exercised with Gamma_max = 1.5 against a Gamma = 2 patch; the paper's 50 against Gamma = 80 inside a
+# step is test_lorentz_cap_inside_a_step_at_the_papers_gamma_max_50 below (a conditioning-aware comparison), and the rescale
+# formula (A12) at Gamma_max = 50 is compared zone by zone in test_floors_stage_matches_the_oracle_zone_by_zone.
 
 
 @pytest.mark.parametrize("label,kw,bscale,gpatch", CEIL_CASES, ids=[c[0] for c in CEIL_CASES])
@@ -74,6 +72,62 @@ def test_ceilings_and_lorentz_cap_fire_and_match(label, kw, bscale, gpatch):
     assert (err < 1e-8).all(), err
     assert s.divb()[1] < 1e-12
     s.close()
+
+
+def _zone_errors(p, got, ref):
+    """The parity-policy measure zone by zone (interior): pointwise relative for rho and u, |dq| / max_grid|q_ref| for
+    utilde^i and B^i."""
+    g, r = interior(p, got), interior(p, ref)
+    e = np.zeros_like(r)
+    for v in range(8):
+        if v < 2:
+            e[v] = np.abs(g[v] - r[v]) / np.abs(r[v])
+        else:
+            grp = slice(2, 5) if v < 5 else slice(5, 8)
+            scale = max(float(np.max(np.abs(r[v]))), 1e-3 * float(np.max(np.abs(r[grp]))))
+            e[v] = np.abs(g[v] - r[v]) / scale
+    return e
+
+
+def test_lorentz_cap_inside_a_step_at_the_papers_gamma_max_50():
+    """P:L265 (A12) at the paper's own Gamma_max = 50 against a Gamma = 80 patch, inside a full RK2 step.  The patch sits
+    next to floor-density zones at rest, whose update is then a difference of terms ~1e5 times the result: in a few tens of
+    zones the two sides differ by more than 1e-11 (up to ~1e-9 in rho).  That this is conditioning and not a difference
+    of method is SHOWN here, not asserted in a comment: the oracle is run again on inputs wiggled by 1e-15 relative (four
+    seeds), and in every zone and primitive where library and oracle differ by more than 1e-11 the oracle's own answer
+    moves by at least a tenth as much (measured: 0.37 at the least).  Everywhere else the one-step tolerance holds; counters are equal; caps fire."""
+    p = config("C4", n1=32, n2=32, n3=20)
+    assert p["gamma_max"] == 50.0
+    prim0 = strong_field_state(p, 1.0, 80.0)
+    ref = prim0.copy()
+    g = oracle.Grid(p)
+    g.bind(ref)
+    dt = g.cfl_dt(0.45)
+    s = cu.Solver(p, prim0)
+    g.step(dt)
+    s.step(dt)
+    st, sr = list(s.stats()), [int(x) for x in g.get_stats()]
+    assert sr[5] > 0 and st[:6] == sr[:6], (st, sr)
+    diff = _zone_errors(p, s.prim.cpu().numpy(), ref)
+    s.close()
+    kappa = (interior(p, ref)[0] + p["gam"] * interior(p, ref)[1]) / interior(p, ref)[1]
+    diff[1] /= np.maximum(1.0, 1e-14 * kappa / 1e-11)             # prim_errors' kappa rule for u
+    loose = diff >= 1e-11
+    nz = int(np.count_nonzero(loose.any(axis=0)))
+    sens = np.zeros_like(diff)
+    for seed in (31, 32, 33, 34):
+        w = prim0 * (1.0 + 1e-15 * rng(seed).choice([-1.0, 1.0], size=prim0.shape))
+        gw = oracle.Grid(p)
+        gw.bind(w)
+        gw.step(dt)
+        e = _zone_errors(p, w, ref)
+        e[1] /= np.maximum(1.0, 1e-14 * kappa / 1e-11)
+        sens = np.maximum(sens, e)
+    print(f"Gamma_max = 50, Gamma = 80 patch: {nz} zones beyond 1e-11 (worst {diff.max():.2e}); the oracle's own response "
+          f"to a 1e-15 input wiggle there: min ratio {np.min(sens[loose] / diff[loose]) if nz else float('nan'):.2f}, "
+          f"caps applied {sr[5]}")
+    assert nz < 200, nz
+    assert (sens[loose] >= 0.1 * diff[loose]).all(), (diff[loose], sens[loose])
 
 
 def test_floors_stage_matches_the_oracle_zone_by_zone():
