@@ -543,6 +543,18 @@ def run_repair_scaling(args):
     s.close()
 
 
+def run_fp64_peak():
+    """--fp64-peak: build and run bench_fp64_peak.cu (beside this file), the DFMA micro-benchmark behind the "alu" roofline
+    peak: cycles per warp-level DFMA per SM sub-partition and the device-wide rate for ILP x
+    resident-warps combinations.  A measurement aid; nothing in the library depends on it."""
+    import tempfile
+    src = os.path.join(ROOT, "bench_fp64_peak.cu")
+    with tempfile.TemporaryDirectory() as tmp:
+        exe = os.path.join(tmp, "fp64_peak")
+        subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", exe, src], check=True)
+        return subprocess.run([exe]).returncode
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -562,7 +574,10 @@ def main():
     ap.add_argument("--decompose", action="store_true", help="one grid cut into WORLD_SIZE slabs (strong scaling) instead of replicas")
     ap.add_argument("--repair-scaling", action="store_true", help="time the eq. 34 repair at 1e3 / 1e5 / 1e6 failed zones")
     ap.add_argument("--threads", type=int, default=0, help="reference arm: OpenMP threads of the oracle (0 = all)")
+    ap.add_argument("--fp64-peak", action="store_true", help="run the DFMA micro-benchmark (bench_fp64_peak.cu) and exit")
     args = ap.parse_args()
+    if args.fp64_peak:
+        sys.exit(run_fp64_peak())
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.repair_scaling:
         run_repair_scaling(args)

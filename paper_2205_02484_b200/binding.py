@@ -52,8 +52,8 @@ def make_params(d: dict) -> CuharmParams:
 
 
 def lib_path() -> str:
-    """The in-tree library; CUHARM_LIB names another build of the same sources (e.g. a tuning variant)."""
-    return os.environ.get("CUHARM_LIB") or os.path.join(HERE, "libcuharm.so")
+    """The in-tree library (the only one this binding loads)."""
+    return os.path.join(HERE, "libcuharm.so")
 
 
 def lib():

@@ -205,7 +205,7 @@ def test_ten_steps_perturbed_torus_and_divb():
     assert list(s.stats()[:6]) == list(g.get_stats()[:6])
 
 
-def test_c1_config_100_steps_parity_and_divb():
+def test_c1_config_100_steps_reported_bound_not_a_north_star_tolerance_and_divb():
     p = config("C1")
     prim0, _ = fm_torus(p, beta_mode="min")
     got, ref, s, g, dt = both(p, prim0, 100, xi=0.9)
