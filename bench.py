@@ -543,6 +543,61 @@ def run_repair_scaling(args):
     s.close()
 
 
+def run_chain_cost(args):
+    """--chain: what the inversion fallback chain of P:L229-239 costs where it is hot.  The headline grid
+    with inv_chain = 1 and beta_min = 1e-2 (eq. 33: zones below it take the entropy method as first and only choice), the
+    torus field scaled up until at least `--chain-frac` of the zones are eq. 33 zones; sustained-style timing of the same
+    state with the chain off and on; chain counters per step in the line."""
+    import torch
+    import paper_2205_02484_b200 as cu
+    p0, prim_host = make_workload(args.config)
+    zones = p0["n1"] * p0["n2"] * p0["n3"]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def run(p, prim, nsteps):
+        s = cu.Solver(p, torch.from_numpy(prim).pin_memory())
+        dt = s.cfl_dt(0.45)
+        s.use_graph(True)
+        for _ in range(3):
+            s.step(dt)
+        c0, st0 = (s.chain_stats() if p["inv_chain"] else [0] * 4), s.stats()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(nsteps):
+            s.step(dt)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / nsteps
+        c1, st1 = (s.chain_stats() if p["inv_chain"] else [0] * 4), s.stats()
+        out = {"ms_per_step": ms, "chain_per_step": [(b - a) / nsteps for a, b in zip(c0, c1)],
+               "failed_inversions_per_step": (st1[0] - st0[0]) / nsteps, "repaired_per_step": (st1[1] - st0[1]) / nsteps,
+               "divb_norm": s.divb()[1], "dt": dt}
+        s.close()
+        return out
+
+    rows = []
+    for bscale in (1.0, 30.0, 100.0, 300.0, 1000.0):
+        prim = prim_host.copy()
+        prim[5:8] *= bscale
+        on = run(dict(p0, inv_chain=1, beta_min=args.beta_min), prim, 3)
+        frac = on["chain_per_step"][3] / (2.0 * zones)          # eq. 33 zones per substep / zones
+        rows.append({"bscale": bscale, "eq33_zone_fraction": frac, "probe_ms_per_step": on["ms_per_step"]})
+        if frac >= args.chain_frac:
+            break
+    prim = prim_host.copy()
+    prim[5:8] *= rows[-1]["bscale"]
+    off = run(dict(p0, inv_chain=0), prim, args.steps)
+    on = run(dict(p0, inv_chain=1, beta_min=args.beta_min), prim, args.steps)
+    base = run(dict(p0, inv_chain=1, beta_min=args.beta_min), prim_host.copy(), args.steps)
+    print(json.dumps({"chain_cost": {"config": args.config, "beta_min": args.beta_min, "steps": args.steps, "search": rows,
+                                     "bscale": rows[-1]["bscale"], "chain_off": off, "chain_on": on,
+                                     "chain_on_unscaled_field": base,
+                                     "extra_ms_per_step": on["ms_per_step"] - off["ms_per_step"],
+                                     "extra_frac_of_step": on["ms_per_step"] / off["ms_per_step"] - 1.0,
+                                     "chain_per_step_legend": ["2D failed -> chain", "recovered by 1D-W", "recovered by entropy",
+                                                               "eq. 33 zones (entropy first and only)"]}}), flush=True)
+
+
 def run_fp64_peak():
     """--fp64-peak: build and run bench_fp64_peak.cu (beside this file), the DFMA micro-benchmark behind the "alu" roofline
     peak: cycles per warp-level DFMA per SM sub-partition and the device-wide rate for ILP x
@@ -574,12 +629,17 @@ def main():
     ap.add_argument("--decompose", action="store_true", help="one grid cut into WORLD_SIZE slabs (strong scaling) instead of replicas")
     ap.add_argument("--repair-scaling", action="store_true", help="time the eq. 34 repair at 1e3 / 1e5 / 1e6 failed zones")
     ap.add_argument("--threads", type=int, default=0, help="reference arm: OpenMP threads of the oracle (0 = all)")
+    ap.add_argument("--chain", action="store_true", help="cost of the inversion fallback chain on a magnetised state")
+    ap.add_argument("--chain-frac", type=float, default=0.05, help="--chain: scale B until this fraction of zones are eq. 33 zones")
+    ap.add_argument("--beta-min", type=float, default=1e-2, help="--chain: eq. 33 threshold")
     ap.add_argument("--fp64-peak", action="store_true", help="run the DFMA micro-benchmark (bench_fp64_peak.cu) and exit")
     args = ap.parse_args()
     if args.fp64_peak:
         sys.exit(run_fp64_peak())
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    if args.repair_scaling:
+    if args.chain:
+        run_chain_cost(args)
+    elif args.repair_scaling:
         run_repair_scaling(args)
     elif args.decompose and args.impl == "ours":
         run_decomposed(args)
