@@ -167,32 +167,55 @@ class SlabRank:
         self.engine, self.p, self.rank, self.world = engine, p, rank, world
         self.n1 = slab_ranges(p["n1"], world)[rank][1]
         self.lo, self.hi = neighbours(p, world, rank)
+        self._bufs = {}     # halo send / receive buffers by (device, layout)
 
-    def _exchange(self, arr):
+    def _exchange(self, arr, flags=None):
+        """Halo planes of `arr` (and, when given, of the flag array) to and from both neighbours: ONE message per neighbour
+        and direction -- planes and flags packed into a byte buffer -- and buffers that are allocated once per layout and
+        reused by every later exchange (no allocation, no .contiguous() copy in the steady state)."""
         import torch
         ng = self.p["ng"]
-        lo, hi, glo, ghi = _planes(arr, ng, self.n1)
+        parts = [arr] if flags is None else [arr, flags]
+        planes = [_planes(a, ng, self.n1) for a in parts]
+        sizes = [pl[0].numel() * pl[0].element_size() for pl in planes]      # bytes per side; the fp64 part comes first, so
+        key = (str(arr.device), tuple(sizes))                                 # every part starts on a multiple of 8 bytes
+        buf = self._bufs.get(key)
+        if buf is None:
+            buf = [torch.empty(sum(sizes), dtype=torch.uint8, device=arr.device) for _ in range(4)]
+            self._bufs[key] = buf
+        send_lo, send_hi, recv_lo, recv_hi = buf
+
+        def pieces(b, which):
+            off = 0
+            for a, pl, sz in zip(parts, planes, sizes):
+                yield b[off:off + sz].view(a.dtype).view(pl[which].shape), pl[which]
+                off += sz
+
         # Order of the operations: [send lowest planes down, receive upper ghosts from above, send highest planes up,
         # receive lower ghosts from below].  NCCL pairs point-to-point operations between two ranks by ORDER, and with two
         # ranks and a periodic direction the lower and the upper neighbour are the same rank: in this order its first send
         # (its lowest planes) meets my first receive (my upper ghosts), as it must.
-        ops, recv = [], []
+        ops = []
         if self.lo >= 0:
-            ops.append(self.dist.P2POp(self.dist.isend, lo.contiguous(), self.lo, self.group))
+            for dst, src in pieces(send_lo, 0):
+                dst.copy_(src)
+            ops.append(self.dist.P2POp(self.dist.isend, send_lo, self.lo, self.group))
         if self.hi >= 0:
-            r = torch.empty(ghi.shape, dtype=arr.dtype, device=arr.device)
-            ops.append(self.dist.P2POp(self.dist.irecv, r, self.hi, self.group))
-            recv.append((ghi, r))
-            ops.append(self.dist.P2POp(self.dist.isend, hi.contiguous(), self.hi, self.group))
+            ops.append(self.dist.P2POp(self.dist.irecv, recv_hi, self.hi, self.group))
+            for dst, src in pieces(send_hi, 1):
+                dst.copy_(src)
+            ops.append(self.dist.P2POp(self.dist.isend, send_hi, self.hi, self.group))
         if self.lo >= 0:
-            r = torch.empty(glo.shape, dtype=arr.dtype, device=arr.device)
-            ops.append(self.dist.P2POp(self.dist.irecv, r, self.lo, self.group))
-            recv.append((glo, r))
+            ops.append(self.dist.P2POp(self.dist.irecv, recv_lo, self.lo, self.group))
         if ops:
             for w in self.dist.batch_isend_irecv(ops):
                 w.wait()
-        for dst, buf in recv:
-            dst.copy_(buf)
+        if self.hi >= 0:
+            for src, dst in pieces(recv_hi, 3):
+                dst.copy_(src)
+        if self.lo >= 0:
+            for src, dst in pieces(recv_lo, 2):
+                dst.copy_(src)
 
     def _allsum(self, a, b):
         import torch
@@ -204,19 +227,16 @@ class SlabRank:
     def _substep(self, which: int):
         e = self.engine
         e.substep_update(which)
-        self._exchange(e.work(which))
-        self._exchange(e.flags[None])
+        self._exchange(e.work(which), e.flags[None])
         nf, left = self._allsum(*e.repair_pass(which, 0))
         if nf == 0:
             return
         npass = 0
-        self._exchange(e.work(which))
-        self._exchange(e.flags[None])
+        self._exchange(e.work(which), e.flags[None])
         while left > 0 and npass < e.max_passes:
             npass += 1
             _, left = self._allsum(*e.repair_pass(which, npass))
-            self._exchange(e.work(which))
-            self._exchange(e.flags[None])
+            self._exchange(e.work(which), e.flags[None])
         e.substep_finish(which)
         self._exchange(e.work(which))
 
