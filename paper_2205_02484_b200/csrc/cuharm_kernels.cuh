@@ -354,6 +354,71 @@ __host__ __device__ constexpr int upd_smem(int tb) { return (UPD_NROW * upd_row(
 struct TileIdx { int i, j, c; };  // zone-row (i, j) (interior numbering) and 128-zone chunk of a tile
 struct TileCnt { int s, i, jj, c; };  // mixed-radix tile counter: j-strip, i, j within the strip, chunk
 
+// The tile walk of the two staged update kernels (update_tma_kernel here, update_tmap_kernel in cuharm_update_tmap.cuh).
+// Tile order: strips of wj rows j; inside a strip i runs slower than j, the chunk fastest.  The blocks resident at one
+// time then cover a patch of (several i) x (wj j) rows, so the rows a tile shares with its i- and j-neighbours (F1[i+1],
+// F2[j+1], the induction fluxes around each edge) are re-read while still in L2.  The first tile of a block and the
+// stride G between its tiles are decomposed once; after that the counter is carried (no division in the tile loop).
+struct TileWalk {
+  TileCnt cur, dlt;
+  int nch, wj, n1;
+  __device__ __forceinline__ TileWalk(int tile, int G, int nch_, int wj_, int n1_) : nch(nch_), wj(wj_), n1(n1_) {
+    int r = tile;
+    cur.c = r % nch; r /= nch; cur.jj = r % wj; r /= wj; cur.i = r % n1; cur.s = r / n1;
+    r = G;
+    dlt.c = r % nch; r /= nch; dlt.jj = r % wj; r /= wj; dlt.i = r % n1; dlt.s = r / n1;
+  }
+  __device__ __forceinline__ void advance() {
+    TileCnt y{cur.s + dlt.s, cur.i + dlt.i, cur.jj + dlt.jj, cur.c + dlt.c};
+    if (y.c >= nch) { y.c -= nch; y.jj++; }
+    if (y.jj >= wj) { y.jj -= wj; y.i++; }
+    if (y.i >= n1) { y.i -= n1; y.s++; }
+    cur = y;
+  }
+  __device__ __forceinline__ TileIdx idx() const { return TileIdx{cur.i, cur.s * wj + cur.jj, cur.c}; }
+};
+
+// Eq. 21 (A3) on the twelve edges of a zone, from the staged induction fluxes: the expressions and the
+// operand order of emf_kernel, written once for both staged kernels.  `S` maps a logical operand -- which induction
+// flux, and its offsets from the zone in the two directions it is indexed by here -- to the kernel's own stage layout:
+//   S::template at<ARRAY, A, B>()   ARRAY = one of the EMF_* below; (A, B) = (dj, dk) for F2B3 / F3B2, (di, dk) for
+//                                   F3B1 / F1B3, (di, dj) for F1B2 / F2B1
+// ex[0..3] = E1 at (j, k), (j+1, k), (j, k+1), (j+1, k+1); ex[4..7] = E2 at (i, k), (i+1, k), (i, k+1), (i+1, k+1);
+// ex[8..11] = E3 at (i, j), (i+1, j), (i, j+1), (i+1, j+1).
+enum { EMF_F2B3 = 0, EMF_F3B2, EMF_F3B1, EMF_F1B3, EMF_F1B2, EMF_F2B1 };
+template <int A, int B, class S>
+__device__ __forceinline__ void edge_emf_triple(const S& st, double ex[12]) {
+  // E1(j',k') = (F2B3[j'][k'] + F2B3[j'][k'-1] - F3B2[j'][k'] - F3B2[j'-1][k']) / 4
+  ex[A + 2 * B] = 0.25 * (st.template at<EMF_F2B3, A, B>() + st.template at<EMF_F2B3, A, B - 1>() -
+                          st.template at<EMF_F3B2, A, B>() - st.template at<EMF_F3B2, A - 1, B>());
+  // E2(i',k') = (F3B1[i'][k'] + F3B1[i'-1][k'] - F1B3[i'][k'] - F1B3[i'][k'-1]) / 4
+  ex[4 + A + 2 * B] = 0.25 * (st.template at<EMF_F3B1, A, B>() + st.template at<EMF_F3B1, A - 1, B>() -
+                              st.template at<EMF_F1B3, A, B>() - st.template at<EMF_F1B3, A, B - 1>());
+  // E3(i',j') = (F1B2[i'][j'] + F1B2[i'][j'-1] - F2B1[i'][j'] - F2B1[i'-1][j']) / 4
+  ex[8 + A + 2 * B] = 0.25 * (st.template at<EMF_F1B2, A, B>() + st.template at<EMF_F1B2, A, B - 1>() -
+                              st.template at<EMF_F2B1, A, B>() - st.template at<EMF_F2B1, A - 1, B>());
+}
+template <class S>
+__device__ __forceinline__ void edge_emfs(const S& st, double ex[12]) {
+  edge_emf_triple<0, 0>(st, ex);
+  edge_emf_triple<1, 0>(st, ex);
+  edge_emf_triple<0, 1>(st, ex);
+  edge_emf_triple<1, 1>(st, ex);
+}
+
+// stage layout of update_tma_kernel (row table above): rows of UPD_ROW doubles, z = this zone in row 0
+template <int UPD_ROW>
+struct RowStage {
+  const double* z;
+  template <int ARR, int A, int B>
+  __device__ __forceinline__ double at() const {
+    constexpr int row = ARR == EMF_F2B3 ? 41 + A : ARR == EMF_F3B2 ? 44 + A : ARR == EMF_F3B1 ? 47 + A : ARR == EMF_F1B3 ? 49 + A
+                        : ARR == EMF_F1B2 ? 51 + 3 * A + (B + 1) : 57 + 3 * B + (A + 1);
+    constexpr int off = ARR == EMF_F1B2 || ARR == EMF_F2B1 ? 0 : B;   // E3's operands sit at the zone's own k
+    return z[row * UPD_ROW + off];
+  }
+};
+
 // Persistent blocks: block b takes tiles b, b + gridDim.x, ...; tile = (i, j, 128-zone chunk of the row), chunk
 // fastest.  One stage per block: the stage is free again as soon as every thread has moved its operands to
 // registers, which is the first thing a tile does, so the copies of tile n+1 fly during the whole of tile n's
@@ -377,26 +442,8 @@ __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kern
   }
   __syncthreads();
   int tile = blockIdx.x;
-  // Tile order: strips of wj rows j; inside a strip i runs slower than j, the chunk fastest.  The blocks resident
-  // at one time then cover a patch of (several i) x (wj j) rows, so the rows a tile shares with its i- and
-  // j-neighbours (F1[i+1], F2[j+1], the induction fluxes around each edge) are re-read while still in L2.
-  // Decomposition of the first tile and of the stride, then carried increments (no division in the loop).
-  TileCnt ccur, cdlt;
-  {
-    int r = tile;
-    ccur.c = r % nch; r /= nch; ccur.jj = r % wj; r /= wj; ccur.i = r % d.n1; ccur.s = r / d.n1;
-    r = G;
-    cdlt.c = r % nch; r /= nch; cdlt.jj = r % wj; r /= wj; cdlt.i = r % d.n1; cdlt.s = r / d.n1;
-  }
-  auto advance_cnt = [&](const TileCnt& x) {
-    TileCnt y{x.s + cdlt.s, x.i + cdlt.i, x.jj + cdlt.jj, x.c + cdlt.c};
-    if (y.c >= nch) { y.c -= nch; y.jj++; }
-    if (y.jj >= wj) { y.jj -= wj; y.i++; }
-    if (y.i >= d.n1) { y.i -= d.n1; y.s++; }
-    return y;
-  };
-  auto to_idx = [&](const TileCnt& x) { return TileIdx{x.i, x.s * wj + x.jj, x.c}; };
-  TileIdx cur = to_idx(ccur), nxt;
+  TileWalk walk(tile, G, nch, wj, d.n1);  // strip order (see TileWalk)
+  TileIdx cur = walk.idx(), nxt;
   auto tile_base = [&](const TileIdx& x) {  // element offset of the first staged zone of the tile's row
     return (long long)(d.ng + x.i) * d.s1 + (long long)(d.ng + x.j) * d.s2 + (d.ng + x.c * TB - 1);
   };
@@ -478,8 +525,8 @@ __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kern
   const double dtau = a.dtfac * __ldg(a.dt);
   int cnt_acc[5] = {0, 0, 0, 0, 0};
   for (int n = 0; tile < ntiles; tile += G, n++, cur = nxt) {
-    ccur = advance_cnt(ccur);
-    nxt = to_idx(ccur);
+    walk.advance();
+    nxt = walk.idx();
     const int j = d.ng + cur.j, i = d.ng + cur.i;
     const int k0 = d.ng + cur.c * TB;
     const bool live = k0 + t < d.ng + d.n3;
@@ -500,22 +547,7 @@ __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB) update_tma_kern
       fx[6 * v + 2] = ROWZ(26 + 2 * v, 0); fx[6 * v + 3] = ROWZ(27 + 2 * v, 0);
       fx[6 * v + 4] = ROWZ(36 + v, 1);     fx[6 * v + 5] = ROWZ(36 + v, 0);
     }
-    // eq. 21, the expressions of emf_kernel:
-    // E1(j',k') = (F2B3[j'][k'] + F2B3[j'][k'-1] - F3B2[j'][k'] - F3B2[j'-1][k']) / 4
-    ex[0] = 0.25 * (ROWZ(41, 0) + ROWZ(41, -1) - ROWZ(44, 0) - ROWZ(43, 0));  // E1(j, k)
-    ex[1] = 0.25 * (ROWZ(42, 0) + ROWZ(42, -1) - ROWZ(45, 0) - ROWZ(44, 0));  // E1(j+1, k)
-    ex[2] = 0.25 * (ROWZ(41, 1) + ROWZ(41, 0) - ROWZ(44, 1) - ROWZ(43, 1));   // E1(j, k+1)
-    ex[3] = 0.25 * (ROWZ(42, 1) + ROWZ(42, 0) - ROWZ(45, 1) - ROWZ(44, 1));   // E1(j+1, k+1)
-    // E2(i',k') = (F3B1[i'][k'] + F3B1[i'-1][k'] - F1B3[i'][k'] - F1B3[i'][k'-1]) / 4
-    ex[4] = 0.25 * (ROWZ(47, 0) + ROWZ(46, 0) - ROWZ(49, 0) - ROWZ(49, -1));  // E2(i, k)
-    ex[5] = 0.25 * (ROWZ(48, 0) + ROWZ(47, 0) - ROWZ(50, 0) - ROWZ(50, -1));  // E2(i+1, k)
-    ex[6] = 0.25 * (ROWZ(47, 1) + ROWZ(46, 1) - ROWZ(49, 1) - ROWZ(49, 0));   // E2(i, k+1)
-    ex[7] = 0.25 * (ROWZ(48, 1) + ROWZ(47, 1) - ROWZ(50, 1) - ROWZ(50, 0));   // E2(i+1, k+1)
-    // E3(i',j') = (F1B2[i'][j'] + F1B2[i'][j'-1] - F2B1[i'][j'] - F2B1[i'-1][j']) / 4
-    ex[8] = 0.25 * (ROWZ(52, 0) + ROWZ(51, 0) - ROWZ(58, 0) - ROWZ(57, 0));   // E3(i, j)
-    ex[9] = 0.25 * (ROWZ(55, 0) + ROWZ(54, 0) - ROWZ(59, 0) - ROWZ(58, 0));   // E3(i+1, j)
-    ex[10] = 0.25 * (ROWZ(53, 0) + ROWZ(52, 0) - ROWZ(61, 0) - ROWZ(60, 0));  // E3(i, j+1)
-    ex[11] = 0.25 * (ROWZ(56, 0) + ROWZ(55, 0) - ROWZ(62, 0) - ROWZ(61, 0));  // E3(i+1, j+1)
+    edge_emfs(RowStage<UPD_ROW>{z}, ex);  // eq. 21
 #undef ROWZ
     // Every thread now holds its operands: once all have arrived the stage can be refilled.  The barrier is split
     // (arrive here, wait after the divergence arithmetic), so nobody idles while the last warp finishes its reads.

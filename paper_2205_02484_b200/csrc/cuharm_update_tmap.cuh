@@ -1,8 +1,8 @@
 // cuharm_update_tmap.cuh — the fused source + update + inversion + floors kernel (S4-S7, S9) fed by TENSOR-MAP bulk
 // copies (cp.async.bulk.tensor, the TMA engine's tiled mode): the operands of a tile of TB zones are twelve boxes of the
 // 4-D arrays [component][i][j][k] (8-byte elements) instead of 63 one-dimensional row copies, so a tile costs a
-// dozen copy instructions instead of 66.  Same tiles, same strip order, same per-zone arithmetic (update_zone) and the
-// same expression for every edge EMF (eq. 21) as update_tma_kernel: results are bit-identical to it.
+// dozen copy instructions instead of 66.  Same tiles, same strip order (TileWalk), same per-zone arithmetic (update_zone)
+// and the same code for the edge EMFs (edge_emfs) as update_tma_kernel: results are bit-identical to it.
 //
 // Boxes (inner extent TB + 2 zones: k0 - 1 .. k0 + TB; zones past the end of the array are zero-filled by the engine
 // and never used), in the order they sit in shared memory, rows = (component, i, j) combinations of the box:
@@ -49,6 +49,23 @@ __device__ __forceinline__ void tensor_g2s_4d(unsigned dst, const CUtensorMap* m
       : "memory");
 }
 
+// stage layout of update_tmap_kernel for edge_emfs (cuharm_kernels.cuh): box 5 F2(B3) rows j, j+1; box 6 F3(B2) rows j-1,
+// j, j+1; box 7 F3(B1) rows i-1, i, i+1; box 8 F1(B3) rows i, i+1; box 9 F1(B2) rows [i' - i][j' - (j-1)]; box 10 F2(B1)
+// rows [i' - (i-1)][j' - j]; a staged row starts one zone below the tile
+template <int TB>
+struct BoxStage {
+  const unsigned char* stage;
+  int tc;
+  template <int ARR, int A, int B>
+  __device__ __forceinline__ double at() const {
+    constexpr int box = 5 + ARR;
+    constexpr int row = ARR == EMF_F2B3 ? A : ARR == EMF_F3B2 ? A + 1 : ARR == EMF_F3B1 ? A + 1 : ARR == EMF_F1B3 ? A
+                        : ARR == EMF_F1B2 ? 3 * A + (B + 1) : 2 * (A + 1) + B;
+    constexpr int off = ARR == EMF_F1B2 || ARR == EMF_F2B1 ? 0 : B;
+    return reinterpret_cast<const double*>(stage + tmap_off(box, TB))[row * (TB + 2) + 1 + tc + off];
+  }
+};
+
 template <bool SAME, int TB, bool CHAIN>
 __global__ void __launch_bounds__(TB, (UPD_TMA_MINB * 128) / TB)
 update_tmap_kernel(UpdArgs a, const __grid_constant__ UpdMaps maps, const double* __restrict__ rec, int ntiles, int nch, int wj) {
@@ -66,23 +83,8 @@ update_tmap_kernel(UpdArgs a, const __grid_constant__ UpdMaps maps, const double
   }
   __syncthreads();
   int tile = blockIdx.x;
-  // tile order: strips of wj rows j, inside a strip i slower than j, the chunk fastest (as update_tma_kernel)
-  TileCnt ccur, cdlt;
-  {
-    int r = tile;
-    ccur.c = r % nch; r /= nch; ccur.jj = r % wj; r /= wj; ccur.i = r % d.n1; ccur.s = r / d.n1;
-    r = G;
-    cdlt.c = r % nch; r /= nch; cdlt.jj = r % wj; r /= wj; cdlt.i = r % d.n1; cdlt.s = r / d.n1;
-  }
-  auto advance_cnt = [&](const TileCnt& x) {
-    TileCnt y{x.s + cdlt.s, x.i + cdlt.i, x.jj + cdlt.jj, x.c + cdlt.c};
-    if (y.c >= nch) { y.c -= nch; y.jj++; }
-    if (y.jj >= wj) { y.jj -= wj; y.i++; }
-    if (y.i >= d.n1) { y.i -= d.n1; y.s++; }
-    return y;
-  };
-  auto to_idx = [&](const TileCnt& x) { return TileIdx{x.i, x.s * wj + x.jj, x.c}; };
-  TileIdx cur = to_idx(ccur), nxt;
+  TileWalk walk(tile, G, nch, wj, d.n1);  // strip order (cuharm_kernels.cuh)
+  TileIdx cur = walk.idx(), nxt;
   double* const tab = reinterpret_cast<double*>(stage + tmap_off(TMAP_NBOX, TB));  // two slots of 64 doubles
   const unsigned st0 = smem_u32(stage);
   constexpr unsigned TX = (unsigned)((SAME ? 55 : 63) * ROW * 8 + TMAP_REC * 8);
@@ -108,8 +110,8 @@ update_tmap_kernel(UpdArgs a, const __grid_constant__ UpdMaps maps, const double
   const double dtau = a.dtfac * __ldg(a.dt);
   int cnt_acc[5] = {0, 0, 0, 0, 0};
   for (int n = 0; tile < ntiles; tile += G, n++, cur = nxt) {
-    ccur = advance_cnt(ccur);
-    nxt = to_idx(ccur);
+    walk.advance();
+    nxt = walk.idx();
     const int j = d.ng + cur.j, i = d.ng + cur.i;
     const int k0 = d.ng + cur.c * TB;
     const bool live = k0 + t < d.ng + d.n3;
@@ -130,23 +132,7 @@ update_tmap_kernel(UpdArgs a, const __grid_constant__ UpdMaps maps, const double
       fx[6 * v + 2] = BOXZ(3, 2 * v + 1, 0); fx[6 * v + 3] = BOXZ(3, 2 * v, 0);   // F2 at j+1, j
       fx[6 * v + 4] = BOXZ(4, v, 1);         fx[6 * v + 5] = BOXZ(4, v, 0);       // F3 at k+1, k
     }
-    // eq. 21, the expressions (and operand order) of emf_kernel:
-    // E1(j',k') = (F2B3[j'][k'] + F2B3[j'][k'-1] - F3B2[j'][k'] - F3B2[j'-1][k']) / 4     box 5: j, j+1; box 6: j-1, j, j+1
-    ex[0] = 0.25 * (BOXZ(5, 0, 0) + BOXZ(5, 0, -1) - BOXZ(6, 1, 0) - BOXZ(6, 0, 0));  // E1(j, k)
-    ex[1] = 0.25 * (BOXZ(5, 1, 0) + BOXZ(5, 1, -1) - BOXZ(6, 2, 0) - BOXZ(6, 1, 0));  // E1(j+1, k)
-    ex[2] = 0.25 * (BOXZ(5, 0, 1) + BOXZ(5, 0, 0) - BOXZ(6, 1, 1) - BOXZ(6, 0, 1));   // E1(j, k+1)
-    ex[3] = 0.25 * (BOXZ(5, 1, 1) + BOXZ(5, 1, 0) - BOXZ(6, 2, 1) - BOXZ(6, 1, 1));   // E1(j+1, k+1)
-    // E2(i',k') = (F3B1[i'][k'] + F3B1[i'-1][k'] - F1B3[i'][k'] - F1B3[i'][k'-1]) / 4     box 7: i-1, i, i+1; box 8: i, i+1
-    ex[4] = 0.25 * (BOXZ(7, 1, 0) + BOXZ(7, 0, 0) - BOXZ(8, 0, 0) - BOXZ(8, 0, -1));  // E2(i, k)
-    ex[5] = 0.25 * (BOXZ(7, 2, 0) + BOXZ(7, 1, 0) - BOXZ(8, 1, 0) - BOXZ(8, 1, -1));  // E2(i+1, k)
-    ex[6] = 0.25 * (BOXZ(7, 1, 1) + BOXZ(7, 0, 1) - BOXZ(8, 0, 1) - BOXZ(8, 0, 0));   // E2(i, k+1)
-    ex[7] = 0.25 * (BOXZ(7, 2, 1) + BOXZ(7, 1, 1) - BOXZ(8, 1, 1) - BOXZ(8, 1, 0));   // E2(i+1, k+1)
-    // E3(i',j') = (F1B2[i'][j'] + F1B2[i'][j'-1] - F2B1[i'][j'] - F2B1[i'-1][j']) / 4
-    // box 9 rows [i' - i][j' - (j-1)]: 3 (i' - i) + (j' - j + 1);  box 10 rows [i' - (i-1)][j' - j]: 2 (i' - i + 1) + (j' - j)
-    ex[8] = 0.25 * (BOXZ(9, 1, 0) + BOXZ(9, 0, 0) - BOXZ(10, 2, 0) - BOXZ(10, 0, 0));   // E3(i, j)
-    ex[9] = 0.25 * (BOXZ(9, 4, 0) + BOXZ(9, 3, 0) - BOXZ(10, 4, 0) - BOXZ(10, 2, 0));   // E3(i+1, j)
-    ex[10] = 0.25 * (BOXZ(9, 2, 0) + BOXZ(9, 1, 0) - BOXZ(10, 3, 0) - BOXZ(10, 1, 0));  // E3(i, j+1)
-    ex[11] = 0.25 * (BOXZ(9, 5, 0) + BOXZ(9, 4, 0) - BOXZ(10, 5, 0) - BOXZ(10, 3, 0));  // E3(i+1, j+1)
+    edge_emfs(BoxStage<TB>{stage, tc}, ex);  // eq. 21
 #undef BOXZ
     // operands are in registers: release the stage (split barrier: arrive here, wait after the divergence arithmetic)
     mbar_arrive(bar0 + 8);
