@@ -251,7 +251,7 @@ struct ChainArgs {
   const double* floors;
   int* flag;             // in: the 2D method's failure code, or KIND_ENTROPY_FIRST; out: the chain's verdict
   const int* list;
-  const double* ustar;   // [8][nz]: the updated conserved variables U* of every zone, as the update kernel formed them
+  const double* ustar;   // [8][nz]: the updated conserved variables U* of the listed zones, as the update kernel formed them
   const unsigned long long* nfail;
   unsigned long long* nbad;   // zones still failed afterwards
   unsigned long long* stats;  // [8] of cuharm_get_stats

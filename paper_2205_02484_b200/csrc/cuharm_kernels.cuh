@@ -177,8 +177,8 @@ struct UpdArgs {
   double idx1, idx2, idx3, gam;
   NewtonCfg nc;
   FloorCfg fc;
-  ChainCfg cc;    // fallback chain: when on, U* of every zone goes to ustar and the zones of eq. 33 are
-  double* ustar;  // listed without trying the 2D method; chain_kernel then works through the list
+  ChainCfg cc;    // fallback chain: when on, U* of every LISTED zone goes to ustar ([8][nz], written sparsely) and
+  double* ustar;  // the zones of eq. 33 are listed without trying the 2D method; chain_kernel then works through the list
 };
 
 // Per-zone work once the streamed operands are in registers.  pb = P^n, pf = the state the fluxes were built from
@@ -243,10 +243,6 @@ __device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8]
   int its = 0;
   int flag;
   if (CHAIN) {
-    if (live) {
-#pragma unroll
-      for (int v = 0; v < 8; v++) a.ustar[v * d.nz + idx] = U[v];
-    }
     if (ent_first) {
       flag = KIND_ENTROPY_FIRST;
       pn[5] = U[5] * G.isg; pn[6] = U[6] * G.isg; pn[7] = U[7] * G.isg;
@@ -262,6 +258,10 @@ __device__ __forceinline__ void update_zone(const UpdArgs& a, const double pb[8]
   } else if (live) {
     const unsigned long long pos = atomicAdd(a.nfail, 1ull);
     a.list[pos] = (int)idx;
+    if (CHAIN) {  // U* of the LISTED zones only: chain_kernel reads it for no other zone
+#pragma unroll
+      for (int v = 0; v < 8; v++) a.ustar[v * d.nz + idx] = U[v];
+    }
   }
   if (live) {
     a.flag[idx] = flag;
