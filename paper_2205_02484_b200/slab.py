@@ -159,7 +159,8 @@ class SlabGroup:
 class SlabRank:
     """One rank of a torch.distributed job: the same sequence with isend / irecv to the neighbouring ranks.
 
-    `engine.prim` / `engine.half` must be torch tensors (CUDA with the NCCL backend, CPU with gloo)."""
+    `engine.prim` / `engine.half` must be torch tensors: CUDA with the NCCL backend; CPU or CUDA with gloo (CUDA arrays are
+    then staged through pinned host buffers -- the way to run the library under this class where NCCL has one GPU only)."""
 
     def __init__(self, engine, p: dict, rank: int, world: int, group=None):
         import torch.distributed as dist
@@ -168,6 +169,9 @@ class SlabRank:
         self.n1 = slab_ranges(p["n1"], world)[rank][1]
         self.lo, self.hi = neighbours(p, world, rank)
         self._bufs = {}     # halo send / receive buffers by (device, layout)
+        # gloo moves host memory only: with that backend and arrays on a GPU the packed halo buffers live in pinned host
+        # memory and the planes are copied device -> host -> (gloo) -> host -> device.  With NCCL they stay on the device.
+        self.stage_host = dist.get_backend(group) == "gloo"
 
     def _exchange(self, arr, flags=None):
         """Halo planes of `arr` (and, when given, of the flag array) to and from both neighbours: ONE message per neighbour
@@ -181,7 +185,10 @@ class SlabRank:
         key = (str(arr.device), tuple(sizes))                                 # every part starts on a multiple of 8 bytes
         buf = self._bufs.get(key)
         if buf is None:
-            buf = [torch.empty(sum(sizes), dtype=torch.uint8, device=arr.device) for _ in range(4)]
+            if self.stage_host and arr.is_cuda:
+                buf = [torch.empty(sum(sizes), dtype=torch.uint8, device="cpu").pin_memory() for _ in range(4)]
+            else:
+                buf = [torch.empty(sum(sizes), dtype=torch.uint8, device=arr.device) for _ in range(4)]
             self._bufs[key] = buf
         send_lo, send_hi, recv_lo, recv_hi = buf
 
@@ -217,9 +224,12 @@ class SlabRank:
             for src, dst in pieces(recv_lo, 2):
                 dst.copy_(src)
 
+    def _scalar_device(self):
+        return "cpu" if self.stage_host else self.engine.prim.device
+
     def _allsum(self, a, b):
         import torch
-        t = torch.tensor([a, b], dtype=torch.int64, device=self.engine.prim.device)
+        t = torch.tensor([a, b], dtype=torch.int64, device=self._scalar_device())
         if self.world > 1:
             self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM, group=self.group)
         return int(t[0]), int(t[1])
@@ -248,7 +258,7 @@ class SlabRank:
 
     def _allmax(self, cw):
         import torch
-        t = torch.tensor(list(cw), dtype=torch.float64, device=self.engine.prim.device)
+        t = torch.tensor(list(cw), dtype=torch.float64, device=self._scalar_device())
         if self.world > 1:
             self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX, group=self.group)
         return [float(x) for x in t.cpu()]

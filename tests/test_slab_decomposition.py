@@ -258,3 +258,67 @@ def test_gpu_slabs_match_the_single_domain_run_and_the_oracle(name, kw, nslabs):
     for _ in range(2):
         s2.set_dt(dt); s2.substep(0); s2.substep(1)
     assert np.array_equal(s2.prim.cpu().numpy(), one)
+
+
+# ------------------------------------------------------------------ GPU: the library under SlabRank, two ranks on one device
+def _gpu_rank_main(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import torch
+    import torch.distributed as dist
+    import paper_2205_02484_b200 as cu
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    torch.cuda.set_device(0)
+    p, prim0 = torus_case("C4", n1=30, n2=16, n3=40)
+    eng = cu.Solver(slab.slab_params(p, world, rank), np.ascontiguousarray(prim0[:, slab.slab_slice(p, world, rank)]))
+    me = slab.SlabRank(eng, p, rank, world)
+    dt = me.cfl_dt(0.45)
+    for _ in range(2):
+        me.step(dt)
+    q.put((rank, dt, me.last_cfl_dt(0.45), eng.prim.cpu().numpy().copy(), eng.stats()[2]))
+    dist.barrier()
+    eng.close()
+    dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_gpu_library_under_slabrank_two_ranks_on_one_device():
+    """slab.SlabRank -- the torch.distributed sequencing a multi-GPU run would use -- with the LIBRARY as its
+    engine: two processes, both on cuda:0, halo planes and flags moved over gloo through pinned host buffers (the box has
+    one GPU, so NCCL cannot pair two ranks here; the kernels of the two ranks never wait on one another, the host
+    sequences them).  Against the library's single-domain run (round-off: the marching kernels restart their
+    reconstruction at extent-dependent segment boundaries) and against the oracle."""
+    torch = pytest.importorskip("torch")
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import torch.multiprocessing as mp
+    import paper_2205_02484_b200 as cu
+    from test_gpu_parity import prim_errors
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 35500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_gpu_rank_main, args=(r, 2, port, q)) for r in range(2)]
+    for pr in procs:
+        pr.start()
+    res = sorted((q.get(timeout=600) for _ in procs), key=lambda t: t[0])
+    for pr in procs:
+        pr.join(timeout=120)
+        assert pr.exitcode == 0
+    p, prim0 = torus_case("C4", n1=30, n2=16, n3=40)
+    ref, dt, dt_next = single_domain(p, prim0, 2)
+    s = cu.Solver(p, prim0)
+    for _ in range(2):
+        s.step(dt)
+    one = s.prim.cpu().numpy()
+    ng = p["ng"]
+    assert res[0][1] == res[1][1] and abs(res[0][1] / dt - 1.0) < 1e-13
+    assert res[0][2] == res[1][2] and abs(res[0][2] / dt_next - 1.0) < 1e-13
+    got = np.concatenate([res[0][3][:, :ng + 15], res[1][3][:, ng:]], axis=1)
+    assert (prim_errors(p, got, one, whole=True, tol=1e-12) < 1e-12).all(), prim_errors(p, got, one, whole=True, tol=1e-12)
+    assert (prim_errors(p, got, ref, whole=True) < 2e-11).all(), prim_errors(p, got, ref, whole=True)
+    assert res[0][4] + res[1][4] == s.stats()[2]
+    # each rank's halo planes are its neighbour's interior planes
+    assert np.array_equal(res[0][3][:, ng + 15:], res[1][3][:, ng:2 * ng])
+    assert np.array_equal(res[1][3][:, :ng], res[0][3][:, 15:15 + ng])
+    s.close()
