@@ -576,7 +576,7 @@ def run_chain_cost(args):
         return out
 
     rows = []
-    for bscale in (1.0, 30.0, 100.0, 300.0, 1000.0):
+    for bscale in ((args.chain_bscale,) if args.chain_bscale > 0 else (1.0, 30.0, 100.0, 300.0, 1000.0)):
         prim = prim_host.copy()
         prim[5:8] *= bscale
         on = run(dict(p0, inv_chain=1, beta_min=args.beta_min), prim, 3)
@@ -632,6 +632,7 @@ def main():
     ap.add_argument("--chain", action="store_true", help="cost of the inversion fallback chain on a magnetised state")
     ap.add_argument("--chain-frac", type=float, default=0.05, help="--chain: scale B until this fraction of zones are eq. 33 zones")
     ap.add_argument("--beta-min", type=float, default=1e-2, help="--chain: eq. 33 threshold")
+    ap.add_argument("--chain-bscale", type=float, default=0.0, help="--chain: use this field scale instead of searching for one")
     ap.add_argument("--fp64-peak", action="store_true", help="run the DFMA micro-benchmark (bench_fp64_peak.cu) and exit")
     args = ap.parse_args()
     if args.fp64_peak:

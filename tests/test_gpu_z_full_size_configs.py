@@ -173,3 +173,31 @@ def test_c2_as_written_three_resolutions_to_t50_and_the_oracle_at_64():
     order0 = np.log2(errs[0] / errs[1])
     print(f"Michel flow, a = 0, to t = 50 M: L1 error vs the exact steady state 64^2 {errs[0]}, 128^2 {errs[1]}, order {order0}")
     assert (order0 > 1.7).all(), (errs, order0)
+
+
+# ------------------------------------------------------------------ the fallback chain at the headline size
+def test_c4_full_size_one_step_with_the_fallback_chain_busy():
+    """256^3 with inv_chain = 1, beta_min = 1e-2 (eq. 33) and the torus field scaled x100, so that about 3 % of
+    the zones (half a million per substep) take the entropy method: chain counters equal, every zone against the oracle to
+    the tolerance of the small chain cases (1e-10: Brent's 1e-14 times the conditioning of the recovery)."""
+    p = config("C4", inv_chain=1, beta_min=1e-2)
+    prim0, _ = fm_torus(p, **TORUS["C4"])
+    prim0[5:8] *= 100.0
+    ref = prim0.copy()
+    g = oracle.Grid(p)
+    g.bind(ref)
+    dt = g.cfl_dt(0.45)
+    s = cu.Solver(p, torch.from_numpy(prim0))
+    s.use_graph(True)
+    g.step(dt)
+    s.step(dt)
+    cs, cr = s.chain_stats(), [int(x) for x in g.get_chain_stats()]
+    print(f"C4 256^3, chain on, field x100: chain counters library {cs}, oracle {cr}")
+    assert cs == cr and cr[3] > 2e5, (cs, cr)
+    st, so = list(s.stats()), [int(x) for x in g.get_stats()]
+    assert st[:6] == so[:6] and st[7] == so[7], (st, so)
+    err = prim_errors(p, s.prim.cpu().numpy(), ref, whole=True, tol=1e-10)
+    print(f"max parity error per primitive {err}")
+    assert (err < 1e-10).all(), err
+    assert s.divb()[1] < 1e-12 and g.divb()[1] < 1e-12
+    s.close()
